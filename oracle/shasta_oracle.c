@@ -1,0 +1,465 @@
+/*
+ * shasta_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, obviously-correct fp64 CPU implementation of the dimensionally
+ * split (3+1)D relativistic SHASTA time step of arXiv:1206.0919,
+ * written straight from the paper's equations, in the paper's order and notation.
+ * It shares no code with the CUDA path (paper_1206_0919_b200/csrc) and must not:
+ * only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may load it.  Build: gcc -O2 -ffp-contract=off -fopenmp -shared.
+ * (-ffp-contract=off: no FMA contraction, so the identities the pins test hold as
+ * stated.  OpenMP is used ONLY over independent pencils/cells: the result is
+ * bitwise identical for any thread count; oracle_set_threads(1) = single thread.)
+ *
+ * What follows the paper (citations are PAPER.md line numbers):
+ *   eqs. (9)-(11)   PAPER.md:58-62    conserved fields from primitives
+ *   eq.  (15)       PAPER.md:83       geometric factors Q+-
+ *   source term     PAPER.md:88       Delta(f) = -1/2 (f_{j+1} - f_{j-1}), f = p (M par.), p v (E)
+ *   eqs. (16),(17)  PAPER.md:90-93    transport + diffusion
+ *   eqs. (18)-(22)  PAPER.md:97-107   phoenical antidiffusion, flux limiter, update
+ *   four phases     PAPER.md:74-79    transport / antidiffusion / relativistic correction / EOS
+ *   half step       PAPER.md:161      "implemented based on a half-step method"
+ *   fixed point     PAPER.md:109      velocity by fixed-point root finding
+ *   axis table      PAPER.md:295-297  branch[] = {0,1,2,0,2,1,2,0,1,2,1,0,1,2,0,1,0,2}
+ *
+ * Where the paper is silent the readings G1-G19 of SURVEY.md 8(c.2), restated in
+ * DESIGN.md section 3, are used; each is marked "reading Gn" below.
+ *
+ * PARITY PINS (tests/test_oracle_*.py, -m "not gpu"): P1-P13 of DESIGN.md section 4.
+ * "parity unpinned" AGAINST THE PAPER'S OWN CODE for: the predictor without
+ * antidiffusion (reading G4), the causality projection Pi and its write-back
+ * (G6-G8) and the ghost-extension boundary rule (G11): the paper prints no value
+ * and no code for them; they are pinned only by self-consistency and by
+ * convergence to the exact Riemann solution.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define NF 5          /* E, Mx, My, Mz, R  (R is the paper's N, eq. (9)) */
+#define G  4          /* ghost depth of one sweep: dependency radius */
+#define PI_DELTA 1e-12            /* reading G7 */
+#define FP_TOL   1e-15            /* reading G9 */
+#define FP_MAXIT 200              /* reading G9 */
+
+enum { BC_OUTFLOW = 0, BC_PERIODIC = 1 };
+
+typedef struct oracle_shasta {
+    int nx, ny, nz;
+    double dx, lambda, gamma, mass;
+    int bc;
+    long long step_index;
+    int table[64];
+    int ntable;
+    double *U[NF];                /* conserved state, x fastest: ix + nx*(iy + ny*iz) */
+    int have_state;
+    unsigned long long counts[4]; /* Pi fired, vacuum cells, e<0 floored, p<0 floored */
+} oracle_t;
+
+static int g_threads = 1;
+void oracle_set_threads(int n) { g_threads = n < 1 ? 1 : n; }
+int oracle_get_threads(void) { return g_threads; }
+
+/* ---------------------------------------------------------------- EOS ---- */
+/* ideal gas, reading G10: P(e,n) = max((Gamma-1)(e - m n), 0) */
+static double eos_P(double e, double n, double gamma, double mass)
+{
+    double p = (gamma - 1.0) * (e - mass * n);
+    return p > 0.0 ? p : 0.0;
+}
+
+/* --------------------------------------------- eqs. (9)-(11): prim -> cons */
+void oracle_prim2cons(double e, double n, double vx, double vy, double vz,
+                      double gamma, double mass, double out[NF])
+{
+    double p = eos_P(e, n, gamma, mass);
+    double v2 = (vx * vx + vy * vy) + vz * vz;
+    double g2 = 1.0 / (1.0 - v2);             /* gamma_L^2 */
+    double w = (e + p) * g2;                  /* (eps + p) gamma^2 */
+    out[0] = w - p;                           /* eq. (11): (eps + p v^2) gamma^2 = w - p */
+    out[1] = w * vx;                          /* eq. (10) */
+    out[2] = w * vy;
+    out[3] = w * vz;
+    out[4] = n * sqrt(g2);                    /* eq. (9) */
+}
+
+/* ------------------- phases 3+4: relativistic correction + EOS (cons2prim) */
+/* Pi, readings G6-G8: enforce |M| <= (1-delta) E; vacuum if !(E > 0).
+   Returns 1 if the projection fired, 2 if vacuum, 0 otherwise.  E, R untouched. */
+int oracle_project(double E, double M[3])
+{
+    if (!(E > 0.0)) { M[0] = M[1] = M[2] = 0.0; return 2; }
+    double Mabs = sqrt((M[0] * M[0] + M[1] * M[1]) + M[2] * M[2]);
+    double lim = (1.0 - PI_DELTA) * E;
+    if (Mabs > lim) {
+        double s = lim / Mabs;
+        M[0] *= s; M[1] *= s; M[2] *= s;
+        return 1;
+    }
+    return 0;
+}
+
+/* out = {e, p, n, vx, vy, vz, |v|}; returns the number of fixed-point iterations.
+   flags (may be NULL): flags[0] += e floored, flags[1] += p floored. */
+int oracle_cons2prim(double E, double Mx, double My, double Mz, double R,
+                     double gamma, double mass, double out[7], int flags[2])
+{
+    double M = sqrt((Mx * Mx + My * My) + Mz * Mz);
+    if (!(E > 0.0)) {                         /* vacuum, reading G7 */
+        for (int i = 0; i < 7; ++i) out[i] = 0.0;
+        return 0;
+    }
+    double lim = (1.0 - PI_DELTA) * E;
+    double Mc = M < lim ? M : lim;            /* same rule as Pi */
+    double v = 0.0;
+    int it = 0;
+    for (it = 0; it < FP_MAXIT; ++it) {       /* PAPER.md:109 fixed point, reading G9 */
+        double P = eos_P(E - Mc * v, R * sqrt(1.0 - v * v), gamma, mass);
+        double vnew = Mc / (E + P);
+        double d = fabs(vnew - v);
+        v = vnew;
+        if (d <= FP_TOL) { ++it; break; }
+    }
+    double e = E - Mc * v;
+    if (e < 0.0) { e = 0.0; if (flags) flags[0]++; }
+    double n = R * sqrt(1.0 - v * v);
+    double praw = (gamma - 1.0) * (e - mass * n);
+    if (praw < 0.0 && flags) flags[1]++;
+    double p = eos_P(e, n, gamma, mass);
+    out[0] = e; out[1] = p; out[2] = n;
+    if (M > 0.0) { out[3] = v * Mx / M; out[4] = v * My / M; out[5] = v * Mz / M; }
+    else         { out[3] = out[4] = out[5] = 0.0; }
+    out[6] = v;
+    return it;
+}
+
+/* ------------------------------------------------------------ eq. (15) --- */
+/* reading G1: upper signs -> Q+, lower signs -> Q-.  eps = lambda * v. */
+double oracle_qplus(double eps_j, double eps_jp1)
+{
+    return (0.5 - eps_j) / (1.0 + (eps_jp1 - eps_j));
+}
+double oracle_qminus(double eps_j, double eps_jm1)
+{
+    return (0.5 + eps_j) / (1.0 - (eps_jm1 - eps_j));
+}
+
+/* ------------------------------------------------- eqs. (16),(17) -------- */
+/* Transport + diffusion of ONE field on an extended pencil.
+   Arrays are indexed 0..n-1; Uhat[j] is written for j = lo..hi-1 and needs
+   U, eps, f at j-1..j+1.  f may be NULL (source-free field).  lam multiplies
+   Delta(f) = -1/2 (f[j+1] - f[j-1]). */
+void oracle_transport(int n, const double *U, const double *eps, const double *f,
+                      double lam, double *Uhat, int lo, int hi)
+{
+    (void)n;
+    for (int j = lo; j < hi; ++j) {
+        double Qp = oracle_qplus(eps[j], eps[j + 1]);
+        double Qm = oracle_qminus(eps[j], eps[j - 1]);
+        double Dj = U[j + 1] - U[j];                         /* eq. (16) */
+        double Djm = U[j] - U[j - 1];
+        double uh = 0.5 * Qp * Qp * Dj - 0.5 * Qm * Qm * Djm + (Qp + Qm) * U[j];
+        if (f) uh += lam * (-0.5 * (f[j + 1] - f[j - 1]));   /* + lambda Delta(f) */
+        Uhat[j] = uh;                                        /* eq. (17) */
+    }
+}
+
+/* ------------------------------------------------- eqs. (18)-(22) -------- */
+static double sgn(double x) { return (x > 0.0) - (x < 0.0); }
+static double min3(double a, double b, double c)
+{
+    double m = a < b ? a : b;
+    return m < c ? m : c;
+}
+/* Phoenical antidiffusion with flux limiter on ONE field of an extended pencil.
+   Unew[j] is written for j = lo..hi-1; needs Uhat at j-2..j+2 and U at j-3..j+3
+   (Fig. 3).  diff multiplies A^ph (Listing 1 'diff', reading G13). */
+void oracle_antidiffuse(int n, const double *U, const double *Uhat, double diff,
+                        double *Unew, int lo, int hi)
+{
+    (void)n;
+    for (int j = lo; j < hi; ++j) {
+        double A[2];                                        /* A_{j-1}, A_j */
+        for (int k = 0; k < 2; ++k) {
+            int i = j - 1 + k;                              /* interface index */
+            double Dh = Uhat[i + 1] - Uhat[i];              /* eq. (18) */
+            double Dhp = Uhat[i + 2] - Uhat[i + 1];
+            double Dhm = Uhat[i] - Uhat[i - 1];
+            double Di = U[i + 1] - U[i];                    /* eq. (16) */
+            double Dip = U[i + 2] - U[i + 1];
+            double Dim = U[i] - U[i - 1];
+            /* eq. (19), evaluation order of reading G14 */
+            double Aph = diff * (0.125 * (Dh - 0.125 * ((Dip + Dim) - 2.0 * Di)));
+            double s = sgn(Aph);                            /* eq. (20) */
+            double m = min3(s * Dhp, fabs(Aph), s * Dhm);
+            A[k] = s * (m > 0.0 ? m : 0.0);                 /* eq. (21) */
+        }
+        Unew[j] = Uhat[j] - A[1] + A[0];                    /* eq. (22) */
+    }
+}
+
+/* ------------------------------------------------------------ boundary --- */
+/* reading G11: ghost-extend the INPUT of a sweep by G cells per side. */
+static int ghost_index(int j, int N, int bc)
+{
+    if (bc == BC_PERIODIC) { int m = j % N; return m < 0 ? m + N : m; }
+    return j < 0 ? 0 : (j >= N ? N - 1 : j);
+}
+
+/* ---------------------------------------------------------- one pencil --- */
+/* One full sweep (phases 1-4) of one pencil along axis a (0=x,1=y,2=z).
+   U[f][0..N-1] is updated in place.  counts (may be NULL): [0] Pi fired, [1] vacuum. */
+void oracle_sweep_pencil(int N, double *U[NF], int a, double lambda, double gamma,
+                         double mass, int bc, unsigned long long counts[2])
+{
+    const int NE = N + 2 * G;                 /* extended length, j = -G .. N+G-1 at offset +G */
+    double *buf = (double *)malloc(sizeof(double) * (size_t)NE * (4 * NF + 8));
+    double *Ue[NF], *Ut[NF], *Uh[NF], *Un[NF];
+    double *p = buf;
+    for (int f = 0; f < NF; ++f) { Ue[f] = p; p += NE; }
+    for (int f = 0; f < NF; ++f) { Ut[f] = p; p += NE; }
+    for (int f = 0; f < NF; ++f) { Uh[f] = p; p += NE; }
+    for (int f = 0; f < NF; ++f) { Un[f] = p; p += NE; }
+    double *v = p;  p += NE;  double *pr = p; p += NE;  double *pv = p; p += NE;
+    double *eps = p; p += NE; double *vh = p; p += NE;  double *ph = p; p += NE;
+    double *pvh = p; p += NE; double *epsh = p; p += NE;
+
+    /* 1. extend j = -4 .. N+3 */
+    for (int i = 0; i < NE; ++i) {
+        int src = ghost_index(i - G, N, bc);
+        for (int f = 0; f < NF; ++f) Ue[f][i] = U[f][src];
+    }
+    /* 2. time-n primitives, j = -4 .. N+3 */
+    for (int i = 0; i < NE; ++i) {
+        double o[7];
+        oracle_cons2prim(Ue[0][i], Ue[1][i], Ue[2][i], Ue[3][i], Ue[4][i], gamma, mass, o, NULL);
+        v[i] = o[3 + a]; pr[i] = o[1]; pv[i] = o[1] * o[3 + a];
+    }
+    /* 3. predictor (readings G4, G5): eq. (17) with lambda/2, time-n v and p, no antidiffusion;
+          j = -3 .. N+2 */
+    const double h = 0.5 * lambda;
+    for (int i = 0; i < NE; ++i) eps[i] = h * v[i];
+    for (int f = 0; f < NF; ++f) {
+        const double *src = (f == 0) ? pv : (f == 1 + a ? pr : NULL);
+        oracle_transport(NE, Ue[f], eps, src, h, Ut[f], 1, NE - 1);
+    }
+    /* 4. half-step primitives, j = -3 .. N+2 */
+    for (int i = 1; i < NE - 1; ++i) {
+        double o[7];
+        oracle_cons2prim(Ut[0][i], Ut[1][i], Ut[2][i], Ut[3][i], Ut[4][i], gamma, mass, o, NULL);
+        vh[i] = o[3 + a]; ph[i] = o[1]; pvh[i] = o[1] * o[3 + a];
+    }
+    /* 5. corrector transport: eq. (17) with lambda, half-step v and p, transports U^n;
+          j = -2 .. N+1 */
+    for (int i = 1; i < NE - 1; ++i) epsh[i] = lambda * vh[i];
+    for (int f = 0; f < NF; ++f) {
+        const double *src = (f == 0) ? pvh : (f == 1 + a ? ph : NULL);
+        oracle_transport(NE, Ue[f], epsh, src, lambda, Uh[f], 2, NE - 2);
+    }
+    /* 6.+7. antidiffusion, limiter, update: j = 0 .. N-1 */
+    for (int f = 0; f < NF; ++f)
+        oracle_antidiffuse(NE, Ue[f], Uh[f], 1.0, Un[f], G, G + N);
+    /* 8. relativistic correction Pi written back (reading G8) */
+    for (int j = 0; j < N; ++j) {
+        double M[3] = { Un[1][G + j], Un[2][G + j], Un[3][G + j] };
+        int r = oracle_project(Un[0][G + j], M);
+        if (counts) { if (r == 1) counts[0]++; else if (r == 2) counts[1]++; }
+        U[0][j] = Un[0][G + j];
+        U[1][j] = M[0]; U[2][j] = M[1]; U[3][j] = M[2];
+        U[4][j] = Un[4][G + j];
+    }
+    free(buf);
+}
+
+/* P5 pin helper: advect ONE source-free field with a PRESCRIBED velocity (cons2prim
+   bypassed): v_half = v, one step = corrector transport + antidiffusion (eqs. 15-22). */
+void oracle_advect_pencil(int N, double *U, const double *vel, double lambda, int bc,
+                          int nsteps, double *Uhat_out)
+{
+    const int NE = N + 2 * G;
+    double *Ue = (double *)malloc(sizeof(double) * (size_t)NE * 4);
+    double *eps = Ue + NE, *Uh = eps + NE, *Un = Uh + NE;
+    for (int s = 0; s < nsteps; ++s) {
+        for (int i = 0; i < NE; ++i) {
+            int src = ghost_index(i - G, N, bc);
+            Ue[i] = U[src]; eps[i] = lambda * vel[src];
+        }
+        oracle_transport(NE, Ue, eps, NULL, lambda, Uh, 2, NE - 2);
+        oracle_antidiffuse(NE, Ue, Uh, 1.0, Un, G, G + N);
+        for (int j = 0; j < N; ++j) U[j] = Un[G + j];
+        if (Uhat_out) for (int j = 0; j < N; ++j) Uhat_out[j] = Uh[G + j];
+    }
+    free(Ue);
+}
+
+/* ---------------------------------------------------------- the grid ----- */
+static const int kBranch[18] = { 0,1,2, 0,2,1, 2,0,1, 2,1,0, 1,2,0, 1,0,2 };
+
+oracle_t *oracle_create(int nx, int ny, int nz, double dx, double lambda, double eos_gamma)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(lambda > 0.0) || lambda > 0.5 ||
+        !(eos_gamma > 1.0)) return NULL;
+    oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
+    o->nx = nx; o->ny = ny; o->nz = nz; o->dx = dx; o->lambda = lambda; o->gamma = eos_gamma;
+    o->mass = 0.0; o->bc = BC_OUTFLOW; o->step_index = 0;
+    memcpy(o->table, kBranch, sizeof(kBranch)); o->ntable = 18;
+    size_t n = (size_t)nx * ny * nz;
+    for (int f = 0; f < NF; ++f) o->U[f] = (double *)calloc(n, sizeof(double));
+    return o;
+}
+void oracle_destroy(oracle_t *o)
+{
+    if (!o) return;
+    for (int f = 0; f < NF; ++f) free(o->U[f]);
+    free(o);
+}
+/* keys: 0 boundary (0 outflow, 1 periodic), 1 EOS mass m, 3 step index */
+int oracle_set_option(oracle_t *o, int key, double value)
+{
+    if (!o) return -1;
+    switch (key) {
+    case 0: if (value != 0.0 && value != 1.0) return -1; o->bc = (int)value; return 0;
+    case 1: if (value < 0.0) return -1; o->mass = value; return 0;
+    case 3: if (value < 0.0) return -1; o->step_index = (long long)value; return 0;
+    default: return -1;
+    }
+}
+int oracle_set_sweep_table(oracle_t *o, const int *axes, int n)
+{
+    if (!o || !axes || n < 3 || n > 63 || n % 3) return -1;
+    for (int i = 0; i < n; ++i) if (axes[i] < 0 || axes[i] > 2) return -1;
+    memcpy(o->table, axes, sizeof(int) * (size_t)n); o->ntable = n;
+    return 0;
+}
+int oracle_set_state(oracle_t *o, const double *e, const double *n, const double *vx,
+                     const double *vy, const double *vz)
+{
+    if (!o || !e || !n || !vx || !vy || !vz) return -1;
+    long long nc = (long long)o->nx * o->ny * o->nz;
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+    for (long long i = 0; i < nc; ++i) {
+        double c[NF];
+        oracle_prim2cons(e[i], n[i], vx[i], vy[i], vz[i], o->gamma, o->mass, c);
+        for (int f = 0; f < NF; ++f) o->U[f][i] = c[f];
+    }
+    o->have_state = 1;
+    return 0;
+}
+int oracle_set_conserved(oracle_t *o, const double *E, const double *Mx, const double *My,
+                         const double *Mz, const double *R)
+{
+    if (!o || !E || !Mx || !My || !Mz || !R) return -1;
+    size_t nb = sizeof(double) * (size_t)o->nx * o->ny * o->nz;
+    const double *src[NF] = { E, Mx, My, Mz, R };
+    for (int f = 0; f < NF; ++f) memcpy(o->U[f], src[f], nb);
+    o->have_state = 1;
+    return 0;
+}
+int oracle_get_conserved(oracle_t *o, double *E, double *Mx, double *My, double *Mz, double *R)
+{
+    if (!o) return -1;
+    if (!o->have_state) return -4;
+    size_t nb = sizeof(double) * (size_t)o->nx * o->ny * o->nz;
+    double *dst[NF] = { E, Mx, My, Mz, R };
+    for (int f = 0; f < NF; ++f) if (dst[f]) memcpy(dst[f], o->U[f], nb);
+    return 0;
+}
+
+/* one sweep of the whole grid along axis a: every pencil independently */
+static void sweep_grid(oracle_t *o, int a)
+{
+    const int n[3] = { o->nx, o->ny, o->nz };
+    const long long stride[3] = { 1, o->nx, (long long)o->nx * o->ny };
+    const int N = n[a];
+    const int b = (a + 1) % 3, c = (a + 2) % 3;      /* the two other axes */
+    const long long npencil = (long long)n[b] * n[c];
+    unsigned long long c0 = 0, c1 = 0;
+#pragma omp parallel for num_threads(g_threads) schedule(static) reduction(+:c0,c1)
+    for (long long q = 0; q < npencil; ++q) {
+        long long ib = q % n[b], ic = q / n[b];
+        long long base = ib * stride[b] + ic * stride[c];
+        double *pen = (double *)malloc(sizeof(double) * (size_t)N * NF);
+        double *P[NF];
+        for (int f = 0; f < NF; ++f) {
+            P[f] = pen + (size_t)f * N;
+            for (int j = 0; j < N; ++j) P[f][j] = o->U[f][base + j * stride[a]];
+        }
+        unsigned long long cnt[2] = { 0, 0 };
+        oracle_sweep_pencil(N, P, a, o->lambda, o->gamma, o->mass, o->bc, cnt);
+        for (int f = 0; f < NF; ++f)
+            for (int j = 0; j < N; ++j) o->U[f][base + j * stride[a]] = P[f][j];
+        c0 += cnt[0]; c1 += cnt[1];
+        free(pen);
+    }
+    o->counts[0] += c0; o->counts[1] += c1;
+}
+
+/* one time step dt = lambda dx = three sweeps (reading G3), order from the table */
+int oracle_step(oracle_t *o, int nsteps)
+{
+    if (!o || nsteps < 0) return -1;
+    if (!o->have_state) return -4;
+    const int n[3] = { o->nx, o->ny, o->nz };
+    for (int s = 0; s < nsteps; ++s) {
+        for (int k = 0; k < 3; ++k) {
+            int a = o->table[(3 * o->step_index + k) % o->ntable];
+            if (n[a] == 1) continue;                 /* reading G15 */
+            sweep_grid(o, a);
+        }
+        o->step_index++;
+    }
+    return 0;
+}
+
+int oracle_get_primitives(oracle_t *o, double *e, double *p, double *n, double *vx,
+                          double *vy, double *vz)
+{
+    if (!o) return -1;
+    if (!o->have_state) return -4;
+    long long nc = (long long)o->nx * o->ny * o->nz;
+    unsigned long long f0 = 0, f1 = 0;
+#pragma omp parallel for num_threads(g_threads) schedule(static) reduction(+:f0,f1)
+    for (long long i = 0; i < nc; ++i) {
+        double out[7]; int fl[2] = { 0, 0 };
+        oracle_cons2prim(o->U[0][i], o->U[1][i], o->U[2][i], o->U[3][i], o->U[4][i],
+                         o->gamma, o->mass, out, fl);
+        if (e) e[i] = out[0];
+        if (p) p[i] = out[1];
+        if (n) n[i] = out[2];
+        if (vx) vx[i] = out[3];
+        if (vy) vy[i] = out[4];
+        if (vz) vz[i] = out[5];
+        f0 += (unsigned)fl[0]; f1 += (unsigned)fl[1];
+    }
+    o->counts[2] += f0; o->counts[3] += f1;
+    return 0;
+}
+
+/* dx^3 * sum over cells, Neumaier-compensated (eqs. (12)-(14): the totals are conserved) */
+int oracle_conserved_totals(oracle_t *o, double totals[NF])
+{
+    if (!o || !totals) return -1;
+    if (!o->have_state) return -4;
+    long long nc = (long long)o->nx * o->ny * o->nz;
+    double dv = o->dx * o->dx * o->dx;
+    for (int f = 0; f < NF; ++f) {
+        double s = 0.0, c = 0.0;
+        for (long long i = 0; i < nc; ++i) {
+            double x = o->U[f][i], t = s + x;
+            if (fabs(s) >= fabs(x)) c += (s - t) + x; else c += (x - t) + s;
+            s = t;
+        }
+        totals[f] = dv * (s + c);
+    }
+    return 0;
+}
+int oracle_diagnostics(oracle_t *o, unsigned long long counts[4])
+{
+    if (!o || !counts) return -1;
+    for (int i = 0; i < 4; ++i) counts[i] = o->counts[i];
+    return 0;
+}
+long long oracle_step_index(oracle_t *o) { return o ? o->step_index : -1; }

@@ -1,0 +1,221 @@
+"""ctypes wrapper around oracle/shasta_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this module.  It shares nothing with paper_1206_0919_b200 (the CUDA path).
+All pointers are HOST pointers (numpy float64, C-contiguous, shape (nz, ny, nx), x fastest).
+See shasta_oracle.c for the citations into PAPER.md.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "shasta_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_shasta.so")
+
+BOUNDARY, EOS_MASS, STEP_INDEX = 0, 1, 3
+OUTFLOW, PERIODIC = 0, 1
+BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off -fopenmp: plain C, no FMA contraction."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c11",
+               "-Wall", "-Wextra", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.oracle_create.restype = C.c_void_p
+        L.oracle_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]
+        L.oracle_destroy.argtypes = [C.c_void_p]
+        L.oracle_set_option.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.oracle_set_sweep_table.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_int]
+        L.oracle_set_state.argtypes = [C.c_void_p] + [_dp] * 5
+        L.oracle_set_conserved.argtypes = [C.c_void_p] + [_dp] * 5
+        L.oracle_get_conserved.argtypes = [C.c_void_p] + [_dp] * 5
+        L.oracle_get_primitives.argtypes = [C.c_void_p] + [_dp] * 6
+        L.oracle_step.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_conserved_totals.argtypes = [C.c_void_p, _dp]
+        L.oracle_diagnostics.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong)]
+        L.oracle_step_index.restype = C.c_longlong
+        L.oracle_step_index.argtypes = [C.c_void_p]
+        L.oracle_set_threads.argtypes = [C.c_int]
+        L.oracle_get_threads.restype = C.c_int
+        L.oracle_qplus.restype = C.c_double
+        L.oracle_qplus.argtypes = [C.c_double, C.c_double]
+        L.oracle_qminus.restype = C.c_double
+        L.oracle_qminus.argtypes = [C.c_double, C.c_double]
+        L.oracle_transport.argtypes = [C.c_int, _dp, _dp, _dp, C.c_double, _dp, C.c_int, C.c_int]
+        L.oracle_antidiffuse.argtypes = [C.c_int, _dp, _dp, C.c_double, _dp, C.c_int, C.c_int]
+        L.oracle_prim2cons.argtypes = [C.c_double] * 7 + [_dp]
+        L.oracle_cons2prim.restype = C.c_int
+        L.oracle_cons2prim.argtypes = [C.c_double] * 7 + [_dp, C.POINTER(C.c_int)]
+        L.oracle_project.restype = C.c_int
+        L.oracle_project.argtypes = [C.c_double, _dp]
+        L.oracle_sweep_pencil.argtypes = [C.c_int, C.POINTER(_dp), C.c_int, C.c_double, C.c_double,
+                                          C.c_double, C.c_int, C.POINTER(C.c_ulonglong)]
+        L.oracle_advect_pencil.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_int, C.c_int, _dp]
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _arr(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a
+
+
+def set_threads(n: int) -> None:
+    lib().oracle_set_threads(int(n))
+
+
+def get_threads() -> int:
+    return lib().oracle_get_threads()
+
+
+# ----------------------------------------------------------- building blocks (pins)
+def qplus(eps_j, eps_jp1):
+    return lib().oracle_qplus(eps_j, eps_jp1)
+
+
+def qminus(eps_j, eps_jm1):
+    return lib().oracle_qminus(eps_j, eps_jm1)
+
+
+def transport(U, eps, f, lam, lo, hi):
+    """eq. (17) on one extended pencil; returns Uhat (only [lo,hi) is meaningful)."""
+    U, eps = _arr(U), _arr(eps)
+    out = np.zeros_like(U)
+    fp = None
+    if f is not None:
+        f = _arr(f)
+        fp = _p(f)
+    lib().oracle_transport(len(U), _p(U), _p(eps), fp, lam, _p(out), lo, hi)
+    return out
+
+
+def antidiffuse(U, Uhat, lo, hi, diff=1.0):
+    U, Uhat = _arr(U), _arr(Uhat)
+    out = np.zeros_like(U)
+    lib().oracle_antidiffuse(len(U), _p(U), _p(Uhat), diff, _p(out), lo, hi)
+    return out
+
+
+def prim2cons(e, n, vx, vy, vz, gamma, mass=0.0):
+    out = np.zeros(5)
+    lib().oracle_prim2cons(e, n, vx, vy, vz, gamma, mass, _p(out))
+    return out
+
+
+def cons2prim(E, Mx, My, Mz, R, gamma, mass=0.0):
+    """returns (array [e,p,n,vx,vy,vz,|v|], iterations, flags[2])."""
+    out = np.zeros(7)
+    fl = (C.c_int * 2)(0, 0)
+    it = lib().oracle_cons2prim(E, Mx, My, Mz, R, gamma, mass, _p(out), fl)
+    return out, it, (fl[0], fl[1])
+
+
+def project(E, M):
+    m = np.array(M, dtype=np.float64)
+    r = lib().oracle_project(E, _p(m))
+    return m, r
+
+
+def sweep_pencil(U5, axis, lam, gamma, mass=0.0, bc=OUTFLOW):
+    """U5: (5, N) array; returns the swept copy and the counts [Pi fired, vacuum]."""
+    U5 = np.array(U5, dtype=np.float64, order="C")
+    N = U5.shape[1]
+    ptrs = (_dp * 5)(*[_p(U5[f]) for f in range(5)])
+    cnt = (C.c_ulonglong * 2)(0, 0)
+    lib().oracle_sweep_pencil(N, ptrs, axis, lam, gamma, mass, bc, cnt)
+    return U5, (cnt[0], cnt[1])
+
+
+def advect_pencil(U, vel, lam, bc, nsteps):
+    """P5 helper: prescribed-velocity source-free advection; returns (U_new, Uhat of last step)."""
+    U = np.array(U, dtype=np.float64)
+    vel = _arr(vel)
+    uh = np.zeros_like(U)
+    lib().oracle_advect_pencil(len(U), _p(U), _p(vel), lam, bc, nsteps, _p(uh))
+    return U, uh
+
+
+# ----------------------------------------------------------------------- the grid
+class Oracle:
+    """Same call sequence as the product's C ABI (include/shasta.h) with host arrays."""
+
+    def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0):
+        self.shape = (nz, ny, nx)
+        self._h = lib().oracle_create(nx, ny, nz, dx, lam, eos_gamma)
+        if not self._h:
+            raise ValueError("oracle_create: bad argument")
+        self.set_option(BOUNDARY, boundary)
+        self.set_option(EOS_MASS, eos_mass)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().oracle_destroy(self._h)
+            self._h = None
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise RuntimeError(f"{what} failed: {rc}")
+
+    def set_option(self, key, value):
+        self._chk(lib().oracle_set_option(self._h, key, float(value)), "oracle_set_option")
+
+    def set_sweep_table(self, axes):
+        a = (C.c_int * len(axes))(*axes)
+        self._chk(lib().oracle_set_sweep_table(self._h, a, len(axes)), "oracle_set_sweep_table")
+
+    def set_state(self, e, n, vx, vy, vz):
+        arrs = [_arr(x).reshape(self.shape) for x in (e, n, vx, vy, vz)]
+        self._chk(lib().oracle_set_state(self._h, *[_p(a) for a in arrs]), "oracle_set_state")
+
+    def set_conserved(self, E, Mx, My, Mz, R):
+        arrs = [_arr(x).reshape(self.shape) for x in (E, Mx, My, Mz, R)]
+        self._chk(lib().oracle_set_conserved(self._h, *[_p(a) for a in arrs]), "oracle_set_conserved")
+
+    def step(self, nsteps=1):
+        self._chk(lib().oracle_step(self._h, int(nsteps)), "oracle_step")
+
+    def get_conserved(self):
+        out = [np.empty(self.shape) for _ in range(5)]
+        self._chk(lib().oracle_get_conserved(self._h, *[_p(a) for a in out]), "oracle_get_conserved")
+        return dict(zip(("E", "Mx", "My", "Mz", "R"), out))
+
+    def get_primitives(self):
+        out = [np.empty(self.shape) for _ in range(6)]
+        self._chk(lib().oracle_get_primitives(self._h, *[_p(a) for a in out]), "oracle_get_primitives")
+        return dict(zip(("e", "p", "n", "vx", "vy", "vz"), out))
+
+    def conserved_totals(self):
+        t = np.zeros(5)
+        self._chk(lib().oracle_conserved_totals(self._h, _p(t)), "oracle_conserved_totals")
+        return t
+
+    def diagnostics(self):
+        c = (C.c_ulonglong * 4)()
+        self._chk(lib().oracle_diagnostics(self._h, c), "oracle_diagnostics")
+        return [int(x) for x in c]
+
+    @property
+    def step_index(self):
+        return int(lib().oracle_step_index(self._h))

@@ -1,0 +1,149 @@
+"""Pins P6, P10, P11, P12 and the axis table: the 3-D assembly of the oracle."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1206_0919_b200 import inputs
+
+
+def _mk(oracle, c, table=None):
+    o = oracle.Oracle(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"])
+    if table is not None:
+        o.set_sweep_table(table)
+    o.set_state(c["e"], c["n"], c["vx"], c["vy"], c["vz"])
+    return o
+
+
+def _fsum_totals(o, dx):
+    return np.array([math.fsum(v.ravel()) * dx ** 3 for v in o.get_conserved().values()])
+
+
+def test_P6_conservation_periodic(oracle):
+    c = inputs.spherical_riemann(32, steps=12)
+    o = _mk(oracle, c)
+    t0 = _fsum_totals(o, c["dx"])
+    o.step(12)
+    t1 = _fsum_totals(o, c["dx"])
+    assert abs(t1[0] - t0[0]) <= 1e-12 * abs(t0[0])          # E
+    assert abs(t1[4] - t0[4]) <= 1e-12 * abs(t0[4])          # R
+    d = o.diagnostics()
+    assert d[0] == 0 and d[1] == 0                           # Pi never fires for 1.0 / 0.01
+    assert np.max(np.abs(t1[1:4])) <= 1e-12 * t0[0]          # symmetric: total momentum stays 0
+    # the library's own compensated totals agree with math.fsum
+    assert np.max(np.abs(o.conserved_totals() - t1)) <= 1e-13 * t0[0]
+    # and something actually happened
+    assert np.abs(o.get_primitives()["vx"]).max() > 0.1
+
+
+def test_P6_momentum_conserved_with_net_flow(oracle):
+    c = inputs.random_state(12, 10, 8, seed=5, kind="smooth", vmax=0.5, boundary=inputs.PERIODIC)
+    o = _mk(oracle, c)
+    t0 = _fsum_totals(o, c["dx"])
+    o.step(6)
+    t1 = _fsum_totals(o, c["dx"])
+    assert o.diagnostics()[0] == 0
+    scale = abs(t0[0])
+    assert np.max(np.abs(t1 - t0)) <= 1e-12 * scale
+
+
+def test_P10_uniform_state_bitwise(oracle):
+    for bc in (inputs.OUTFLOW, inputs.PERIODIC):
+        sh = (8, 8, 8)
+        c = dict(nx=8, ny=8, nz=8, dx=0.1, lam=0.4, gamma=4.0 / 3.0, mass=0.0, boundary=bc,
+                 e=np.full(sh, 1.7), n=np.full(sh, 0.9), vx=np.full(sh, 0.3), vy=np.full(sh, -0.2),
+                 vz=np.full(sh, 0.5))
+        o = _mk(oracle, c)
+        before = {k: v.copy() for k, v in o.get_conserved().items()}
+        o.step(6)
+        after = o.get_conserved()
+        for k in before:
+            assert np.array_equal(before[k], after[k]), k
+
+
+def test_P11_plane_symmetric_3d_equals_1d(oracle):
+    ref = _mk(oracle, inputs.shock_tube(100, 0.01, steps=40)); ref.step(40)
+    r = ref.get_conserved()
+    thick = _mk(oracle, inputs.shock_tube(100, 0.01, transverse=3, steps=40)); thick.step(40)
+    t = thick.get_conserved()
+    assert ref.diagnostics()[0] > 0                           # Pi fired on this path
+    for k in r:
+        assert np.max(np.abs(t[k] - r[k].reshape(1, 1, 100))) <= 1e-13, k
+    # the same tube laid along z (Mx <-> Mz) and along y
+    for axis, mom in ((2, "Mz"), (1, "My")):
+        oz = _mk(oracle, inputs.shock_tube(100, 0.01, axis=axis, transverse=2, steps=40)); oz.step(40)
+        z = oz.get_conserved()
+        prof = np.moveaxis(z["E"], 2 - axis, -1).reshape(-1, 100)
+        assert np.max(np.abs(prof - r["E"].ravel())) <= 1e-13
+        profm = np.moveaxis(z[mom], 2 - axis, -1).reshape(-1, 100)
+        assert np.max(np.abs(profm - r["Mx"].ravel())) <= 1e-13
+        assert np.all(z["Mx"] == 0.0)
+
+
+def test_P12_mirror_and_transpose_symmetry(oracle):
+    zc = np.abs(np.arange(16) - 7.5)                          # mirror symmetric but not x<->z symmetric
+    c = inputs.fireball(16, steps=8)
+    c["e"] = c["e"] * (1.0 + 0.05 * zc)[:, None, None]
+    c["n"] = c["e"] ** 0.75
+    o = _mk(oracle, c); o.step(8)
+    u = o.get_conserved()
+    sc = np.abs(u["E"]).max()
+    # (i) mirror in every axis
+    assert np.max(np.abs(u["E"] - u["E"][:, :, ::-1])) <= 1e-13 * sc
+    assert np.max(np.abs(u["Mx"] + u["Mx"][:, :, ::-1])) <= 1e-13 * sc
+    assert np.max(np.abs(u["Mz"] + u["Mz"][::-1, :, :])) <= 1e-13 * sc
+    assert np.max(np.abs(u["My"] - u["My"][::-1, :, :])) <= 1e-13 * sc
+    # (ii) transpose x<->z with the axis table relabelled 0<->2
+    ct = dict(c)
+    for k in ("e", "n", "vx", "vy", "vz"):
+        ct[k] = np.ascontiguousarray(np.transpose(c[k], (2, 1, 0)))
+    ct["vx"], ct["vz"] = ct["vz"], ct["vx"]
+    relabel = [2 - a if a != 1 else 1 for a in oracle.BRANCH]
+    ot = _mk(oracle, ct, table=relabel); ot.step(8)
+    ut = ot.get_conserved()
+    assert np.max(np.abs(np.transpose(ut["E"], (2, 1, 0)) - u["E"])) <= 1e-13 * sc
+    assert np.max(np.abs(np.transpose(ut["Mx"], (2, 1, 0)) - u["Mz"])) <= 1e-13 * sc
+    assert np.max(np.abs(np.transpose(ut["R"], (2, 1, 0)) - u["R"])) <= 1e-13 * np.abs(u["R"]).max()
+
+
+def test_P12_spherical_blob_axis_symmetry_to_splitting_error(oracle):
+    c = inputs.fireball(32, steps=12)
+    o = _mk(oracle, c); o.step(12)
+    E = o.get_conserved()["E"]
+    asym = np.max(np.abs(E - np.transpose(E, (2, 1, 0)))) / np.abs(E).max()
+    assert asym < 1e-3
+
+
+def test_axis_table_and_step_index(oracle):
+    # six permutations, period 6 steps; a run split in two equals the run in one go
+    assert sorted(tuple(oracle.BRANCH[i:i + 3]) for i in range(0, 18, 3)) == sorted(
+        [(0, 1, 2), (0, 2, 1), (1, 0, 2), (1, 2, 0), (2, 0, 1), (2, 1, 0)])
+    c = inputs.random_state(9, 7, 5, seed=3, kind="rough")
+    a = _mk(oracle, c); a.step(7)
+    b = _mk(oracle, c); b.step(3); b.step(4)
+    assert a.step_index == 7 and b.step_index == 7
+    for k, v in a.get_conserved().items():
+        assert np.array_equal(v, b.get_conserved()[k])
+    # different order gives a (slightly) different answer: the table is really used
+    d = _mk(oracle, c, table=[2, 1, 0]); d.step(7)
+    assert not np.array_equal(d.get_conserved()["E"], a.get_conserved()["E"])
+    # extent-1 axes are skipped (reading G15): 1D run has no y/z dependence
+    e = _mk(oracle, inputs.shock_tube(50, 0.01, steps=5)); e.step(5)
+    assert np.all(e.get_conserved()["My"] == 0.0)
+
+
+def test_boundary_rules(oracle):
+    # periodic: shifting the data by k cells shifts the answer (translation invariance, reading G11)
+    c = inputs.random_state(16, 1, 1, seed=11, kind="rough", boundary=inputs.PERIODIC)
+    a = _mk(oracle, c); a.step(5)
+    cs = dict(c)
+    for k in ("e", "n", "vx", "vy", "vz"):
+        cs[k] = np.ascontiguousarray(np.roll(c[k], 5, axis=2))
+    b = _mk(oracle, cs); b.step(5)
+    for k, v in a.get_conserved().items():
+        assert np.array_equal(np.roll(v, 5, axis=2), b.get_conserved()[k]), k
+    # outflow: a state uniform near the edges keeps them bitwise unchanged until the wave arrives
+    c = inputs.shock_tube(100, 0.01, steps=10)
+    o = _mk(oracle, c); before = o.get_conserved()["E"].copy(); o.step(10)
+    after = o.get_conserved()["E"]
+    assert np.array_equal(before[..., :20], after[..., :20]) and np.array_equal(before[..., -20:], after[..., -20:])

@@ -1,0 +1,97 @@
+"""Pins P7, P13: phases 3+4 -- relativistic correction and EOS inversion."""
+import numpy as np
+import pytest
+
+
+def _rand_prims(rng, n, vmax=0.9999):
+    e = 10.0 ** rng.uniform(-8, 2, n)
+    v = rng.uniform(0, vmax, n)
+    d = rng.normal(size=(n, 3)); d /= np.linalg.norm(d, axis=1)[:, None]
+    return e, v[:, None] * d
+
+
+@pytest.mark.parametrize("gamma,mass", [(4.0 / 3.0, 0.0), (5.0 / 3.0, 1.0), (5.0 / 3.0, 0.0)])
+def test_P7_round_trip(oracle, gamma, mass):
+    rng = np.random.default_rng(7)
+    e, v = _rand_prims(rng, 4000)
+    nd = e ** 0.75 * (0.3 if mass else 1.0)
+    for i in range(len(e)):
+        c = oracle.prim2cons(e[i], nd[i], *v[i], gamma, mass)
+        out, it, _ = oracle.cons2prim(*c, gamma, mass)
+        g2 = 1.0 / (1.0 - v[i] @ v[i])
+        assert it < 200
+        assert np.max(np.abs(out[3:6] - v[i])) < 2e-14
+        assert abs(out[0] - e[i]) / e[i] < 1e-14 * g2
+        assert abs(out[2] - nd[i]) / nd[i] < 1e-14 * g2
+
+
+def test_P7_eqs_9_to_11_literal(oracle):
+    # eqs. (9)-(11) retyped: N = rho gamma, M = (e+p) gamma^2 v, E = (e + p v^2) gamma^2
+    e, n, v = 2.5, 0.7, np.array([0.3, -0.4, 0.5])
+    p = e / 3.0
+    g2 = 1.0 / (1.0 - v @ v)
+    c = oracle.prim2cons(e, n, *v, 4.0 / 3.0, 0.0)
+    assert abs(c[0] - (e + p * (v @ v)) * g2) < 1e-14
+    assert np.max(np.abs(c[1:4] - (e + p) * g2 * v)) < 1e-14
+    assert abs(c[4] - n * np.sqrt(g2)) < 1e-15
+
+
+def test_P7_closed_form_gamma_law(oracle):
+    # m = 0: v = 2M / (G E + sqrt(G^2 E^2 - 4 (G-1) M^2))  (root of the quadratic, textbook)
+    rng = np.random.default_rng(8)
+    for G in (4.0 / 3.0, 5.0 / 3.0, 1.1):
+        for _ in range(1000):
+            E = 10.0 ** rng.uniform(-6, 2)
+            M = E * rng.uniform(0, 0.9999)
+            out, _, _ = oracle.cons2prim(E, 0.0, M, 0.0, 1.0, G, 0.0)
+            v = 2 * M / (G * E + np.sqrt(G * G * E * E - 4 * (G - 1) * M * M))
+            assert abs(out[6] - v) < 1e-14
+            assert abs(out[4] - v) < 1e-14 and out[3] == 0.0 and out[5] == 0.0
+
+
+def test_P7_bisection_general_eos(oracle):
+    # m = 1: root of g(v) = v (E + P(E - M v, R sqrt(1-v^2))) - M on [0,1), by brute-force bracketing
+    rng = np.random.default_rng(9)
+    G = 5.0 / 3.0
+    for _ in range(500):
+        e = 10.0 ** rng.uniform(-2, 2); n = e * rng.uniform(0.0, 0.9); v0 = rng.uniform(0, 0.99)
+        c = oracle.prim2cons(e, n, v0, 0.0, 0.0, G, 1.0)
+        E, M, R = c[0], c[1], c[4]
+        g = lambda v: v * (E + max((G - 1) * ((E - M * v) - R * np.sqrt(1 - v * v)), 0.0)) - M
+        lo, hi = 0.0, 1.0                                     # g(0) = -M <= 0 < g(1): 200-step bisection
+        for _ in range(200):
+            mid = 0.5 * (lo + hi)
+            if g(mid) > 0.0:
+                hi = mid
+            else:
+                lo = mid
+        vb = 0.5 * (lo + hi)
+        out, it, _ = oracle.cons2prim(*c, G, 1.0)
+        assert abs(out[6] - vb) < 1e-14, (e, n, v0, it)
+
+
+def test_P7_special_cases(oracle):
+    out, it, _ = oracle.cons2prim(2.0, 0.0, 0.0, 0.0, 0.5, 4.0 / 3.0, 0.0)
+    assert out[6] == 0.0 and out[0] == 2.0 and out[2] == 0.5 and abs(out[1] - 2.0 / 3.0) < 3e-16
+    # R = 0 with m = 1 reduces to the m = 0 closed form
+    a, _, _ = oracle.cons2prim(3.0, 1.0, 0.5, -0.2, 0.0, 5.0 / 3.0, 1.0)
+    b, _, _ = oracle.cons2prim(3.0, 1.0, 0.5, -0.2, 0.0, 5.0 / 3.0, 0.0)
+    assert np.array_equal(a, b)
+
+
+def test_P13_vacuum_and_projection(oracle):
+    out, _, _ = oracle.cons2prim(0.0, 1.0, 0.0, 0.0, 1.0, 4.0 / 3.0, 0.0)
+    assert np.all(out == 0.0)
+    out, _, _ = oracle.cons2prim(-1.0, 0.1, 0.0, 0.0, 1.0, 4.0 / 3.0, 0.0)
+    assert np.all(out == 0.0)
+    m, r = oracle.project(-1.0, [1.0, 2.0, 3.0])
+    assert r == 2 and np.all(m == 0.0)
+    m, r = oracle.project(1.0, [0.0, 2.0, 0.0])               # M = 2E -> scaled to (1-delta) E
+    assert r == 1 and m[0] == 0.0 and m[2] == 0.0 and abs(m[1] - (1.0 - 1e-12)) < 1e-16
+    m, r = oracle.project(1.0, [1.2, -1.6, 0.0])              # direction kept
+    assert r == 1 and abs(m[0] / m[1] + 0.75) < 1e-15 and abs(np.linalg.norm(m) - (1 - 1e-12)) < 1e-15
+    m, r = oracle.project(1.0, [0.3, 0.4, 0.0])
+    assert r == 0 and list(m) == [0.3, 0.4, 0.0]
+    # cons2prim applies the same min internally: superluminal input gives v just below 1, e >= 0
+    out, _, _ = oracle.cons2prim(1.0, 0.0, 0.0, 5.0, 1.0, 4.0 / 3.0, 0.0)
+    assert 0.999999 < out[5] < 1.0 and out[0] >= 0.0
