@@ -1,0 +1,118 @@
+/*
+ * shasta.h -- C ABI of libshasta.so: the dimensionally split (3+1)D relativistic SHASTA
+ * flux-corrected-transport time step of arXiv:1206.0919 on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are "PAPER.md:<line>" (the paper's text) and "DESIGN.md n" (this repo).
+ *
+ * Conventions (all entry points)
+ *  - Return 0 on success, <0 on error: SHASTA_EINVAL bad argument, SHASTA_ECUDA CUDA error,
+ *    SHASTA_ENOMEM out of device memory, SHASTA_ESTATE wrong state (e.g. step before
+ *    set_state).  Nothing throws or aborts; shasta_last_error(h) gives the message.
+ *  - Fields are SoA arrays of nx*ny*nz doubles, x fastest: index ix + nx*(iy + ny*iz)
+ *    (the paper's flat index).  Field order of conserved fields: E, Mx, My, Mz, R
+ *    (R is the paper's N, eq. (9)); of primitives: e, p, n, vx, vy, vz.
+ *  - Pointers named *_dev are DEVICE pointers, pointers named *_host are HOST pointers (pinned
+ *    or pageable).  The caller owns every buffer it passes; the library copies and never keeps
+ *    a caller pointer.  The handle owns all device memory it allocates.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the default stream).  Unless stated
+ *    otherwise a call only enqueues work on `stream` and returns; it is the caller's job to
+ *    keep the buffers alive until the stream has run.
+ *  - There is no CPU fallback: without a CUDA device shasta_create returns SHASTA_ECUDA.
+ */
+#ifndef SHASTA_H
+#define SHASTA_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct shasta shasta_t;   /* opaque */
+
+#define SHASTA_OK      0
+#define SHASTA_EINVAL (-1)
+#define SHASTA_ECUDA  (-2)
+#define SHASTA_ENOMEM (-3)
+#define SHASTA_ESTATE (-4)
+
+/* option keys for shasta_set_option */
+#define SHASTA_BOUNDARY   0   /* 0 = outflow (default): ghost = copy of the edge cell; 1 = periodic   */
+#define SHASTA_EOS_MASS   1   /* m in p = (eos_gamma-1)(e - m n); default 0 -> p = (Gamma-1) e         */
+#define SHASTA_PRECISION  2   /* 64 (default) | 32: storage and transport arithmetic (before set_state) */
+#define SHASTA_STEP_INDEX 3   /* step counter s indexing the axis table (resume / tests)                */
+#define SHASTA_SEGMENT    4   /* tuning: cells marched per work item along the sweep axis (0 = auto)    */
+
+/*
+ * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only
+ * (eqs. (15)-(17)); dx enters shasta_conserved_totals.  0 < lambda <= 0.5
+ * (SHASTA's stability range, the denominators of eq. (15) stay > 0), eos_gamma > 1
+ * (4/3 gives p = e/3).  Allocates 2x5 conserved fields (ping-pong, the paper's double
+ * buffering PAPER.md:161) + 6 primitive fields on the current device.
+ */
+int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lambda, double eos_gamma);
+void shasta_destroy(shasta_t* h);
+
+/* Options; BOUNDARY, EOS_MASS and PRECISION must be set before shasta_set_state. */
+int shasta_set_option(shasta_t* h, int key, double value);
+
+/* Axis order: step s runs sweeps along axes[(3s+k) % n], k = 0,1,2 (0=x,1=y,2=z).  Default: the
+ * paper's 18-entry table branch[], i.e. the six permutations.  n % 3 == 0, n <= 63.
+ * `axes` is a host pointer. */
+int shasta_set_sweep_table(shasta_t* h, const int* axes_host, int n);
+
+/* Primitive initial state -> conserved fields, eqs. (9)-(11) PAPER.md:58-62:
+ * p = EOS(e,n), w = (e+p)/(1-v^2), E = w - p, M = w v, R = n/sqrt(1-v^2).  Requires |v| < 1.
+ * Also fills the primitive output fields (they equal the input up to round-off). */
+int shasta_set_state(shasta_t* h, const double* e_dev, const double* n_dev, const double* vx_dev,
+                     const double* vy_dev, const double* vz_dev, void* stream);
+/* Same with HOST pointers: the host->device copies are enqueued on `stream` (asynchronous only if
+ * the host memory is pinned). */
+int shasta_set_state_host(shasta_t* h, const double* e_host, const double* n_host,
+                          const double* vx_host, const double* vy_host, const double* vz_host,
+                          void* stream);
+/* Set / get the conserved fields directly (checkpoint-resume, parity on conserved fields).
+ * set: all five required; the causality projection Pi (G6-G8) is NOT applied.
+ * get: any pointer may be NULL = skip. */
+int shasta_set_conserved(shasta_t* h, const double* E_dev, const double* Mx_dev, const double* My_dev,
+                         const double* Mz_dev, const double* R_dev, void* stream);
+int shasta_get_conserved(shasta_t* h, double* E_dev, double* Mx_dev, double* My_dev, double* Mz_dev,
+                         double* R_dev, void* stream);
+
+/*
+ * Advance nsteps time steps dt = lambda*dx.  One step = three fused sweep kernels, one per axis in
+ * table order (axes of extent 1 are skipped); each sweep does, per pencil, in one pass over the five
+ * conserved fields: ghost extension (boundary), cons2prim, half-step predictor transport (eq. (17) with
+ * lambda/2), cons2prim, full-step transport with diffusion (eqs. (15)-(17)), phoenical antidiffusion with
+ * the flux limiter (eqs. (18)-(22)), the causality projection, and -- in the last
+ * sweep of a step -- cons2prim of the new state into the primitive fields.  Asynchronous on `stream`.
+ */
+int shasta_step(shasta_t* h, int nsteps, void* stream);
+
+/* Primitive fields of the current state (phases 3-4): e = E - |M| v,
+ * n = R sqrt(1-v^2), p = EOS(e,n), v = root of v (E + p) = |M|.  Any pointer may be NULL = skip. */
+int shasta_get_primitives(shasta_t* h, double* e_dev, double* p_dev, double* n_dev, double* vx_dev,
+                          double* vy_dev, double* vz_dev, void* stream);
+int shasta_get_primitives_host(shasta_t* h, double* e_host, double* p_host, double* n_host,
+                               double* vx_host, double* vy_host, double* vz_host, void* stream);
+
+/* dx^3 * sum over cells of E, Mx, My, Mz, R (the conserved totals of eqs. (12)-(14)),
+ * compensated fp64 summation.  `totals_host` is a host pointer to 5 doubles.  SYNCHRONISES `stream`. */
+int shasta_conserved_totals(shasta_t* h, double* totals_host, void* stream);
+
+/* Cumulative counters since create (host pointer to 4 values): [0] cells where the projection Pi
+ * (|M| <= (1-1e-12) E) fired at the end of a sweep, [1] vacuum cells (E <= 0) seen there,
+ * [2] e < 0 floored, [3] p < 0 floored in the primitive output.  SYNCHRONISES the device. */
+int shasta_diagnostics(shasta_t* h, unsigned long long* counts_host);
+
+/* Number of kernels this handle has launched since create (bench.py's gpu_launches). */
+long long shasta_launch_count(const shasta_t* h);
+/* Step counter s (number of steps taken, or the value set by SHASTA_STEP_INDEX). */
+long long shasta_step_index(const shasta_t* h);
+/* Name of the sweep kernel variant used for `axis` with the current options (for profiles/). */
+const char* shasta_kernel_name(const shasta_t* h, int axis);
+
+const char* shasta_last_error(const shasta_t* h);   /* h may be NULL: error of the last failed create */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHASTA_H */

@@ -1,0 +1,617 @@
+// shasta.cu -- host side of libshasta.so: the C ABI of include/shasta.h.
+// Orchestration only (Listing 2): axis table, ping-pong buffers, launches.
+// Every arithmetic step of the path runs in the kernels of shasta_kernels.cuh.
+#include "shasta.h"
+#include "shasta_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace shk;
+
+namespace {
+
+thread_local char g_create_err[256] = "";
+
+const int kBranch[18] = {0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2};
+
+constexpr int XROWS64 = 128;    // rows per CTA of the x sweep, fp64
+constexpr int XROWS32 = 256;    // fp32
+constexpr int STRIDED_BLOCK = 128;
+constexpr int RED_BLOCKS = 592; // 4 per SM
+constexpr int RED_THREADS = 256;
+
+}  // namespace
+
+struct shasta {
+    int nx, ny, nz;
+    long long ncell;
+    double dx, lambda, gamma, mass;
+    int periodic;
+    int precision;          // 64 | 32
+    int seg_override;
+    long long step;
+    int table[64];
+    int ntable;
+    void* U[2][NF];         // conserved, ping-pong, natural order E,Mx,My,Mz,R
+    void* prim[6];          // e,p,n,vx,vy,vz
+    double* stage;          // fp64 staging (5 fields) for host<->device and fp32 conversion
+    int cur;
+    bool allocated, have_state, prims_valid;
+    unsigned long long* d_counts;
+    double* d_partial;      // RED_BLOCKS*NF*2
+    double* h_partial;      // pinned
+    long long launches;
+    int sm_count;
+    char err[256];
+};
+
+namespace {
+
+int fail(shasta_t* h, int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(h ? h->err : g_create_err, 256, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CK(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(h, e_ == cudaErrorMemoryAllocation ? SHASTA_ENOMEM : SHASTA_ECUDA,    \
+                        "%s: %s", #call, cudaGetErrorString(e_));                             \
+    } while (0)
+
+size_t esize(const shasta_t* h) { return h->precision == 64 ? 8 : 4; }
+
+int ensure_alloc(shasta_t* h)
+{
+    if (h->allocated) return 0;
+    const size_t nb = (size_t)h->ncell * esize(h);
+    for (int b = 0; b < 2; ++b)
+        for (int f = 0; f < NF; ++f) CK(cudaMalloc(&h->U[b][f], nb));
+    for (int q = 0; q < 6; ++q) CK(cudaMalloc(&h->prim[q], nb));
+    CK(cudaMalloc(&h->d_counts, 4 * sizeof(unsigned long long)));
+    CK(cudaMemset(h->d_counts, 0, 4 * sizeof(unsigned long long)));
+    CK(cudaMalloc(&h->d_partial, sizeof(double) * RED_BLOCKS * NF * 2));
+    CK(cudaMallocHost(&h->h_partial, sizeof(double) * RED_BLOCKS * NF * 2));
+    h->allocated = true;
+    return 0;
+}
+
+int ensure_stage(shasta_t* h)
+{
+    if (!h->stage) CK(cudaMalloc(&h->stage, sizeof(double) * (size_t)h->ncell * 6));
+    return 0;
+}
+
+template <typename T>
+Consts<T> make_consts(const shasta_t* h)
+{
+    Consts<T> k;
+    k.lam = (T)h->lambda;
+    k.hlam = (T)(0.5 * h->lambda);
+    k.gam = (T)h->gamma;
+    k.gm1 = (T)(h->gamma - 1.0);
+    k.g2 = (T)(h->gamma * h->gamma);
+    k.c4 = (T)(4.0 * (h->gamma - 1.0));
+    k.hg = (T)(0.5 * h->gamma);
+    k.omd = (T)(1.0 - 1e-12);
+    k.mass = (T)h->mass;
+    return k;
+}
+
+// ---------------------------------------------------------------- elementwise kernels
+// eqs. (9)-(11).  Computed in fp64, stored in T.
+template <typename T>
+__global__ void prim2cons_kernel(long long n, const double* __restrict__ e, const double* __restrict__ nd,
+                                 const double* __restrict__ vx, const double* __restrict__ vy,
+                                 const double* __restrict__ vz, double gm1, double mass,
+                                 T* E, T* Mx, T* My, T* Mz, T* R, T* pe, T* pp, T* pn, T* pvx, T* pvy, T* pvz)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const double ee = e[i], nn = nd[i], ax = vx[i], ay = vy[i], az = vz[i];
+        double p = gm1 * (ee - mass * nn);
+        p = p > 0.0 ? p : 0.0;
+        const double v2 = fma(ax, ax, fma(ay, ay, az * az));
+        const double g2 = 1.0 / (1.0 - v2);
+        const double w = (ee + p) * g2;
+        E[i] = (T)(w - p);
+        Mx[i] = (T)(w * ax); My[i] = (T)(w * ay); Mz[i] = (T)(w * az);
+        R[i] = (T)(nn * sqrt(g2));
+        pe[i] = (T)ee; pp[i] = (T)p; pn[i] = (T)nn; pvx[i] = (T)ax; pvy[i] = (T)ay; pvz[i] = (T)az;
+    }
+}
+
+template <typename T, int EOS>
+__global__ void cons2prim_kernel(long long n, Consts<T> k, const T* E, const T* Mx, const T* My, const T* Mz,
+                                 const T* R, T* pe, T* pp, T* pn, T* pvx, T* pvy, T* pvz,
+                                 unsigned long long* counts)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        T u[NF] = {E[i], Mx[i], My[i], Mz[i], R[i]};
+        T pr[6];
+        primitives<T, EOS>(k, u, pr, counts);
+        pe[i] = pr[0]; pp[i] = pr[1]; pn[i] = pr[2]; pvx[i] = pr[3]; pvy[i] = pr[4]; pvz[i] = pr[5];
+    }
+}
+
+template <typename A, typename B>
+__global__ void convert_kernel(long long n, const A* __restrict__ a, B* __restrict__ b)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x)
+        b[i] = (B)a[i];
+}
+
+// per-block Neumaier-compensated partial sums of the five fields (sum, compensation)
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) totals_kernel(long long n, const T* f0, const T* f1, const T* f2,
+                                                            const T* f3, const T* f4, double* partial)
+{
+    const T* fld[NF] = {f0, f1, f2, f3, f4};
+    __shared__ double sh[RED_THREADS / 32][NF][2];
+    double s[NF], c[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { s[f] = 0.0; c[f] = 0.0; }
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            const double x = (double)fld[f][i];
+            const double t = s[f] + x;
+            c[f] += (fabs(s[f]) >= fabs(x)) ? ((s[f] - t) + x) : ((x - t) + s[f]);
+            s[f] = t;
+        }
+    }
+    // warp tree with two-sum so the compensation survives
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        for (int o = 16; o > 0; o >>= 1) {
+            const double so = __shfl_down_sync(0xffffffffu, s[f], o);
+            const double co = __shfl_down_sync(0xffffffffu, c[f], o);
+            const double t = s[f] + so;
+            c[f] += co + ((fabs(s[f]) >= fabs(so)) ? ((s[f] - t) + so) : ((so - t) + s[f]));
+            s[f] = t;
+        }
+        if ((threadIdx.x & 31) == 0) { sh[threadIdx.x >> 5][f][0] = s[f]; sh[threadIdx.x >> 5][f][1] = c[f]; }
+    }
+    __syncthreads();
+    if (threadIdx.x < NF) {
+        const int f = threadIdx.x;
+        double ss = 0.0, cc = 0.0;
+        for (int w = 0; w < RED_THREADS / 32; ++w) {
+            const double x = sh[w][f][0];
+            const double t = ss + x;
+            cc += sh[w][f][1] + ((fabs(ss) >= fabs(x)) ? ((ss - t) + x) : ((x - t) + ss));
+            ss = t;
+        }
+        partial[(blockIdx.x * NF + f) * 2 + 0] = ss;
+        partial[(blockIdx.x * NF + f) * 2 + 1] = cc;
+    }
+}
+
+int ew_grid(const shasta_t* h, int threads)
+{
+    long long b = (h->ncell + threads - 1) / threads;
+    long long cap = (long long)h->sm_count * 16;
+    return (int)(b < cap ? (b < 1 ? 1 : b) : cap);
+}
+
+// ---------------------------------------------------------------- sweep launch
+int auto_segment(const shasta_t* h, int axis, int N, long long npencil)
+{
+    if (h->seg_override > 0) return h->seg_override < N ? h->seg_override : N;
+    // enough work items for ~4 waves of resident threads, segments not shorter than 32 cells
+    const long long resident = (long long)h->sm_count * 256;
+    long long nseg = (4 * resident + npencil - 1) / npencil;
+    if (nseg < 1) nseg = 1;
+    long long seg = (N + nseg - 1) / nseg;
+    if (seg < 32) seg = 32;
+    if (axis == 0) seg = ((seg + XCH - 1) / XCH) * XCH;   // chunk-aligned segments for the x sweep
+    return (int)(seg < N ? seg : N);
+}
+
+template <typename T, int EOS, bool EMIT>
+int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
+{
+    const int n[3] = {h->nx, h->ny, h->nz};
+    const long long stride[3] = {1, h->nx, (long long)h->nx * h->ny};
+    const int perm[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};   // parallel, perp1, perp2 momentum components
+    SweepParams P;
+    const int src = h->cur, dst = 1 - h->cur;
+    P.in[0] = h->U[src][0]; P.out[0] = h->U[dst][0];
+    for (int c = 0; c < 3; ++c) {
+        P.in[1 + c] = h->U[src][1 + perm[axis][c]];
+        P.out[1 + c] = h->U[dst][1 + perm[axis][c]];
+        P.prim[3 + c] = h->prim[3 + perm[axis][c]];
+    }
+    P.in[4] = h->U[src][4]; P.out[4] = h->U[dst][4];
+    P.prim[0] = h->prim[0]; P.prim[1] = h->prim[1]; P.prim[2] = h->prim[2];
+    P.nx = h->nx;
+    P.N = n[axis];
+    P.stride_axis = stride[axis];
+    P.periodic = h->periodic;
+    P.counts = h->d_counts;
+    const Consts<T> k = make_consts<T>(h);
+    if (axis == 0) {
+        constexpr int ROWS = sizeof(T) == 8 ? XROWS64 : XROWS32;
+        P.npencil = (long long)h->ny * h->nz;
+        P.stride_other = 0;
+        P.seg = auto_segment(h, axis, P.N, P.npencil);
+        P.nseg = (P.N + P.seg - 1) / P.seg;
+        auto kern = sweep_x_kernel<T, EOS, EMIT, ROWS>;
+        const size_t smem = sizeof(XSmem<T, ROWS>);
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        dim3 grid((unsigned)((P.npencil + ROWS - 1) / ROWS), (unsigned)P.nseg);
+        kern<<<grid, ROWS, smem, st>>>(P, k);
+    } else {
+        // y sweep: pencils (x,z), base = x + z*nx*ny;  z sweep: pencils (x,y), base = x + y*nx = flat
+        const int other = axis == 1 ? 2 : 1;
+        P.npencil = (long long)h->nx * n[other];
+        P.stride_other = stride[other];
+        P.seg = auto_segment(h, axis, P.N, P.npencil);
+        P.nseg = (P.N + P.seg - 1) / P.seg;
+        dim3 grid((unsigned)((P.npencil + STRIDED_BLOCK - 1) / STRIDED_BLOCK), (unsigned)P.nseg);
+        sweep_strided_kernel<T, EOS, EMIT><<<grid, STRIDED_BLOCK, 0, st>>>(P, k);
+    }
+    CK(cudaGetLastError());
+    h->launches++;
+    h->cur = dst;
+    return 0;
+}
+
+int launch_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
+{
+    const bool general = h->mass != 0.0;
+    if (h->precision == 64) {
+        if (general) return emit ? launch_sweep_t<double, EOS_MASS, true>(h, axis, st)
+                                 : launch_sweep_t<double, EOS_MASS, false>(h, axis, st);
+        return emit ? launch_sweep_t<double, EOS_GAMMA, true>(h, axis, st)
+                    : launch_sweep_t<double, EOS_GAMMA, false>(h, axis, st);
+    }
+    if (general) return emit ? launch_sweep_t<float, EOS_MASS, true>(h, axis, st)
+                             : launch_sweep_t<float, EOS_MASS, false>(h, axis, st);
+    return emit ? launch_sweep_t<float, EOS_GAMMA, true>(h, axis, st)
+                : launch_sweep_t<float, EOS_GAMMA, false>(h, axis, st);
+}
+
+template <typename T>
+int refresh_prims_t(shasta_t* h, cudaStream_t st)
+{
+    void** U = h->U[h->cur];
+    const int g = ew_grid(h, 256);
+    const Consts<T> k = make_consts<T>(h);
+    if (h->mass != 0.0)
+        cons2prim_kernel<T, EOS_MASS><<<g, 256, 0, st>>>(h->ncell, k, (T*)U[0], (T*)U[1], (T*)U[2], (T*)U[3],
+            (T*)U[4], (T*)h->prim[0], (T*)h->prim[1], (T*)h->prim[2], (T*)h->prim[3], (T*)h->prim[4],
+            (T*)h->prim[5], h->d_counts);
+    else
+        cons2prim_kernel<T, EOS_GAMMA><<<g, 256, 0, st>>>(h->ncell, k, (T*)U[0], (T*)U[1], (T*)U[2], (T*)U[3],
+            (T*)U[4], (T*)h->prim[0], (T*)h->prim[1], (T*)h->prim[2], (T*)h->prim[3], (T*)h->prim[4],
+            (T*)h->prim[5], h->d_counts);
+    CK(cudaGetLastError());
+    h->launches++;
+    h->prims_valid = true;
+    return 0;
+}
+
+// copy one stored field (T) into a caller fp64 device buffer
+int export_field(shasta_t* h, const void* src, double* dst_dev, cudaStream_t st)
+{
+    if (h->precision == 64) {
+        CK(cudaMemcpyAsync(dst_dev, src, sizeof(double) * (size_t)h->ncell, cudaMemcpyDeviceToDevice, st));
+    } else {
+        convert_kernel<float, double><<<ew_grid(h, 256), 256, 0, st>>>(h->ncell, (const float*)src, dst_dev);
+        CK(cudaGetLastError());
+        h->launches++;
+    }
+    return 0;
+}
+
+}  // namespace
+
+// =========================================================================== C ABI
+extern "C" {
+
+int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lambda, double eos_gamma)
+{
+    shasta_t* h = nullptr;
+    if (!out) return fail(h, SHASTA_EINVAL, "shasta_create: out is NULL");
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return fail(h, SHASTA_EINVAL, "shasta_create: grid extents must be >= 1");
+    if (!(dx > 0.0)) return fail(h, SHASTA_EINVAL, "shasta_create: dx must be > 0");
+    if (!(lambda > 0.0) || lambda > 0.5) return fail(h, SHASTA_EINVAL, "shasta_create: need 0 < lambda <= 0.5");
+    if (!(eos_gamma > 1.0) || !(eos_gamma < 2.0))
+        return fail(h, SHASTA_EINVAL, "shasta_create: need 1 < eos_gamma < 2");
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+        return fail(h, SHASTA_ECUDA, "shasta_create: no CUDA device (there is no CPU fallback)");
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(h, SHASTA_ECUDA, "shasta_create: cudaGetDevice failed");
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+        return fail(h, SHASTA_ECUDA, "shasta_create: cudaGetDeviceProperties failed");
+    if (prop.major < 10)
+        return fail(h, SHASTA_ECUDA, "shasta_create: device sm_%d%d is not sm_100 (B200) -- kernels are built for sm_100a only",
+                    prop.major, prop.minor);
+    h = new (std::nothrow) shasta();
+    if (!h) return fail(nullptr, SHASTA_ENOMEM, "shasta_create: host allocation failed");
+    memset(h, 0, sizeof(*h));
+    h->nx = nx; h->ny = ny; h->nz = nz;
+    h->ncell = (long long)nx * ny * nz;
+    h->dx = dx; h->lambda = lambda; h->gamma = eos_gamma; h->mass = 0.0;
+    h->precision = 64;
+    memcpy(h->table, kBranch, sizeof(kBranch));
+    h->ntable = 18;
+    h->sm_count = prop.multiProcessorCount;
+    *out = h;
+    return 0;
+}
+
+void shasta_destroy(shasta_t* h)
+{
+    if (!h) return;
+    for (int b = 0; b < 2; ++b)
+        for (int f = 0; f < NF; ++f) cudaFree(h->U[b][f]);
+    for (int q = 0; q < 6; ++q) cudaFree(h->prim[q]);
+    cudaFree(h->stage);
+    cudaFree(h->d_counts);
+    cudaFree(h->d_partial);
+    if (h->h_partial) cudaFreeHost(h->h_partial);
+    delete h;
+}
+
+int shasta_set_option(shasta_t* h, int key, double value)
+{
+    if (!h) return SHASTA_EINVAL;
+    switch (key) {
+    case SHASTA_BOUNDARY:
+        if (value != 0.0 && value != 1.0) return fail(h, SHASTA_EINVAL, "SHASTA_BOUNDARY must be 0 or 1");
+        h->periodic = (int)value;
+        return 0;
+    case SHASTA_EOS_MASS:
+        if (!(value >= 0.0)) return fail(h, SHASTA_EINVAL, "SHASTA_EOS_MASS must be >= 0");
+        h->mass = value;
+        h->prims_valid = false;
+        return 0;
+    case SHASTA_PRECISION:
+        if (value != 64.0 && value != 32.0) return fail(h, SHASTA_EINVAL, "SHASTA_PRECISION must be 64 or 32");
+        if (h->allocated && (int)value != h->precision)
+            return fail(h, SHASTA_ESTATE, "SHASTA_PRECISION must be set before the first set_state");
+        h->precision = (int)value;
+        return 0;
+    case SHASTA_STEP_INDEX:
+        if (!(value >= 0.0)) return fail(h, SHASTA_EINVAL, "SHASTA_STEP_INDEX must be >= 0");
+        h->step = (long long)value;
+        return 0;
+    case SHASTA_SEGMENT:
+        if (!(value >= 0.0)) return fail(h, SHASTA_EINVAL, "SHASTA_SEGMENT must be >= 0");
+        h->seg_override = (int)value;
+        if (h->seg_override > 0 && h->seg_override < 8) h->seg_override = 8;
+        return 0;
+    default:
+        return fail(h, SHASTA_EINVAL, "shasta_set_option: unknown key %d", key);
+    }
+}
+
+int shasta_set_sweep_table(shasta_t* h, const int* axes, int n)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!axes || n < 3 || n > 63 || n % 3) return fail(h, SHASTA_EINVAL, "sweep table: need n % 3 == 0, 3 <= n <= 63");
+    for (int i = 0; i < n; ++i)
+        if (axes[i] < 0 || axes[i] > 2) return fail(h, SHASTA_EINVAL, "sweep table: axes must be 0, 1 or 2");
+    memcpy(h->table, axes, sizeof(int) * (size_t)n);
+    h->ntable = n;
+    return 0;
+}
+
+int shasta_set_state(shasta_t* h, const double* e, const double* n, const double* vx, const double* vy,
+                     const double* vz, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!e || !n || !vx || !vy || !vz) return fail(h, SHASTA_EINVAL, "shasta_set_state: NULL field pointer");
+    int rc = ensure_alloc(h);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    h->cur = 0;
+    void** U = h->U[0];
+    const int g = ew_grid(h, 256);
+    if (h->precision == 64)
+        prim2cons_kernel<double><<<g, 256, 0, st>>>(h->ncell, e, n, vx, vy, vz, h->gamma - 1.0, h->mass,
+            (double*)U[0], (double*)U[1], (double*)U[2], (double*)U[3], (double*)U[4], (double*)h->prim[0],
+            (double*)h->prim[1], (double*)h->prim[2], (double*)h->prim[3], (double*)h->prim[4], (double*)h->prim[5]);
+    else
+        prim2cons_kernel<float><<<g, 256, 0, st>>>(h->ncell, e, n, vx, vy, vz, h->gamma - 1.0, h->mass,
+            (float*)U[0], (float*)U[1], (float*)U[2], (float*)U[3], (float*)U[4], (float*)h->prim[0],
+            (float*)h->prim[1], (float*)h->prim[2], (float*)h->prim[3], (float*)h->prim[4], (float*)h->prim[5]);
+    CK(cudaGetLastError());
+    h->launches++;
+    h->have_state = true;
+    h->prims_valid = true;
+    return 0;
+}
+
+int shasta_set_state_host(shasta_t* h, const double* e, const double* n, const double* vx, const double* vy,
+                          const double* vz, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!e || !n || !vx || !vy || !vz) return fail(h, SHASTA_EINVAL, "shasta_set_state_host: NULL field pointer");
+    int rc = ensure_stage(h);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nb = sizeof(double) * (size_t)h->ncell;
+    const double* src[5] = {e, n, vx, vy, vz};
+    for (int f = 0; f < 5; ++f)
+        CK(cudaMemcpyAsync(h->stage + (size_t)f * h->ncell, src[f], nb, cudaMemcpyHostToDevice, st));
+    return shasta_set_state(h, h->stage, h->stage + h->ncell, h->stage + 2 * h->ncell, h->stage + 3 * h->ncell,
+                            h->stage + 4 * h->ncell, stream);
+}
+
+int shasta_set_conserved(shasta_t* h, const double* E, const double* Mx, const double* My, const double* Mz,
+                         const double* R, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!E || !Mx || !My || !Mz || !R) return fail(h, SHASTA_EINVAL, "shasta_set_conserved: NULL field pointer");
+    int rc = ensure_alloc(h);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const double* src[NF] = {E, Mx, My, Mz, R};
+    h->cur = 0;
+    for (int f = 0; f < NF; ++f) {
+        if (h->precision == 64) {
+            CK(cudaMemcpyAsync(h->U[0][f], src[f], sizeof(double) * (size_t)h->ncell, cudaMemcpyDeviceToDevice, st));
+        } else {
+            convert_kernel<double, float><<<ew_grid(h, 256), 256, 0, st>>>(h->ncell, src[f], (float*)h->U[0][f]);
+            CK(cudaGetLastError());
+            h->launches++;
+        }
+    }
+    h->have_state = true;
+    h->prims_valid = false;
+    return 0;
+}
+
+int shasta_get_conserved(shasta_t* h, double* E, double* Mx, double* My, double* Mz, double* R, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_get_conserved: no state set");
+    double* dst[NF] = {E, Mx, My, Mz, R};
+    for (int f = 0; f < NF; ++f)
+        if (dst[f]) {
+            int rc = export_field(h, h->U[h->cur][f], dst[f], (cudaStream_t)stream);
+            if (rc) return rc;
+        }
+    return 0;
+}
+
+int shasta_step(shasta_t* h, int nsteps, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (nsteps < 0) return fail(h, SHASTA_EINVAL, "shasta_step: nsteps < 0");
+    if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_step: call shasta_set_state first");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n[3] = {h->nx, h->ny, h->nz};
+    for (int s = 0; s < nsteps; ++s) {
+        int axes[3], na = 0;
+        for (int k = 0; k < 3; ++k) {
+            const int a = h->table[(3 * h->step + k) % h->ntable];
+            if (n[a] > 1) axes[na++] = a;                 // reading G15: axes of extent 1 are skipped
+        }
+        for (int k = 0; k < na; ++k) {
+            int rc = launch_sweep(h, axes[k], k == na - 1, st);
+            if (rc) return rc;
+        }
+        if (na > 0) h->prims_valid = true;
+        h->step++;
+    }
+    return 0;
+}
+
+int shasta_get_primitives(shasta_t* h, double* e, double* p, double* n, double* vx, double* vy, double* vz,
+                          void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_get_primitives: no state set");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!h->prims_valid) {
+        int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
+        if (rc) return rc;
+    }
+    double* dst[6] = {e, p, n, vx, vy, vz};
+    for (int q = 0; q < 6; ++q)
+        if (dst[q]) {
+            int rc = export_field(h, h->prim[q], dst[q], st);
+            if (rc) return rc;
+        }
+    return 0;
+}
+
+int shasta_get_primitives_host(shasta_t* h, double* e, double* p, double* n, double* vx, double* vy, double* vz,
+                               void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_get_primitives_host: no state set");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!h->prims_valid) {
+        int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
+        if (rc) return rc;
+    }
+    double* dst[6] = {e, p, n, vx, vy, vz};
+    const size_t nb = sizeof(double) * (size_t)h->ncell;
+    for (int q = 0; q < 6; ++q) {
+        if (!dst[q]) continue;
+        if (h->precision == 64) {
+            CK(cudaMemcpyAsync(dst[q], h->prim[q], nb, cudaMemcpyDeviceToHost, st));
+        } else {
+            int rc = ensure_stage(h);
+            if (rc) return rc;
+            double* tmp = h->stage + (size_t)q * h->ncell;
+            rc = export_field(h, h->prim[q], tmp, st);
+            if (rc) return rc;
+            CK(cudaMemcpyAsync(dst[q], tmp, nb, cudaMemcpyDeviceToHost, st));
+        }
+    }
+    return 0;
+}
+
+int shasta_conserved_totals(shasta_t* h, double* totals, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!totals) return fail(h, SHASTA_EINVAL, "shasta_conserved_totals: NULL output");
+    if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_conserved_totals: no state set");
+    cudaStream_t st = (cudaStream_t)stream;
+    void** U = h->U[h->cur];
+    if (h->precision == 64)
+        totals_kernel<double><<<RED_BLOCKS, RED_THREADS, 0, st>>>(h->ncell, (double*)U[0], (double*)U[1],
+            (double*)U[2], (double*)U[3], (double*)U[4], h->d_partial);
+    else
+        totals_kernel<float><<<RED_BLOCKS, RED_THREADS, 0, st>>>(h->ncell, (float*)U[0], (float*)U[1],
+            (float*)U[2], (float*)U[3], (float*)U[4], h->d_partial);
+    CK(cudaGetLastError());
+    h->launches++;
+    CK(cudaMemcpyAsync(h->h_partial, h->d_partial, sizeof(double) * RED_BLOCKS * NF * 2, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const double dv = h->dx * h->dx * h->dx;
+    for (int f = 0; f < NF; ++f) {
+        double s = 0.0, c = 0.0;
+        for (int b = 0; b < RED_BLOCKS; ++b) {
+            const double x = h->h_partial[(b * NF + f) * 2 + 0];
+            const double t = s + x;
+            c += h->h_partial[(b * NF + f) * 2 + 1] + ((fabs(s) >= fabs(x)) ? ((s - t) + x) : ((x - t) + s));
+            s = t;
+        }
+        totals[f] = dv * (s + c);
+    }
+    return 0;
+}
+
+int shasta_diagnostics(shasta_t* h, unsigned long long* counts)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!counts) return fail(h, SHASTA_EINVAL, "shasta_diagnostics: NULL output");
+    if (!h->allocated) { counts[0] = counts[1] = counts[2] = counts[3] = 0; return 0; }
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpy(counts, h->d_counts, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    return 0;
+}
+
+long long shasta_launch_count(const shasta_t* h) { return h ? h->launches : -1; }
+long long shasta_step_index(const shasta_t* h) { return h ? h->step : -1; }
+
+const char* shasta_kernel_name(const shasta_t* h, int axis)
+{
+    if (!h || axis < 0 || axis > 2) return "";
+    return axis == 0 ? "sweep_x_kernel" : "sweep_strided_kernel";
+}
+
+const char* shasta_last_error(const shasta_t* h) { return h ? h->err : g_create_err; }
+
+}  // extern "C"

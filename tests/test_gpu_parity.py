@@ -1,0 +1,235 @@
+"""GPU-vs-oracle parity through the C ABI (-m gpu).  Tolerances (north_star):
+fp64 err_max <= 1e-10 per field (err_L1 reported, expected <= 1e-12); fp32 err_L1 <= 1e-4."""
+import numpy as np
+import pytest
+
+from paper_1206_0919_b200 import inputs
+import parity
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-10
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1206_0919_b200 import build
+    build.build()
+
+
+# ------------------------------------------------------------------ T1: kernel-level parity
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("kind", ["smooth", "rough"])
+def test_single_axis_sweeps_ragged(oracle, axis, bc, kind):
+    # 37x19x23: not a multiple of any tile, warp or chunk size; three sweeps along one axis
+    c = inputs.random_state(37, 19, 23, seed=10 * axis + bc, kind=kind, boundary=bc)
+    ref, o = parity.run_oracle(oracle, c, steps=1, table=[axis] * 3)
+    got, s = parity.run_gpu(c, steps=1, table=[axis] * 3)
+    parity.assert_parity(got, ref, 1e-12, label=f"axis {axis} bc {bc} {kind}")
+    assert abs(s.diagnostics()[0] - o.diagnostics()[0]) <= max(2, o.diagnostics()[0] // 50)
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 50), (1, 40, 1), (64, 1, 1), (5, 1, 9), (2, 3, 4), (3, 3, 3), (130, 2, 1),
+                                   (33, 65, 2)])
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+def test_degenerate_shapes(oracle, shape, bc):
+    nx, ny, nz = shape
+    c = inputs.random_state(nx, ny, nz, seed=nx + ny + nz, kind="rough", boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=3)
+    got, _ = parity.run_gpu(c, steps=3)
+    parity.assert_parity(got, ref, 1e-12, label=f"shape {shape} bc {bc}")
+
+
+@pytest.mark.parametrize("segment", [8, 16, 40, 1000])
+def test_segmentation_does_not_change_the_answer(oracle, segment):
+    c = inputs.random_state(70, 45, 50, seed=77, kind="rough")
+    ref, _ = parity.run_oracle(oracle, c, steps=2)
+    got, _ = parity.run_gpu(c, steps=2, segment=segment)
+    parity.assert_parity(got, ref, 1e-12, label=f"segment {segment}")
+
+
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+def test_general_eos_mass(oracle, bc):
+    c = inputs.random_state(24, 20, 28, seed=4, kind="rough", gamma=5.0 / 3.0, mass=1.0, boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=6)
+    got, _ = parity.run_gpu(c, steps=6)
+    parity.assert_parity(got, ref, 1e-11, label="general EOS")
+
+
+def test_uniform_state_stays_uniform_bitwise():
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    sh = (12, 10, 40)
+    s = Shasta(40, 10, 12, 0.1, 0.4, 4.0 / 3.0)
+    mk = lambda v: torch.full(sh, v, dtype=torch.float64, device="cuda")
+    s.set_state(mk(1.7), mk(0.9), mk(0.3), mk(-0.2), mk(0.5))
+    before = {k: v.clone() for k, v in s.get_conserved().items()}
+    s.step(6)
+    after = s.get_conserved()
+    for k in before:
+        assert torch.equal(before[k], after[k]), k
+
+
+def test_vacuum_and_superluminal_cells(oracle):
+    # E <= 0 cells and |M| > E cells fed through set_conserved: projection + vacuum rule (P13)
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    rng = np.random.default_rng(5)
+    sh = (6, 7, 16)
+    E = rng.uniform(0.5, 2.0, sh); E[2, 3, 4:7] = 0.0; E[4, 1, 9] = -0.1
+    M = [rng.uniform(-0.4, 0.4, sh) for _ in range(3)]
+    M[0][1, 2, 3] = 5.0
+    R = rng.uniform(0.1, 1.0, sh)
+    o = oracle.Oracle(16, 7, 6, 0.1, 0.4, 4.0 / 3.0)
+    o.set_conserved(E, *M, R); o.step(2)
+    s = Shasta(16, 7, 6, 0.1, 0.4, 4.0 / 3.0)
+    s.set_conserved(*[torch.from_numpy(a).cuda() for a in (E, *M, R)]); s.step(2)
+    ref = dict(o.get_conserved()); ref.update(o.get_primitives())
+    got = {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
+    got.update({k: v.cpu().numpy() for k, v in s.get_primitives().items()})
+    parity.assert_parity(got, ref, 1e-11, label="vacuum")
+    assert all(np.all(np.isfinite(v)) for v in got.values())
+
+
+def test_step_split_and_step_index(oracle):
+    c = inputs.random_state(20, 18, 16, seed=3, kind="rough")
+    a, sa = parity.run_gpu(c, steps=7)
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"])
+    s.set_state(*[torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")])
+    s.step(3); s.step(4)
+    assert s.step_index == 7 and sa.step_index == 7
+    for k, v in s.get_conserved().items():
+        assert np.array_equal(v.cpu().numpy(), a[k]), k
+    assert s.launch_count >= 21
+
+
+def test_host_buffer_entry_points(oracle):
+    c = inputs.random_state(21, 17, 13, seed=8, kind="smooth")
+    ref, _ = parity.run_oracle(oracle, c, steps=2)
+    got, _ = parity.run_gpu(c, steps=2, host_io=True)
+    parity.assert_parity(got, ref, 1e-12, label="host io")
+
+
+def test_conserved_totals_periodic(oracle):
+    c = inputs.spherical_riemann(32, steps=12)
+    ref, o = parity.run_oracle(oracle, c)
+    got, s = parity.run_gpu(c)
+    t_ref = o.conserved_totals()
+    t = np.array(s.conserved_totals())
+    assert np.max(np.abs(t - t_ref)) <= 1e-12 * abs(t_ref[0])
+    # conservation on the GPU path itself: E and R to 1e-12 relative
+    s0 = parity.run_gpu(c, steps=0)[1].conserved_totals()
+    assert abs(t[0] - s0[0]) <= 1e-12 * abs(s0[0]) and abs(t[4] - s0[4]) <= 1e-12 * abs(s0[4])
+    assert np.max(np.abs(t[1:4])) <= 1e-12 * abs(s0[0])
+
+
+# ------------------------------------------------------------------ T2: the configs
+def test_config1_shock_tube(oracle):
+    for e_right in (0.01, 1e-8):
+        c = inputs.shock_tube(400, e_right)
+        ref, o = parity.run_oracle(oracle, c)
+        got, s = parity.run_gpu(c)
+        errs = parity.assert_parity(got, ref, TOL64, label=f"config1 eR={e_right}")
+        print("config1", e_right, errs)
+        assert s.diagnostics()[0] == o.diagnostics()[0]
+
+
+def test_config1_along_y_and_z(oracle):
+    for axis in (1, 2):
+        c = inputs.shock_tube(400, 0.01, axis=axis, transverse=3)
+        ref, _ = parity.run_oracle(oracle, c)
+        got, _ = parity.run_gpu(c)
+        parity.assert_parity(got, ref, TOL64, label=f"config1 axis {axis}")
+
+
+def test_config2_fireball(oracle):
+    c = inputs.fireball(64, steps=100)
+    ref, _ = parity.run_oracle(oracle, c)
+    got, _ = parity.run_gpu(c)
+    errs = parity.assert_parity(got, ref, TOL64, label="config2")
+    print("config2", errs)
+
+
+def test_config3_spherical_riemann(oracle):
+    c = inputs.spherical_riemann(128, steps=100)
+    ref, o = parity.run_oracle(oracle, c)
+    got, s = parity.run_gpu(c)
+    errs = parity.assert_parity(got, ref, TOL64, label="config3")
+    print("config3", errs, o.diagnostics(), s.diagnostics())
+    t = np.array(s.conserved_totals())
+    t0 = np.array(parity.run_gpu(c, steps=0)[1].conserved_totals())
+    assert abs(t[0] - t0[0]) <= 1e-12 * t0[0] and abs(t[4] - t0[4]) <= 1e-12 * t0[4]
+    assert np.max(np.abs(t[1:4])) <= 1e-12 * t0[0]
+
+
+def test_config4_hotspots_reduced(oracle):
+    # same box, flow and hotspots on 96^3 for the full 200 steps (the 256^3 run is sampled below)
+    c = inputs.hotspots(96, steps=200)
+    ref, _ = parity.run_oracle(oracle, c)
+    got, _ = parity.run_gpu(c)
+    errs = parity.assert_parity(got, ref, TOL64, label="config4@96")
+    print("config4@96", errs)
+
+
+def test_config4_hotspots_fp32(oracle):
+    c = inputs.hotspots(96, steps=200)
+    ref, _ = parity.run_oracle(oracle, c)
+    got, _ = parity.run_gpu(c, precision=32)
+    errs = parity.field_errors(got, ref)
+    print("config4@96 fp32", errs)
+    for k, (emax, el1) in errs.items():
+        assert el1 <= 1e-4, (k, emax, el1)
+
+
+def test_config4_full_size_sampled(oracle):
+    # 256^3 in the launch configuration bench.py times; the oracle recomputes sampled sub-boxes:
+    # after s steps a cell depends on +-12 s cells... per axis only +-4 s (one sweep per axis per step)
+    steps, w = 6, 16
+    halo = 4 * steps
+    c = inputs.hotspots(256, steps=steps)
+    got, _ = parity.run_gpu(c)
+    rng = np.random.default_rng(1)
+    for _ in range(3):
+        lo = rng.integers(0, 256 - (w + 2 * halo), 3)
+        sl = tuple(slice(l, l + w + 2 * halo) for l in lo)
+        sub = dict(c)
+        for k in ("e", "n", "vx", "vy", "vz"):
+            sub[k] = np.ascontiguousarray(c[k][sl])
+        sub["nx"] = sub["ny"] = sub["nz"] = w + 2 * halo
+        ref, _ = parity.run_oracle(oracle, sub, steps=steps)
+        inner = tuple(slice(halo, halo + w) for _ in range(3))
+        g = {k: v[sl][inner] for k, v in got.items()}
+        r = {k: v[inner] for k, v in ref.items()}
+        # normalise by the global field scale, not the sub-box's
+        for k in r:
+            d = np.abs(g[k] - r[k]).max()
+            scale = np.abs(got[k]).max() if k not in parity.GROUPS else max(np.abs(got[q]).max() for q in parity.GROUPS[k])
+            assert d <= TOL64 * scale, (k, d, scale)
+
+
+def test_config5_slabs_full_size(oracle):
+    # 512^3; uniform in x,y => the oracle is the 1x1x512 column broadcast (pin P11)
+    c1 = inputs.slabs(512, steps=100, nxy=1)
+    ref, _ = parity.run_oracle(oracle, c1)
+    c = inputs.slabs(512, steps=100)
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    s = Shasta(512, 512, 512, c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"])
+    s.set_state(*[torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")])
+    del c
+    s.step(100)
+    cons = s.get_conserved()
+    prim = s.get_primitives()
+    for k, v in list(cons.items()) + list(prim.items()):
+        r = torch.from_numpy(ref[k]).cuda()                       # (512,1,1)
+        if k in parity.GROUPS:
+            scale = max(np.abs(ref[q]).max() for q in parity.GROUPS[k])
+        else:
+            scale = np.abs(ref[k]).max()
+        d = (v - r).abs().max().item()
+        assert d <= TOL64 * max(scale, 1e-300), (k, d, scale)
