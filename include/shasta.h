@@ -87,6 +87,12 @@ int shasta_get_conserved(shasta_t* h, double* E_dev, double* Mx_dev, double* My_
  */
 int shasta_step(shasta_t* h, int nsteps, void* stream);
 
+/* One sweep ("round") along `axis` (0=x,1=y,2=z) by the full dt: the fused kernel of
+ * shasta_step, launched once.  emit_primitives != 0 also writes the primitive fields of the new state (as
+ * the last sweep of a step does).  Does not advance the step counter.  An axis of extent 1 is a no-op
+ * (reading G15).  Used by tests (single-axis parity) and by bench.py to time each kernel with CUDA events. */
+int shasta_sweep(shasta_t* h, int axis, int emit_primitives, void* stream);
+
 /* Primitive fields of the current state (phases 3-4): e = E - |M| v,
  * n = R sqrt(1-v^2), p = EOS(e,n), v = root of v (E + p) = |M|.  Any pointer may be NULL = skip. */
 int shasta_get_primitives(shasta_t* h, double* e_dev, double* p_dev, double* n_dev, double* vx_dev,

@@ -515,6 +515,19 @@ int shasta_step(shasta_t* h, int nsteps, void* stream)
     return 0;
 }
 
+int shasta_sweep(shasta_t* h, int axis, int emit_primitives, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (axis < 0 || axis > 2) return fail(h, SHASTA_EINVAL, "shasta_sweep: axis must be 0, 1 or 2");
+    if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_sweep: call shasta_set_state first");
+    const int n[3] = {h->nx, h->ny, h->nz};
+    if (n[axis] == 1) return 0;
+    int rc = launch_sweep(h, axis, emit_primitives != 0, (cudaStream_t)stream);
+    if (rc) return rc;
+    h->prims_valid = emit_primitives != 0;
+    return 0;
+}
+
 int shasta_get_primitives(shasta_t* h, double* e, double* p, double* n, double* vx, double* vy, double* vz,
                           void* stream)
 {

@@ -85,6 +85,17 @@ def hotspots(n=256, steps=200, seed=SEED):
     return _cfg("hotspots", n, n, n, dx, steps, OUTFLOW, 4.0 / 3.0, 0.0, e, e ** 0.75, 0.0, 0.0, vz)
 
 
+def hotspots_crop(n=96, steps=200, lo=(80, 80, 160), seed=SEED):
+    """Config 4 at its own resolution on a sub-box: the n^3 cells starting at lo=(ix,iy,iz) of the 256^3
+    hotspots state (dx = 0.1 fm).  The default box touches the +z face, where vz = tanh(z/4) reaches
+    gamma = 12, so the outflow boundary is exercised at high Lorentz factor."""
+    c = hotspots(256, steps=steps, seed=seed)
+    sl = (slice(lo[2], lo[2] + n), slice(lo[1], lo[1] + n), slice(lo[0], lo[0] + n))
+    f = {k: np.ascontiguousarray(c[k][sl]) for k in ("e", "n", "vx", "vy", "vz")}
+    return _cfg("hotspots_crop", n, n, n, c["dx"], steps, OUTFLOW, c["gamma"], c["mass"],
+                f["e"], f["n"], f["vx"], f["vy"], f["vz"])
+
+
 def slabs(n=512, steps=100, nxy=None):
     """Config 5: two Woods-Saxon slabs at z=+-6 moving with vz=-+0.9; uniform in x,y
     (nxy=1 gives the 1x1xn column whose broadcast is the full 3D answer, pin P11)."""
@@ -134,5 +145,5 @@ def random_state(nx, ny, nz, seed=0, kind="smooth", vmax=0.6, gamma=4.0 / 3.0, m
 
 CONFIGS = {
     "shock_tube": shock_tube, "fireball": fireball, "spherical_riemann": spherical_riemann,
-    "hotspots": hotspots, "slabs": slabs,
+    "hotspots": hotspots, "hotspots_crop": hotspots_crop, "slabs": slabs,
 }

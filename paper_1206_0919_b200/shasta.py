@@ -19,7 +19,7 @@ BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 # every symbol include/shasta.h declares
 SYMBOLS = (
     "shasta_create", "shasta_destroy", "shasta_set_option", "shasta_set_sweep_table", "shasta_set_state",
-    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_step",
+    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_step", "shasta_sweep",
     "shasta_get_primitives", "shasta_get_primitives_host", "shasta_conserved_totals", "shasta_diagnostics",
     "shasta_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
 )
@@ -48,6 +48,7 @@ def load():
     L.shasta_set_conserved.argtypes = [_vp] + [_dp] * 5 + [_vp]
     L.shasta_get_conserved.argtypes = [_vp] + [_dp] * 5 + [_vp]
     L.shasta_step.argtypes = [_vp, C.c_int, _vp]
+    L.shasta_sweep.argtypes = [_vp, C.c_int, C.c_int, _vp]
     L.shasta_get_primitives.argtypes = [_vp] + [_dp] * 6 + [_vp]
     L.shasta_get_primitives_host.argtypes = [_vp] + [_dp] * 6 + [_vp]
     L.shasta_conserved_totals.argtypes = [_vp, C.POINTER(C.c_double), _vp]
@@ -145,6 +146,10 @@ class Shasta:
 
     def step(self, nsteps=1, stream=None):
         self._chk(self._L.shasta_step(self._h, int(nsteps), _stream_ptr(stream)), "shasta_step")
+
+    def sweep(self, axis, emit_primitives=False, stream=None):
+        self._chk(self._L.shasta_sweep(self._h, int(axis), int(bool(emit_primitives)), _stream_ptr(stream)),
+                  "shasta_sweep")
 
     def get_conserved(self, stream=None):
         import torch
