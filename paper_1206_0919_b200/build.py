@@ -15,6 +15,9 @@ DEPS = SOURCES + [os.path.join(CSRC, "shasta_kernels.cuh"), os.path.join(ROOT, "
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "--use_fast_math=false",
+    # no implicit mul+add contraction: every FMA in the kernels is written out, so that the same formula rounds
+    # the same way in every unrolled phase of the march (a uniform state then stays uniform to the last bit, P10)
+    "-fmad=false",
 ]
 
 

@@ -20,7 +20,7 @@ const int kBranch[18] = {0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2}; 
 
 constexpr int XROWS64 = 128;    // rows per CTA of the x sweep, fp64
 constexpr int XROWS32 = 256;    // fp32
-constexpr int STRIDED_BLOCK = 128;
+constexpr int STRIDED_BLOCK = shk::SBLOCK;
 constexpr int RED_BLOCKS = 592; // 4 per SM
 constexpr int RED_THREADS = 256;
 
@@ -104,6 +104,11 @@ Consts<T> make_consts(const shasta_t* h)
     k.hg = (T)(0.5 * h->gamma);
     k.omd = (T)(1.0 - 1e-12);
     k.mass = (T)h->mass;
+    k.qlam = (T)(0.25 * h->lambda);
+    k.omd2 = (T)((1.0 - 1e-12) * (1.0 - 1e-12));
+    // fast cons2prim path (shasta_kernels.cuh, c2p_fast_y): its frozen-slope Newton converges in two steps while
+    // (Gamma-1)/(2-Gamma) <= 2, i.e. Gamma <= 5/3; above that every cell takes the general path.
+    k.fast = (h->gamma <= 5.0 / 3.0 + 1e-12) ? 1 : 0;
     return k;
 }
 
@@ -135,13 +140,17 @@ __global__ void cons2prim_kernel(long long n, Consts<T> k, const T* E, const T* 
                                  const T* R, T* pe, T* pp, T* pn, T* pvx, T* pvy, T* pvz,
                                  unsigned long long* counts)
 {
+    unsigned lc[4] = {0u, 0u, 0u, 0u};
+    Cnt cnt;
+    cnt.p = lc; cnt.stride = 1;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
         T u[NF] = {E[i], Mx[i], My[i], Mz[i], R[i]};
         T pr[6];
-        primitives<T, EOS>(k, u, pr, counts);
+        emit_primitives<T, EOS>(k, u, pr, cnt);
         pe[i] = pr[0]; pp[i] = pr[1]; pn[i] = pr[2]; pvx[i] = pr[3]; pvy[i] = pr[4]; pvz[i] = pr[5];
     }
+    flush_counts(cnt, counts);
 }
 
 template <typename A, typename B>

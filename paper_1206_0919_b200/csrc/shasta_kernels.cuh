@@ -17,6 +17,13 @@
 // The fields arrive PERMUTED by the host: slot 0 = E, slot 1 = the momentum PARALLEL to the sweep
 // axis (source term lambda*Delta(p)), slots 2,3 = the perpendicular momenta (source
 // free), slot 4 = R.  The kernels therefore never branch on the axis.
+//
+// The kernel is bound by the fp64 pipe (64 results/clk/SM on B200, measured) about as much as by HBM
+// (DESIGN.md 7), so the arithmetic is written for a minimal fp64 instruction count:
+//   * no fp64 division or library sqrt on the common path: MUFU.RCP64H / MUFU.RSQ64H seeds (2^-20,
+//     measured) + Newton steps written out below;
+//   * the flux limiter's min/max/sign run on the integer pipe (sign-magnitude ordering of doubles);
+//   * the register window rotates by NAME (march loop unrolled by 4, compile-time slots), not by moves.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -39,6 +46,9 @@ struct Consts {
     T hg;       // Gamma/2
     T omd;      // 1 - delta, delta = 1e-12 (reading G7)
     T mass;     // m
+    T qlam;     // lambda/4   (predictor source factor 1/2 * lambda/2)
+    T omd2;     // (1 - delta)^2
+    int fast;   // 1: fp64 Gamma-law fast path usable (Gamma <= 5/3), 0: general path for every cell
 };
 
 struct SweepParams {
@@ -55,6 +65,26 @@ struct SweepParams {
     int periodic;           // boundary rule (reading G11)
     unsigned long long* counts;   // diagnostics [4]
 };
+
+// Diagnostics are counted per thread in shared memory (or registers) and flushed once per warp at the end of
+// the kernel: one global atomic per event on a single address serialises in L2 and cost 60 % of the step
+// time once the causality projection fires in ~0.2 % of the cells (profiles/, round 1).
+struct Cnt {
+    unsigned* p;    // this thread's four counters: p[w * stride]
+    int stride;
+    __device__ __forceinline__ void add(int w) const { p[w * stride] += 1u; }
+    __device__ __forceinline__ void zero() const { p[0] = p[stride] = p[2 * stride] = p[3 * stride] = 0u; }
+};
+__device__ __forceinline__ void flush_counts(const Cnt& c, unsigned long long* g)
+{
+    const unsigned mask = __activemask();
+    const int leader = __ffs(mask) - 1;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const unsigned v = __reduce_add_sync(mask, c.p[w * c.stride]);
+        if ((int)(threadIdx.x & 31) == leader && v) atomicAdd(g + w, (unsigned long long)v);
+    }
+}
 
 // reading G11: ghost-extend the INPUT of the sweep: outflow = copy of the edge cell, periodic = wrap
 __device__ __forceinline__ int ghost_index(int j, int N, int periodic)
@@ -79,26 +109,70 @@ template <> __device__ __forceinline__ double t_abs<double>(double a) { return f
 template <> __device__ __forceinline__ float t_abs<float>(float a) { return fabsf(a); }
 
 // ------------------------------------------------------------------------------------------------
+// fp64 seeds: MUFU.RCP64H / MUFU.RSQ64H work on the high word, relative error <= 2^-19.9 (measured
+// on B200); the low word of the result is 0.
+__device__ __forceinline__ double rcp64h(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    return r;
+}
+__device__ __forceinline__ double rsq64h(double x)
+{
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    return r;
+}
+// 1/d for a normal, finite d: seed e0 = 2^-20, one cubic Newton step (e0^3 = 2^-60), 3 DFMA.
+__device__ __forceinline__ double fast_rcp(double d)
+{
+    const double r = rcp64h(d);
+    double e = fma(-d, r, 1.0);
+    e = fma(e, e, e);
+    return fma(r, e, r);
+}
+__device__ __forceinline__ float fast_rcp(float d) { return __frcp_rn(d); }
+// sqrt(w) for a normal w > 0: s0 = w r (2^-20), two Heron steps with the frozen seed r/2 as slope
+// (error e -> e*2^-20 + e^2/2: 2^-40, 2^-60), 6 fp64 ops.
+__device__ __forceinline__ double fast_sqrt(double w)
+{
+    const double r = rsq64h(w);
+    const double hr = 0.5 * r;
+    double s = w * r;
+    s = fma(fma(-s, s, w), hr, s);
+    s = fma(fma(-s, s, w), hr, s);
+    return s;
+}
+__device__ __forceinline__ float fast_sqrt(float w) { return sqrtf(w); }
+
+// ------------------------------------------------------------------------------------------------
 // cons2prim: relativistic correction + EOS (phases 3-4; readings G6-G10).
 // Solves v (E + P(E - Mc v, R sqrt(1-v^2))) = Mc, Mc = min(|M|, (1-delta) E), on [0,1).
+// Results: y with v_i = M_i * y; e; p; w = 1 - v^2 (for n = R sqrt(w)); fl = floor flags.
+//
+// General path (every T, every EOS; also the RARE path of the fp64 Gamma-law kernels):
 //   EOS_GAMMA: closed form v = 2 Mc / (Gamma E + sqrt(Gamma^2 E^2 - 4 (Gamma-1) Mc^2)) (pin P7 ii).
 //   EOS_MASS : Newton with bisection safeguard on the bracket [v(m=0), Mc/E]; the warp leaves the loop
 //              together (__all_sync), so there is no intra-warp divergence in the iteration.
-// Returns vfac such that v_i = M_i * vfac, plus e, p, and v^2 (for n = R sqrt(1-v^2)).
-// The rare clamp branch (|M| > (1-delta) E) is the only data-dependent branch.
+template <typename T>
+struct Prim {
+    T y, e, p, w;
+    int fl;
+};
+
 template <typename T, int EOS>
-__device__ __forceinline__ void cons2prim(const Consts<T>& k, T E, T Ma, T Mb, T Mc, T R,
-                                          T& vfac, T& e, T& p, T& v2, int& floored)
+__device__ __forceinline__ Prim<T> cons2prim_general(const Consts<T>& k, T E, T Ma, T Mb, T Mc, T R)
 {
+    Prim<T> o;
     const bool vac = !(E > T(0));                   // vacuum (reading G7); also catches NaN
     if (vac) { E = T(1); Ma = Mb = Mc = T(0); }     // keep the arithmetic below finite; result discarded
-    floored = 0;
+    o.fl = 0;
     const T M2 = t_fma(Ma, Ma, t_fma(Mb, Mb, Mc * Mc));
     const T lim = k.omd * E;
     const T lim2 = lim * lim;
     T Mq = M2;          // Mc^2 (clamped)
     T s = T(1);         // Mc / |M|
-    if (M2 > lim2) {    // rare: causality clamp, same rule as Pi
+    if (M2 > lim2) {    // causality clamp, same rule as Pi
         Mq = lim2;
         s = lim * t_rsqrt(M2);
     }
@@ -108,11 +182,11 @@ __device__ __forceinline__ void cons2prim(const Consts<T>& k, T E, T Ma, T Mb, T
     T inv = T(1) / hden;                            // v = Mc * inv   (m = 0 root)
     if (EOS == EOS_GAMMA) {
         const T eraw = t_fma(-Mq, inv, E);
-        if (eraw < T(0)) floored |= 1;
-        e = t_max(eraw, T(0));
-        p = k.gm1 * e;
-        v2 = Mq * inv * inv;
-        vfac = s * inv;
+        if (eraw < T(0)) o.fl |= 1;
+        o.e = t_max(eraw, T(0));
+        o.p = k.gm1 * o.e;
+        o.w = t_max(T(1) - Mq * inv * inv, T(0));
+        o.y = s * inv;
     } else {
         const T Mabs = t_sqrt(Mq);
         T lo = Mabs * inv;                          // m = 0 root: lower bound (P_m <= P_0)
@@ -137,17 +211,95 @@ __device__ __forceinline__ void cons2prim(const Consts<T>& k, T E, T Ma, T Mb, T
             const T tol = sizeof(T) == 8 ? T(1e-15) : T(2e-7);
             if (__all_sync(__activemask(), dv <= tol)) break;
         }
-        v2 = v * v;
+        o.w = t_max(t_fma(-v, v, T(1)), T(0));
         const T eraw = t_fma(-Mabs, v, E);
-        if (eraw < T(0)) floored |= 1;
-        e = t_max(eraw, T(0));
-        const T n = R * t_sqrt(t_fma(-v, v, T(1)));
-        const T praw = k.gm1 * (e - k.mass * n);
-        if (praw < T(0)) floored |= 2;
-        p = t_max(praw, T(0));
-        vfac = (M2 > T(0)) ? v * t_rsqrt(M2) : T(0);
+        if (eraw < T(0)) o.fl |= 1;
+        o.e = t_max(eraw, T(0));
+        const T n = R * t_sqrt(o.w);
+        const T praw = k.gm1 * (o.e - k.mass * n);
+        if (praw < T(0)) o.fl |= 2;
+        o.p = t_max(praw, T(0));
+        o.y = (M2 > T(0)) ? v * t_rsqrt(M2) : T(0);
     }
-    if (vac) { vfac = T(0); e = T(0); p = T(0); v2 = T(0); floored = 0; }
+    if (vac) { o.y = T(0); o.e = T(0); o.p = T(0); o.w = T(0); o.fl = 0; }   // n = R sqrt(w) = 0 (reading G7)
+    return o;
+}
+
+// out-of-line copy for the rare cells of the fp64 Gamma-law kernels (keeps the march loop small)
+__device__ __noinline__ Prim<double> cons2prim_rare(const Consts<double>& k, double E, double Ma, double Mb,
+                                                    double Mc, double R)
+{
+    return cons2prim_general<double, EOS_GAMMA>(k, E, Ma, Mb, Mc, R);
+}
+
+// Only vacuum / non-positive E (high word <= 0; also -0, NaN with the sign set) leaves the fast path for the
+// out-of-line general routine.  The causality clamp Mc = min(|M|, (1-delta) E) stays inline: Mc^2 is a
+// select on the bit patterns (non-negative doubles order like integers), and only a clamped cell (~0.2 % of
+// the cells of config 4) pays the extra rsqrt for the direction-preserving scale factor.
+__device__ __forceinline__ bool c2p_is_vacuum(const Consts<double>& k, double E)
+{
+    return (__double2hiint(E) <= 0) | (k.fast == 0);
+}
+__device__ __forceinline__ bool gt_nonneg(double a, double b)      // a > b for a, b >= 0, on the integer pipe
+{
+    return __double_as_longlong(a) > __double_as_longlong(b);
+}
+// 1/sqrt(x), normal x > 0: seed 2^-20, two Newton steps (only on the clamped branch)
+__device__ __forceinline__ double fast_rsqrt(double x)
+{
+    double r = rsq64h(x);
+    r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
+    r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
+    return r;
+}
+
+// Fast path, fp64, p = (Gamma-1) e.  y = 1/h, h = (b + sqrt(disc))/2 with b = Gamma E, disc = b^2 - 4 c,
+// c = (Gamma-1)|M|^2, is the smaller root of f(y) = c y^2 - b y + 1 and f'(y*) = -sqrt(disc).  Seeds:
+// r = rsq64h(disc) ~ 1/sqrt(disc), y0 = 2 rcp64h(disc r + b) (both 2^-20); Newton with the FROZEN slope r:
+// y <- y + f(y) r.  Error e -> e 2^-20 + (c y/sqrt(disc)) e^2 with c y/sqrt(disc) <= (Gamma-1)/(2-Gamma)
+// (= 1/2 for Gamma = 4/3): 2^-20 -> 2^-39 -> 2^-58.  15 fp64 ops including |M|^2, no division, no sqrt.
+__device__ __forceinline__ double c2p_fast_y(const Consts<double>& k, double E, double M2, double t)
+{
+    const double disc = fma(k.g2, t, -(k.c4 * M2));
+    const double r = rsq64h(disc);
+    const double b = k.gam * E;
+    const double s = fma(disc, r, b);
+    const double y0 = rcp64h(s);
+    double y = __hiloint2double(__double2hiint(y0) + 0x00100000, 0);      // 2 * y0 (exponent + 1)
+    const double c = k.gm1 * M2;
+    y = fma(fma(fma(c, y, -b), y, 1.0), r, y);
+    y = fma(fma(fma(c, y, -b), y, 1.0), r, y);
+    return y;
+}
+
+// In-sweep cons2prim (S1, S3): only v_par = M_par y and p are needed.
+template <typename T, int EOS>
+__device__ __forceinline__ void c2p_sweep(const Consts<T>& k, const T (&u)[NF], T& v, T& p)
+{
+    const Prim<T> o = cons2prim_general<T, EOS>(k, u[0], u[1], u[2], u[3], u[4]);
+    v = u[1] * o.y;
+    p = o.p;
+}
+template <>
+__device__ __forceinline__ void c2p_sweep<double, EOS_GAMMA>(const Consts<double>& k, const double (&u)[NF],
+                                                             double& v, double& p)
+{
+    const double M2 = fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3]));
+    double y, e;
+    if (c2p_is_vacuum(k, u[0])) {
+        const Prim<double> o = cons2prim_rare(k, u[0], u[1], u[2], u[3], u[4]);
+        y = o.y; e = o.e;
+    } else {
+        const double t = u[0] * u[0];
+        const double lim2 = k.omd2 * t;
+        const bool clamped = gt_nonneg(M2, lim2);
+        const double Mq = clamped ? lim2 : M2;
+        y = c2p_fast_y(k, u[0], Mq, t);
+        e = fma(-Mq, y, u[0]);          // e = E - Mc v >= delta E > 0: no floor
+        if (clamped) y *= (k.omd * u[0]) * fast_rsqrt(M2);
+    }
+    v = u[1] * y;
+    p = k.gm1 * e;
 }
 
 // eq. (21) branch-free (reading G12): A = sigma max(0, min(sigma D^_{j+1}, |A^ph|, sigma D^_{j-1}))
@@ -158,193 +310,237 @@ __device__ __forceinline__ T limiter(T aph, T dhp, T dhm)
     const T m = t_min(t_min(sg * dhp, t_abs(aph)), sg * dhm);
     return sg * t_max(m, T(0));
 }
+// fp64 on the INTEGER pipe: multiplying by sigma = flipping the sign bit; IEEE doubles order like
+// sign-magnitude integers, so min over non-negative doubles = min over their bit patterns as signed
+// 64-bit integers, and any negative operand makes that integer minimum negative, which max(.,0)
+// clips to +0 -- exactly the max{0, min{...}} of eq. (21).  No fp64-pipe instruction.
+template <>
+__device__ __forceinline__ double limiter<double>(double aph, double dhp, double dhm)
+{
+    const long long ia = __double_as_longlong(aph);
+    const long long sg = ia & (long long)0x8000000000000000ULL;
+    const long long z = ia ^ sg;
+    const long long x = __double_as_longlong(dhp) ^ sg;
+    const long long y = __double_as_longlong(dhm) ^ sg;
+    long long m = min(min(x, z), y);
+    if ((int)(m >> 32) < 0) m = 0;
+    return __longlong_as_double(m ^ sg);
+}
 
 // ------------------------------------------------------------------------------------------------
-// The rolling window of one marching thread.  Index names: member "x<k>" holds the quantity at cell
-// (or interface) i-k where i is the front cell of the CURRENT step.
+// The rolling window of one marching thread.  "X_k" below means the quantity at cell (or interface)
+// i-k, where i is the front cell of the CURRENT step.  Each window is a small ring whose slot is a
+// compile-time function of the phase PH = (step number) mod 4: the march loop is unrolled by 4, so
+// every slot is a fixed register and the window advances without a single move instruction.
 template <typename T, int EOS>
 struct Marcher {
-    T u1[NF], u2[NF];                       // U^n_{i-1}, U^n_{i-2}
-    T dl2[NF], dl3[NF], dl4[NF], dl5[NF];   // Delta_{i-2..i-5}, eq. (16)
-    T ft[NF];                               // predictor flux F~ at interface (i-2,i-1)
-    T fc[NF];                               // corrector flux F at interface (i-3,i-2)
-    T uh3[NF], uh4[NF];                     // U^_{i-3}, U^_{i-4}
-    T dh4[NF], dh5[NF];                     // D^_{i-4}, D^_{i-5}, eq. (18)
-    T a5[NF];                               // limited antidiffusive flux A_{i-5}
-    T eps1, fE1, fE2, fM1, fM2;             // time-n: (lambda/2) v_{i-1}, (p v)_{i-1,i-2}, p_{i-1,i-2}
-    T epsh2, gE2, gE3, gM2, gM3;            // half step: lambda v_{i-2}, (p v)_{i-2,i-3}, p_{i-2,i-3}
+    T u[2][NF];         // U^n_1, U^n_2                    slot of U^n_k : (PH-k)&1
+    T dl[4][NF];        // Delta_2..Delta_5, eq. (16)      slot of Delta_k: (PH-k)&3
+    T ft[NF];           // predictor flux F~ at interface (i-2,i-1)
+    T fc[NF];           // corrector flux F at interface (i-3,i-2)
+    T uh[2][NF];        // U^_3, U^_4                      slot of U^_k : (PH-k)&1
+    T dh[2][NF];        // D^_4, D^_5, eq. (18)            slot of D^_k : (PH-k)&1
+    T a5[NF];           // limited antidiffusive flux A_5
+    T eps1;             // (lambda/2) v_1 (time n)
+    T fE[2], fM[2];     // (p v)_1,_2 and p_1,_2 (time n)  slot (PH-k)&1
+    T epsh2;            // lambda v^{1/2}_2
+    T gE[2], gM[2];     // (p v)^{1/2}_2,_3 and p^{1/2}_2,_3   slot (PH-k)&1
 
     __device__ __forceinline__ void init()
     {
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-            u1[f] = u2[f] = dl2[f] = dl3[f] = dl4[f] = dl5[f] = ft[f] = fc[f] = T(0);
-            uh3[f] = uh4[f] = dh4[f] = dh5[f] = a5[f] = T(0);
+            u[0][f] = u[1][f] = dl[0][f] = dl[1][f] = dl[2][f] = dl[3][f] = ft[f] = fc[f] = T(0);
+            uh[0][f] = uh[1][f] = dh[0][f] = dh[1][f] = a5[f] = T(0);
         }
-        eps1 = fE1 = fE2 = fM1 = fM2 = epsh2 = gE2 = gE3 = gM2 = gM3 = T(0);
+        eps1 = epsh2 = fE[0] = fE[1] = fM[0] = fM[1] = gE[0] = gE[1] = gM[0] = gM[1] = T(0);
     }
 
     // One march step: consumes U^n at the front cell, produces U^{n+1} of cell i-4 in un[].
+    template <int PH>
     __device__ __forceinline__ void step(const Consts<T>& k, const T (&u0)[NF], T (&un)[NF])
     {
+        constexpr int U1 = (PH + 3) & 1, U2 = (PH + 2) & 1;                 // U^n_1, U^n_2 (new U^n_0 -> U2)
+        constexpr int D2 = (PH + 2) & 3, D3 = (PH + 1) & 3, D4 = PH & 3, D5 = (PH + 3) & 3;   // new Delta_1 -> D5
+        constexpr int H3 = (PH + 1) & 1, H4 = PH & 1;                       // U^_3, U^_4 (new U^_2 -> H4)
+        constexpr int E4 = PH & 1, E5 = (PH + 1) & 1;                       // D^_4, D^_5 (new D^_3 -> E5)
+        constexpr int S1 = (PH + 1) & 1, S2 = PH & 1;                       // time-n scalars _1,_2 (new _0 -> S2)
+        constexpr int G2 = PH & 1, G3 = (PH + 1) & 1;                       // half-step scalars _2,_3 (new _1 -> G3)
+        (void)S1; (void)G2;
         // S1: time-n primitives of the front cell
-        T vf0, e0, p0, v20;
-        int fl;
-        cons2prim<T, EOS>(k, u0[0], u0[1], u0[2], u0[3], u0[4], vf0, e0, p0, v20, fl);
-        const T v0 = u0[1] * vf0;
+        T v0, p0;
+        c2p_sweep<T, EOS>(k, u0, v0, p0);
         const T eps0 = k.hlam * v0;
         const T fE0 = p0 * v0;
         // S2: predictor (half step, no antidiffusion: reading G4), interface (i-1,i), cell i-1
         T ut[NF], dl1[NF];
         {
-            const T q = (T(0.5) - eps1) / (T(1) + (eps0 - eps1));   // Q+_{i-1}, eq. (15); Q-_i = 1-q (P1)
-            const T a = T(0.5) - q, b = T(0.5) * q * q;
+            const T q = (T(0.5) - eps1) * fast_rcp(T(1) + (eps0 - eps1));   // Q+_1, eq. (15); Q-_0 = 1-q (P1)
+            const T a = T(0.5) - q, b = (T(0.5) * q) * q;
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
-                dl1[f] = u0[f] - u1[f];                             // eq. (16)
-                const T fl = t_fma(a, u1[f], -b * dl1[f]);          // F = (1/2-q) U - 1/2 q^2 Delta (P2)
-                ut[f] = (u1[f] - fl) + ft[f];
+                dl1[f] = u0[f] - u[U1][f];                                  // eq. (16)
+                const T fl = t_fma(a, u[U1][f], -(b * dl1[f]));             // F = (1/2-q) U - 1/2 q^2 Delta (P2)
+                ut[f] = u[U1][f] - (fl - ft[f]);                               // exact no-op on uniform data (P10)
                 ft[f] = fl;
             }
-            ut[0] = t_fma(T(-0.5) * k.hlam, fE0 - fE2, ut[0]);      // + (lambda/2) Delta(p v)
-            ut[1] = t_fma(T(-0.5) * k.hlam, p0 - fM2, ut[1]);       // + (lambda/2) Delta(p)
+            ut[0] = t_fma(-k.qlam, fE0 - fE[S2], ut[0]);                    // + (lambda/2) Delta(p v)
+            ut[1] = t_fma(-k.qlam, p0 - fM[S2], ut[1]);                     // + (lambda/2) Delta(p)
         }
         // S3: half-step primitives of cell i-1
-        T vfh, eh, ph, v2h;
-        cons2prim<T, EOS>(k, ut[0], ut[1], ut[2], ut[3], ut[4], vfh, eh, ph, v2h, fl);
-        const T vh1 = ut[1] * vfh;
+        T vh1, ph;
+        c2p_sweep<T, EOS>(k, ut, vh1, ph);
         const T epsh1 = k.lam * vh1;
         const T gE1 = ph * vh1;
         // S4: corrector transport of U^n, interface (i-2,i-1), cell i-2
         T uh2[NF];
         {
-            const T q = (T(0.5) - epsh2) / (T(1) + (epsh1 - epsh2));
-            const T a = T(0.5) - q, b = T(0.5) * q * q;
+            const T q = (T(0.5) - epsh2) * fast_rcp(T(1) + (epsh1 - epsh2));
+            const T a = T(0.5) - q, b = (T(0.5) * q) * q;
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
-                const T fl = t_fma(a, u2[f], -b * dl2[f]);
-                uh2[f] = (u2[f] - fl) + fc[f];
+                const T fl = t_fma(a, u[U2][f], -(b * dl[D2][f]));
+                uh2[f] = u[U2][f] - (fl - fc[f]);
                 fc[f] = fl;
             }
-            uh2[0] = t_fma(T(-0.5) * k.lam, gE1 - gE3, uh2[0]);     // + lambda Delta(p v)^{n+1/2}
-            uh2[1] = t_fma(T(-0.5) * k.lam, ph - gM3, uh2[1]);      // + lambda Delta(p)^{n+1/2}
+            uh2[0] = t_fma(-k.hlam, gE1 - gE[G3], uh2[0]);                  // + lambda Delta(p v)^{n+1/2}
+            uh2[1] = t_fma(-k.hlam, ph - gM[G3], uh2[1]);                   // + lambda Delta(p)^{n+1/2}
         }
         // S5+S6: antidiffusion at interface (i-4,i-3), update of cell i-4
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-            const T dh3 = uh2[f] - uh3[f];                                       // eq. (18)
-            const T d2 = (dl3[f] + dl5[f]) - T(2) * dl4[f];                      // reading G14
-            const T aph = T(0.125) * (dh4[f] - T(0.125) * d2);                   // eq. (19)
-            const T a4 = limiter<T>(aph, dh3, dh5[f]);                           // eqs. (20),(21)
-            un[f] = (uh4[f] - a4) + a5[f];                                       // eq. (22)
-            // shift the window
+            const T dh3 = uh2[f] - uh[H3][f];                                    // eq. (18)
+            const T d2 = t_fma(T(-2), dl[D4][f], dl[D3][f] + dl[D5][f]);         // reading G14
+            const T aph = T(0.125) * t_fma(T(-0.125), d2, dh[E4][f]);            // eq. (19)
+            const T a4 = limiter<T>(aph, dh3, dh[E5][f]);                        // eqs. (20),(21)
+            un[f] = uh[H4][f] - (a4 - a5[f]);                                    // eq. (22)
+            // advance the window: the new values take the slots of the oldest ones
             a5[f] = a4;
-            dh5[f] = dh4[f]; dh4[f] = dh3;
-            uh4[f] = uh3[f]; uh3[f] = uh2[f];
-            dl5[f] = dl4[f]; dl4[f] = dl3[f]; dl3[f] = dl2[f]; dl2[f] = dl1[f];
-            u2[f] = u1[f]; u1[f] = u0[f];
+            dh[E5][f] = dh3;
+            uh[H4][f] = uh2[f];
+            dl[D5][f] = dl1[f];
+            u[U2][f] = u0[f];
         }
-        eps1 = eps0; fE2 = fE1; fE1 = fE0; fM2 = fM1; fM1 = p0;
-        epsh2 = epsh1; gE3 = gE2; gE2 = gE1; gM3 = gM2; gM2 = ph;
+        eps1 = eps0; fE[S2] = fE0; fM[S2] = p0;
+        epsh2 = epsh1; gE[G3] = gE1; gM[G3] = ph;
     }
 };
 
 // Pi, readings G6-G8: written back to M at the end of every sweep.  E and R are never modified.
 template <typename T>
-__device__ __forceinline__ void project(const Consts<T>& k, T (&un)[NF], unsigned long long* counts)
+__device__ __forceinline__ void project(const Consts<T>& k, T (&un)[NF], Cnt counts)
 {
     const T E = un[0];
     const T M2 = t_fma(un[1], un[1], t_fma(un[2], un[2], un[3] * un[3]));
     const T lim = k.omd * E;
     if (!(E > T(0))) {
         un[1] = un[2] = un[3] = T(0);
-        atomicAdd(counts + 1, 1ULL);
+        counts.add(1);
     } else if (M2 > lim * lim) {
         const T s = lim * t_rsqrt(M2);
         un[1] *= s; un[2] *= s; un[3] *= s;
-        atomicAdd(counts + 0, 1ULL);
+        counts.add(0);
     }
 }
 
 // primitives of one cell from its (projected) conserved state, slots permuted like the momenta
 template <typename T, int EOS>
 __device__ __forceinline__ void primitives(const Consts<T>& k, const T (&u)[NF], T (&pr)[6],
-                                           unsigned long long* counts)
+                                           Cnt counts)
 {
-    T vf, e, p, v2;
-    int fl;
-    cons2prim<T, EOS>(k, u[0], u[1], u[2], u[3], u[4], vf, e, p, v2, fl);
-    pr[0] = e; pr[1] = p;
-    pr[2] = u[4] * t_sqrt(t_max(T(1) - v2, T(0)));
-    pr[3] = u[1] * vf; pr[4] = u[2] * vf; pr[5] = u[3] * vf;
-    if (fl) {                                       // rare: diagnostics [2] e floored, [3] p floored
-        if (fl & 1) atomicAdd(counts + 2, 1ULL);
-        if (fl & 2) atomicAdd(counts + 3, 1ULL);
+    const Prim<T> o = cons2prim_general<T, EOS>(k, u[0], u[1], u[2], u[3], u[4]);
+    pr[0] = o.e; pr[1] = o.p;
+    pr[2] = u[4] * t_sqrt(o.w);
+    pr[3] = u[1] * o.y; pr[4] = u[2] * o.y; pr[5] = u[3] * o.y;
+    if (o.fl) {                                     // rare: diagnostics [2] e floored, [3] p floored
+        if (o.fl & 1) counts.add(2);
+        if (o.fl & 2) counts.add(3);
     }
 }
 
-// ------------------------------------------------------------------------------------------------
-// Sweep along y or z: lanes run along the contiguous x axis, so every load and store of a warp is a
-// coalesced 256 B (fp64) row piece; no shared memory is needed.  Work item = (pencil, segment).
+__device__ __noinline__ void finish_rare(const Consts<double>& k, double (&un)[NF], double (&pr)[6], int emit,
+                                         Cnt counts)
+{
+    project<double>(k, un, counts);
+    if (emit) primitives<double, EOS_GAMMA>(k, un, pr, counts);
+}
+
+// S6 tail + S7 of one output cell: Pi on un[], and (EMIT) its primitives pr[].
 template <typename T, int EOS, bool EMIT>
-__global__ void __launch_bounds__(128) sweep_strided_kernel(SweepParams P, Consts<T> k)
+__device__ __forceinline__ void finish_cell(const Consts<T>& k, T (&un)[NF], T (&pr)[6], Cnt counts)
 {
-    const long long pen = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (pen >= P.npencil) return;
-    const int sg = blockIdx.y;
-    const int j0 = sg * P.seg;
-    const int j1 = min(P.N, j0 + P.seg);
-    const long long base = (pen % P.nx) + (pen / P.nx) * P.stride_other;
-    const long long sa = P.stride_axis;
-    const T* __restrict__ in[NF];
-    T* __restrict__ out[NF];
-#pragma unroll
-    for (int f = 0; f < NF; ++f) { in[f] = (const T*)P.in[f] + base; out[f] = (T*)P.out[f] + base; }
-
-    Marcher<T, EOS> m;
-    m.init();
-    T nxt[NF];
-    {
-        const long long o = (long long)ghost_index(j0 - GH, P.N, P.periodic) * sa;
-#pragma unroll
-        for (int f = 0; f < NF; ++f) nxt[f] = __ldg(in[f] + o);
-    }
-    for (int i = j0 - GH; i < j1 + GH; ++i) {
-        T u0[NF], un[NF];
-#pragma unroll
-        for (int f = 0; f < NF; ++f) u0[f] = nxt[f];
-        if (i + 1 < j1 + GH) {                           // prefetch the next front cell
-            const long long o = (long long)ghost_index(i + 1, P.N, P.periodic) * sa;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) nxt[f] = __ldg(in[f] + o);
-        }
-        m.step(k, u0, un);
-        const int jo = i - GH;
-        if (jo >= j0) {
-            project<T>(k, un, P.counts);
-            const long long o = (long long)jo * sa;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) out[f][o] = un[f];
-            if (EMIT) {
-                T pr[6];
-                primitives<T, EOS>(k, un, pr, P.counts);
-#pragma unroll
-                for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[base + o] = pr[q];
-            }
-        }
-    }
+    project<T>(k, un, counts);
+    if (EMIT) primitives<T, EOS>(k, un, pr, counts);
+}
+// fp64 Gamma-law: Pi and the primitives share |M|^2 and E^2; everything but vacuum is inline.
+// primitives from (E, Mc^2, E^2) on the fast path: y 12 ops, e/w 3, sqrt 6, n/p/v 5
+__device__ __forceinline__ void prims_fast(const Consts<double>& k, const double (&u)[NF], double Mq, double t,
+                                           double s, double (&pr)[6])
+{
+    double y = c2p_fast_y(k, u[0], Mq, t);
+    const double e = fma(-Mq, y, u[0]);
+    const double w = fma(-(Mq * y), y, 1.0);
+    y *= s;
+    pr[0] = e;
+    pr[1] = k.gm1 * e;
+    pr[2] = u[4] * fast_sqrt(w);
+    pr[3] = u[1] * y; pr[4] = u[2] * y; pr[5] = u[3] * y;
 }
 
-// ------------------------------------------------------------------------------------------------
-// Sweep along x (the contiguous axis): a CTA owns ROWS rows; thread r marches along row r.  The rows
-// are staged through shared memory in chunks of CH cells per row (cp.async, double buffered) so that
-// global traffic stays coalesced (64 B row pieces) while each thread reads its own row conflict-free
-// (row pitch CH+1: odd).  Results go to an output tile and are written back coalesced; the primitives
-// of the last sweep are computed element-wise during that write-back.
-constexpr int XCH = 8;            // cells per row per chunk
-constexpr int XPITCH = XCH + 1;   // odd pitch: conflict-free column access for 8 B elements
-constexpr int XNS = 2;            // input stages
+template <bool EMIT>
+__device__ __forceinline__ void finish_cell_fast(const Consts<double>& k, double (&un)[NF], double (&pr)[6],
+                                                 Cnt counts)
+{
+    if (c2p_is_vacuum(k, un[0])) {
+        finish_rare(k, un, pr, EMIT ? 1 : 0, counts);
+        return;
+    }
+    double M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
+    const double t = un[0] * un[0];
+    const double lim2 = k.omd2 * t;
+    double s = 1.0;
+    if (gt_nonneg(M2, lim2)) {                          // Pi fires: scale M onto |M| = (1-delta) E
+        const double sc = (k.omd * un[0]) * fast_rsqrt(M2);
+        un[1] *= sc; un[2] *= sc; un[3] *= sc;
+        counts.add(0);
+        if (EMIT) {                                     // primitives of the PROJECTED state, like the oracle
+            M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
+            if (gt_nonneg(M2, lim2)) s = (k.omd * un[0]) * fast_rsqrt(M2);
+        }
+    }
+    if (EMIT) prims_fast(k, un, gt_nonneg(M2, lim2) ? lim2 : M2, t, s, pr);
+}
+template <> __device__ __forceinline__ void finish_cell<double, EOS_GAMMA, true>(
+    const Consts<double>& k, double (&un)[NF], double (&pr)[6], Cnt counts)
+{ finish_cell_fast<true>(k, un, pr, counts); }
+template <> __device__ __forceinline__ void finish_cell<double, EOS_GAMMA, false>(
+    const Consts<double>& k, double (&un)[NF], double (&pr)[6], Cnt counts)
+{ finish_cell_fast<false>(k, un, pr, counts); }
 
+// primitives of an already projected cell (x sweep write-back): fast path + rare fallback
+template <typename T, int EOS>
+__device__ __forceinline__ void emit_primitives(const Consts<T>& k, const T (&u)[NF], T (&pr)[6],
+                                                Cnt counts)
+{
+    primitives<T, EOS>(k, u, pr, counts);
+}
+template <>
+__device__ __forceinline__ void emit_primitives<double, EOS_GAMMA>(const Consts<double>& k, const double (&u)[NF],
+                                                                   double (&pr)[6], Cnt counts)
+{
+    if (c2p_is_vacuum(k, u[0])) {
+        primitives<double, EOS_GAMMA>(k, u, pr, counts);
+        return;
+    }
+    const double M2 = fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3]));
+    const double t = u[0] * u[0];
+    const double lim2 = k.omd2 * t;
+    const bool clamped = gt_nonneg(M2, lim2);
+    const double s = clamped ? (k.omd * u[0]) * fast_rsqrt(M2) : 1.0;
+    prims_fast(k, u, clamped ? lim2 : M2, t, s, pr);
+}
+
+// cp.async (LDGSTS) helpers: one element per thread, global -> shared without touching registers
 template <typename T>
 __device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc)
 {
@@ -357,20 +553,153 @@ __device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
+// ------------------------------------------------------------------------------------------------
+// Sweep along y or z: lanes run along the contiguous x axis, so every load and store of a warp is a
+// coalesced 256 B (fp64) row piece.  Work item = (pencil, segment).  The marching thread is latency-
+// bound unless many cells are in flight per pencil, and registers are full (the window), so the input
+// is PREFETCHED SD-1 cells ahead with cp.async into a per-thread ring in shared memory
+// (ring[slot][field][thread]: conflict-free).  A thread only ever reads what it copied itself:
+// cp.async.wait_group is the only synchronisation.
+constexpr int SD = 8;             // ring slots = cells in flight per pencil + 1
+constexpr int SBLOCK = 128;       // threads per CTA
+
+template <typename T>
+struct StridedCtx {
+    const T* in[NF];
+    T* out[NF];
+    T* prim[6];
+    long long sa;       // element stride along the sweep axis
+    int N, periodic, j0, j1;
+    int ipf, jpf;       // next cell to prefetch: true index and ghost-mapped index (reading G11)
+    Cnt counts;
+};
+
+// issue the copy of the next cell into ring slot `slot`; one commit group per cell
+template <typename T>
+__device__ __forceinline__ void strided_prefetch(StridedCtx<T>& c, T* slot)
+{
+    const long long o = (long long)c.jpf * c.sa;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) cp_async_elem<T>(slot + f * SBLOCK, c.in[f] + o);
+    cp_async_commit();
+    c.ipf += 1;
+    if (c.periodic) { c.jpf = (c.jpf + 1 == c.N) ? 0 : c.jpf + 1; }     // wrap
+    else            { c.jpf = min(max(c.ipf, 0), c.N - 1); }            // copy of the edge cell
+}
+
+// PH = step number mod 4 (compile time: window phase and ring slot inside the current half of the ring);
+// cur / oth = the two halves (4 slots each) of this thread's ring, swapped every 4 steps by the caller.
+template <typename T, int EOS, bool EMIT, int PH>
+__device__ __forceinline__ void strided_substep(Marcher<T, EOS>& m, const Consts<T>& k, StridedCtx<T>& c, int i,
+                                                T* cur, T* oth)
+{
+    // refill the slot consumed by the PREVIOUS step (its reads are long retired), then wait for cell i
+    strided_prefetch<T>(c, PH == 0 ? oth + 3 * NF * SBLOCK : cur + (PH - 1) * NF * SBLOCK);
+    cp_async_wait<SD - 1>();
+    T u0[NF], un[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) u0[f] = cur[(PH * NF + f) * SBLOCK];
+    m.template step<PH>(k, u0, un);
+    const int jo = i - GH;
+    if (jo >= c.j0 && jo < c.j1) {
+        T pr[6];
+        finish_cell<T, EOS, EMIT>(k, un, pr, c.counts);
+        const long long o = (long long)jo * c.sa;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) c.out[f][o] = un[f];
+        if (EMIT) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) c.prim[q][o] = pr[q];
+        }
+    }
+}
+
+template <typename T, int EOS, bool EMIT>
+__global__ void __launch_bounds__(SBLOCK) sweep_strided_kernel(SweepParams P, Consts<T> k)
+{
+    __shared__ T ring[SD * NF * SBLOCK];
+    __shared__ unsigned cnt[4 * SBLOCK];
+    const long long pen = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pen >= P.npencil) return;
+    const int sg = blockIdx.y;
+    StridedCtx<T> c;
+    c.j0 = sg * P.seg;
+    c.j1 = min(P.N, c.j0 + P.seg);
+    c.N = P.N; c.periodic = P.periodic; c.sa = P.stride_axis;
+    c.counts.p = cnt + threadIdx.x; c.counts.stride = SBLOCK;
+    c.counts.zero();
+    const long long base = (pen % P.nx) + (pen / P.nx) * P.stride_other;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { c.in[f] = (const T*)P.in[f] + base; c.out[f] = (T*)P.out[f] + base; }
+#pragma unroll
+    for (int q = 0; q < 6; ++q) c.prim[q] = (T*)P.prim[q] + base;
+
+    Marcher<T, EOS> m;
+    m.init();
+    c.ipf = c.j0 - GH;
+    c.jpf = ghost_index(c.ipf, P.N, P.periodic);
+    T* cur = ring + threadIdx.x;
+    T* oth = cur + 4 * NF * SBLOCK;
+#pragma unroll
+    for (int d = 0; d < SD - 1; ++d) strided_prefetch<T>(c, cur + d * NF * SBLOCK);      // cells j0-4 .. j0+2
+    // front cells j0-4 .. j1+3, rounded up to a multiple of 4 steps (the surplus steps store nothing)
+    for (int i = c.j0 - GH; i < c.j1 + GH; i += 4) {
+        strided_substep<T, EOS, EMIT, 0>(m, k, c, i, cur, oth);
+        strided_substep<T, EOS, EMIT, 1>(m, k, c, i + 1, cur, oth);
+        strided_substep<T, EOS, EMIT, 2>(m, k, c, i + 2, cur, oth);
+        strided_substep<T, EOS, EMIT, 3>(m, k, c, i + 3, cur, oth);
+        T* tmp = cur; cur = oth; oth = tmp;
+    }
+    cp_async_wait<0>();
+    flush_counts(c.counts, P.counts);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Sweep along x (the contiguous axis): a WARP owns 32 rows; lane r marches along row r.  The rows
+// are staged through shared memory in chunks of XCH cells per row (cp.async, double buffered) so that
+// global traffic stays coalesced (64 B row pieces) while each thread reads its own row conflict-free
+// (row pitch XCH+1: odd).  The result of cell i-4 is written IN PLACE over the slot of the front cell i
+// just consumed, so a chunk buffer holds the inputs [8c, 8c+8) before and the outputs [8c-4, 8c+4)
+// after its march; the write-back is coalesced (the primitives of the last sweep are computed element-wise there).
+constexpr int XCH = 8;            // cells per row per chunk
+constexpr int XPITCH = XCH + 1;   // odd pitch: conflict-free column access for 8 B elements
+constexpr int XNS = 2;            // stages
+
+constexpr int XW = 32;            // rows per warp: every warp runs its own pipeline, no CTA barrier
+
 template <typename T, int ROWS>
 struct XSmem {
-    T in[XNS][NF][ROWS * XPITCH];
-    T out[NF][ROWS * XPITCH];
+    T buf[ROWS / XW][XNS][NF][XW * XPITCH];
+    unsigned cnt[4][ROWS];
 };
+
+template <typename T, int EOS, int PH>
+__device__ __forceinline__ void x_substep(Marcher<T, EOS>& m, const Consts<T>& k, T* sb, int i, int ilo, int ihi,
+                                          int j0, Cnt counts)
+{
+    // sb = &buf[warp][stage][0][lane * XPITCH + 4 h]: column 4 h + PH of the chunk; window phase = PH
+    if (i < ilo || i >= ihi) return;
+    T u0[NF], un[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) u0[f] = sb[f * (XW * XPITCH) + PH];
+    m.template step<PH>(k, u0, un);
+    if (i - GH >= j0) {
+        T pr[6];
+        finish_cell<T, EOS, false>(k, un, pr, counts);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) sb[f * (XW * XPITCH) + PH] = un[f];
+    }
+}
 
 template <typename T, int EOS, bool EMIT, int ROWS>
 __global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> k)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     XSmem<T, ROWS>& S = *reinterpret_cast<XSmem<T, ROWS>*>(smem_raw);
-    const int t = threadIdx.x;
-    const long long row0 = (long long)blockIdx.x * ROWS;
-    const int nrows = (int)min((long long)ROWS, P.npencil - row0);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long row0 = (long long)blockIdx.x * ROWS + warp * XW;
+    if (row0 >= P.npencil) return;                        // whole warp idle (no CTA barrier below)
+    const int nrows = (int)min((long long)XW, P.npencil - row0);
     const int sg = blockIdx.y;
     const int j0 = sg * P.seg;
     const int j1 = min(P.N, j0 + P.seg);
@@ -379,23 +708,28 @@ __global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> 
     const int c_last = (ihi - 1) / XCH;
     const int N = P.N;
 
-    // cooperative chunk loader: element (row, col) of chunk c <- in[f][(row0+row)*nx + ghost(XCH*c+col)]
+    // warp-cooperative chunk loader: element (row, col) of chunk c <- in[f][(row0+row)*nx + ghost(XCH*c+col)]
+    // (lane -> 8 consecutive lanes cover one 64 B row piece)
     auto load_chunk = [&](int c, int stage) {
         if (c <= c_last) {
-            for (int e = t; e < ROWS * XCH; e += ROWS) {
+#pragma unroll
+            for (int e = lane; e < XW * XCH; e += 32) {
                 const int row = e / XCH, col = e % XCH;
                 const int i = c * XCH + col;
                 if (row < nrows && i >= ilo && i < ihi) {
                     const long long g = (row0 + row) * (long long)N + ghost_index(i, N, P.periodic);
 #pragma unroll
                     for (int f = 0; f < NF; ++f)
-                        cp_async_elem<T>(&S.in[stage][f][row * XPITCH + col], (const T*)P.in[f] + g);
+                        cp_async_elem<T>(&S.buf[warp][stage][f][row * XPITCH + col], (const T*)P.in[f] + g);
                 }
             }
         }
         cp_async_commit();
     };
 
+    Cnt cnt;
+    cnt.p = &S.cnt[0][threadIdx.x]; cnt.stride = ROWS;
+    cnt.zero();
     Marcher<T, EOS> m;
     m.init();
     load_chunk(c_first, 0);
@@ -403,25 +737,24 @@ __global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> 
     for (int c = c_first; c <= c_last; ++c) {
         const int stage = (c - c_first) % XNS;
         cp_async_wait<XNS - 1>();
-        __syncthreads();
-        if (t < nrows) {
-            for (int s = 0; s < XCH; ++s) {
-                const int i = c * XCH + s;
-                if (i < ilo || i >= ihi) continue;
-                T u0[NF], un[NF];
-#pragma unroll
-                for (int f = 0; f < NF; ++f) u0[f] = S.in[stage][f][t * XPITCH + s];
-                m.step(k, u0, un);
-                if (i - GH >= j0) {
-                    project<T>(k, un, P.counts);
-#pragma unroll
-                    for (int f = 0; f < NF; ++f) S.out[f][t * XPITCH + s] = un[f];
-                }
+        __syncwarp();
+        if (lane < nrows) {
+#pragma unroll 1
+            for (int h = 0; h < XCH / 4; ++h) {
+                T* sb = &S.buf[warp][stage][0][lane * XPITCH + 4 * h];
+                const int i = c * XCH + 4 * h;
+                x_substep<T, EOS, 0>(m, k, sb, i + 0, ilo, ihi, j0, cnt);
+                x_substep<T, EOS, 1>(m, k, sb, i + 1, ilo, ihi, j0, cnt);
+                x_substep<T, EOS, 2>(m, k, sb, i + 2, ilo, ihi, j0, cnt);
+                x_substep<T, EOS, 3>(m, k, sb, i + 3, ilo, ihi, j0, cnt);
             }
         }
-        __syncthreads();
-        // write-back of output cells [XCH*c - 4, XCH*c + 4) and refill of the stage just consumed
-        for (int e = t; e < ROWS * XCH; e += ROWS) {
+        __syncwarp();
+        // write-back of output cells [XCH*c - 4, XCH*c + 4), then refill of the same stage.  Every lane
+        // refills exactly the elements it has just read (same e -> (row, col) map), so program order
+        // (LDS -> STG -> LDGSTS) keeps the refill behind the read.
+#pragma unroll
+        for (int e = lane; e < XW * XCH; e += 32) {
             const int row = e / XCH, col = e % XCH;
             const int jo = c * XCH - GH + col;
             if (row < nrows && jo >= j0 && jo < j1) {
@@ -429,12 +762,12 @@ __global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> 
                 T u[NF];
 #pragma unroll
                 for (int f = 0; f < NF; ++f) {
-                    u[f] = S.out[f][row * XPITCH + col];
+                    u[f] = S.buf[warp][stage][f][row * XPITCH + col];
                     ((T*)P.out[f])[g] = u[f];
                 }
                 if (EMIT) {
                     T pr[6];
-                    primitives<T, EOS>(k, u, pr, P.counts);
+                    emit_primitives<T, EOS>(k, u, pr, cnt);
 #pragma unroll
                     for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[g] = pr[q];
                 }
@@ -443,6 +776,7 @@ __global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> 
         load_chunk(c + XNS, stage);
     }
     cp_async_wait<0>();
+    flush_counts(cnt, P.counts);
 }
 
 }  // namespace shk
