@@ -33,6 +33,7 @@ struct shasta {
     int periodic;
     int precision;          // 64 | 32
     int seg_override;
+    int variant;            // 0: single-role y/z march (default), 1: warp-specialised march (experimental)
     long long step;
     int table[64];
     int ntable;
@@ -97,18 +98,18 @@ Consts<T> make_consts(const shasta_t* h)
     Consts<T> k;
     k.lam = (T)h->lambda;
     k.hlam = (T)(0.5 * h->lambda);
-    k.gam = (T)h->gamma;
-    k.gm1 = (T)(h->gamma - 1.0);
-    k.g2 = (T)(h->gamma * h->gamma);
-    k.c4 = (T)(4.0 * (h->gamma - 1.0));
-    k.hg = (T)(0.5 * h->gamma);
-    k.omd = (T)(1.0 - 1e-12);
-    k.mass = (T)h->mass;
     k.qlam = (T)(0.25 * h->lambda);
-    k.omd2 = (T)((1.0 - 1e-12) * (1.0 - 1e-12));
+    k.d.gam = h->gamma;
+    k.d.gm1 = h->gamma - 1.0;
+    k.d.g2 = h->gamma * h->gamma;
+    k.d.c4 = 4.0 * (h->gamma - 1.0);
+    k.d.hg = 0.5 * h->gamma;
+    k.d.omd = 1.0 - 1e-12;
+    k.d.omd2 = (1.0 - 1e-12) * (1.0 - 1e-12);
+    k.d.mass = h->mass;
     // fast cons2prim path (shasta_kernels.cuh, c2p_fast_y): its frozen-slope Newton converges in two steps while
     // (Gamma-1)/(2-Gamma) <= 2, i.e. Gamma <= 5/3; above that every cell takes the general path.
-    k.fast = (h->gamma <= 5.0 / 3.0 + 1e-12) ? 1 : 0;
+    k.d.fast = (h->gamma <= 5.0 / 3.0 + 1e-12) ? 1 : 0;
     return k;
 }
 
@@ -269,8 +270,17 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
         P.stride_other = stride[other];
         P.seg = auto_segment(h, axis, P.N, P.npencil);
         P.nseg = (P.N + P.seg - 1) / P.seg;
-        dim3 grid((unsigned)((P.npencil + STRIDED_BLOCK - 1) / STRIDED_BLOCK), (unsigned)P.nseg);
-        sweep_strided_kernel<T, EOS, EMIT><<<grid, STRIDED_BLOCK, 0, st>>>(P, k);
+        if (h->variant == 1) {
+            // warp-specialised march (experimental): 128 pencils per CTA, 4 producer + 4 consumer warps
+            auto kern = sweep_strided_ws_kernel<T, EOS, EMIT>;
+            const size_t smem = sizeof(WsSmem<T>);
+            CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            dim3 grid((unsigned)((P.npencil + WS_P - 1) / WS_P), (unsigned)P.nseg);
+            kern<<<grid, 2 * WS_P, smem, st>>>(P, k);
+        } else {
+            dim3 grid((unsigned)((P.npencil + STRIDED_BLOCK - 1) / STRIDED_BLOCK), (unsigned)P.nseg);
+            sweep_strided_kernel<T, EOS, EMIT><<<grid, STRIDED_BLOCK, 0, st>>>(P, k);
+        }
     }
     CK(cudaGetLastError());
     h->launches++;
@@ -405,6 +415,10 @@ int shasta_set_option(shasta_t* h, int key, double value)
         if (!(value >= 0.0)) return fail(h, SHASTA_EINVAL, "SHASTA_SEGMENT must be >= 0");
         h->seg_override = (int)value;
         if (h->seg_override > 0 && h->seg_override < 8) h->seg_override = 8;
+        return 0;
+    case SHASTA_VARIANT:
+        if (value != 0.0 && value != 1.0) return fail(h, SHASTA_EINVAL, "SHASTA_VARIANT must be 0 or 1");
+        h->variant = (int)value;
         return 0;
     default:
         return fail(h, SHASTA_EINVAL, "shasta_set_option: unknown key %d", key);

@@ -35,20 +35,27 @@ constexpr int GH = 4;       // ghost depth = dependency radius of one sweep
 constexpr int EOS_GAMMA = 0;    // p = (Gamma-1) e            (m = 0): closed-form velocity
 constexpr int EOS_MASS = 1;     // p = (Gamma-1)(e - m n)     (m > 0): safeguarded Newton
 
+// EOS / cons2prim constants.  cons2prim, the causality projection and the primitive output ALWAYS run in
+// fp64, also on the fp32 storage path (the paper's own plan: "double precision for ... the calculation of
+// the boost"): e = E - |M| v cancels gamma^2 digits, which fp32 does not have.
+struct EosD {
+    double gam;     // Gamma
+    double gm1;     // Gamma-1
+    double g2;      // Gamma^2
+    double c4;      // 4 (Gamma-1)
+    double hg;      // Gamma/2
+    double omd;     // 1 - delta, delta = 1e-12 (reading G7)
+    double omd2;    // (1 - delta)^2
+    double mass;    // m
+    int fast;       // 1: Gamma-law fast path usable (Gamma <= 5/3), 0: general path for every cell
+};
+
 template <typename T>
 struct Consts {
     T lam;      // lambda = dt/dx
-    T hlam;     // lambda/2 (predictor)
-    T gam;      // Gamma
-    T gm1;      // Gamma-1
-    T g2;       // Gamma^2
-    T c4;       // 4 (Gamma-1)
-    T hg;       // Gamma/2
-    T omd;      // 1 - delta, delta = 1e-12 (reading G7)
-    T mass;     // m
-    T qlam;     // lambda/4   (predictor source factor 1/2 * lambda/2)
-    T omd2;     // (1 - delta)^2
-    int fast;   // 1: fp64 Gamma-law fast path usable (Gamma <= 5/3), 0: general path for every cell
+    T hlam;     // lambda/2 (predictor; corrector source factor)
+    T qlam;     // lambda/4 (predictor source factor 1/2 * lambda/2)
+    EosD d;
 };
 
 struct SweepParams {
@@ -154,89 +161,88 @@ __device__ __forceinline__ float fast_sqrt(float w) { return sqrtf(w); }
 //   EOS_GAMMA: closed form v = 2 Mc / (Gamma E + sqrt(Gamma^2 E^2 - 4 (Gamma-1) Mc^2)) (pin P7 ii).
 //   EOS_MASS : Newton with bisection safeguard on the bracket [v(m=0), Mc/E]; the warp leaves the loop
 //              together (__all_sync), so there is no intra-warp divergence in the iteration.
-template <typename T>
 struct Prim {
-    T y, e, p, w;
+    double y, e, p, w;
     int fl;
 };
 
-template <typename T, int EOS>
-__device__ __forceinline__ Prim<T> cons2prim_general(const Consts<T>& k, T E, T Ma, T Mb, T Mc, T R)
+template <int EOS>
+__device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, double Ma, double Mb, double Mc, double R)
 {
-    Prim<T> o;
-    const bool vac = !(E > T(0));                   // vacuum (reading G7); also catches NaN
-    if (vac) { E = T(1); Ma = Mb = Mc = T(0); }     // keep the arithmetic below finite; result discarded
+    Prim o;
+    const bool vac = !(E > double(0));                   // vacuum (reading G7); also catches NaN
+    if (vac) { E = double(1); Ma = Mb = Mc = double(0); }     // keep the arithmetic below finite; result discarded
     o.fl = 0;
-    const T M2 = t_fma(Ma, Ma, t_fma(Mb, Mb, Mc * Mc));
-    const T lim = k.omd * E;
-    const T lim2 = lim * lim;
-    T Mq = M2;          // Mc^2 (clamped)
-    T s = T(1);         // Mc / |M|
+    const double M2 = fma(Ma, Ma, fma(Mb, Mb, Mc * Mc));
+    const double lim = k.omd * E;
+    const double lim2 = lim * lim;
+    double Mq = M2;          // Mc^2 (clamped)
+    double s = double(1);         // Mc / |M|
     if (M2 > lim2) {    // causality clamp, same rule as Pi
         Mq = lim2;
-        s = lim * t_rsqrt(M2);
+        s = lim * rsqrt(M2);
     }
-    const T disc = t_fma(k.g2, E * E, -k.c4 * Mq);
-    const T sq = t_sqrt(disc);
-    const T hden = t_fma(k.hg, E, T(0.5) * sq);     // (Gamma E + sqrt(disc)) / 2
-    T inv = T(1) / hden;                            // v = Mc * inv   (m = 0 root)
+    const double disc = fma(k.g2, E * E, -k.c4 * Mq);
+    const double sq = sqrt(disc);
+    const double hden = fma(k.hg, E, double(0.5) * sq);     // (Gamma E + sqrt(disc)) / 2
+    double inv = double(1) / hden;                            // v = Mc * inv   (m = 0 root)
     if (EOS == EOS_GAMMA) {
-        const T eraw = t_fma(-Mq, inv, E);
-        if (eraw < T(0)) o.fl |= 1;
-        o.e = t_max(eraw, T(0));
+        const double eraw = fma(-Mq, inv, E);
+        if (eraw < double(0)) o.fl |= 1;
+        o.e = fmax(eraw, double(0));
         o.p = k.gm1 * o.e;
-        o.w = t_max(T(1) - Mq * inv * inv, T(0));
+        o.w = fmax(double(1) - Mq * inv * inv, double(0));
         o.y = s * inv;
     } else {
-        const T Mabs = t_sqrt(Mq);
-        T lo = Mabs * inv;                          // m = 0 root: lower bound (P_m <= P_0)
-        T hi = t_min(Mabs / E, k.omd);              // P = 0 root: upper bound
-        lo = t_min(lo, hi);
-        const T mR = k.mass * R;
-        T v = lo;
+        const double Mabs = sqrt(Mq);
+        double lo = Mabs * inv;                          // m = 0 root: lower bound (P_m <= P_0)
+        double hi = fmin(Mabs / E, k.omd);              // P = 0 root: upper bound
+        lo = fmin(lo, hi);
+        const double mR = k.mass * R;
+        double v = lo;
         for (int it = 0; it < 48; ++it) {
-            const T w2 = t_fma(-v, v, T(1));
-            const T w = t_sqrt(w2);
-            const T praw = k.gm1 * ((E - Mabs * v) - mR * w);
-            const bool pos = praw > T(0);
-            const T P = pos ? praw : T(0);
-            const T dP = pos ? k.gm1 * (mR * v / w - Mabs) : T(0);
-            const T g = t_fma(v, E + P, -Mabs);
-            const T dg = t_fma(v, dP, E + P);
-            if (g > T(0)) hi = v; else lo = v;
-            T vn = v - g / dg;
-            if (!(vn >= lo && vn <= hi)) vn = T(0.5) * (lo + hi);
-            const T dv = t_abs(vn - v);
+            const double w2 = fma(-v, v, double(1));
+            const double w = sqrt(w2);
+            const double praw = k.gm1 * ((E - Mabs * v) - mR * w);
+            const bool pos = praw > double(0);
+            const double P = pos ? praw : double(0);
+            const double dP = pos ? k.gm1 * (mR * v / w - Mabs) : double(0);
+            const double g = fma(v, E + P, -Mabs);
+            const double dg = fma(v, dP, E + P);
+            if (g > double(0)) hi = v; else lo = v;
+            double vn = v - g / dg;
+            if (!(vn >= lo && vn <= hi)) vn = double(0.5) * (lo + hi);
+            const double dv = fabs(vn - v);
             v = vn;
-            const T tol = sizeof(T) == 8 ? T(1e-15) : T(2e-7);
+            const double tol = 1e-15;
             if (__all_sync(__activemask(), dv <= tol)) break;
         }
-        o.w = t_max(t_fma(-v, v, T(1)), T(0));
-        const T eraw = t_fma(-Mabs, v, E);
-        if (eraw < T(0)) o.fl |= 1;
-        o.e = t_max(eraw, T(0));
-        const T n = R * t_sqrt(o.w);
-        const T praw = k.gm1 * (o.e - k.mass * n);
-        if (praw < T(0)) o.fl |= 2;
-        o.p = t_max(praw, T(0));
-        o.y = (M2 > T(0)) ? v * t_rsqrt(M2) : T(0);
+        o.w = fmax(fma(-v, v, double(1)), double(0));
+        const double eraw = fma(-Mabs, v, E);
+        if (eraw < double(0)) o.fl |= 1;
+        o.e = fmax(eraw, double(0));
+        const double n = R * sqrt(o.w);
+        const double praw = k.gm1 * (o.e - k.mass * n);
+        if (praw < double(0)) o.fl |= 2;
+        o.p = fmax(praw, double(0));
+        o.y = (M2 > double(0)) ? v * rsqrt(M2) : double(0);
     }
-    if (vac) { o.y = T(0); o.e = T(0); o.p = T(0); o.w = T(0); o.fl = 0; }   // n = R sqrt(w) = 0 (reading G7)
+    if (vac) { o.y = double(0); o.e = double(0); o.p = double(0); o.w = double(0); o.fl = 0; }   // n = R sqrt(w) = 0 (reading G7)
     return o;
 }
 
 // out-of-line copy for the rare cells of the fp64 Gamma-law kernels (keeps the march loop small)
-__device__ __noinline__ Prim<double> cons2prim_rare(const Consts<double>& k, double E, double Ma, double Mb,
+__device__ __noinline__ Prim cons2prim_rare(const EosD& k, double E, double Ma, double Mb,
                                                     double Mc, double R)
 {
-    return cons2prim_general<double, EOS_GAMMA>(k, E, Ma, Mb, Mc, R);
+    return cons2prim_general<EOS_GAMMA>(k, E, Ma, Mb, Mc, R);
 }
 
 // Only vacuum / non-positive E (high word <= 0; also -0, NaN with the sign set) leaves the fast path for the
 // out-of-line general routine.  The causality clamp Mc = min(|M|, (1-delta) E) stays inline: Mc^2 is a
 // select on the bit patterns (non-negative doubles order like integers), and only a clamped cell (~0.2 % of
 // the cells of config 4) pays the extra rsqrt for the direction-preserving scale factor.
-__device__ __forceinline__ bool c2p_is_vacuum(const Consts<double>& k, double E)
+__device__ __forceinline__ bool c2p_is_vacuum(const EosD& k, double E)
 {
     return (__double2hiint(E) <= 0) | (k.fast == 0);
 }
@@ -258,7 +264,7 @@ __device__ __forceinline__ double fast_rsqrt(double x)
 // r = rsq64h(disc) ~ 1/sqrt(disc), y0 = 2 rcp64h(disc r + b) (both 2^-20); Newton with the FROZEN slope r:
 // y <- y + f(y) r.  Error e -> e 2^-20 + (c y/sqrt(disc)) e^2 with c y/sqrt(disc) <= (Gamma-1)/(2-Gamma)
 // (= 1/2 for Gamma = 4/3): 2^-20 -> 2^-39 -> 2^-58.  15 fp64 ops including |M|^2, no division, no sqrt.
-__device__ __forceinline__ double c2p_fast_y(const Consts<double>& k, double E, double M2, double t)
+__device__ __forceinline__ double c2p_fast_y(const EosD& k, double E, double M2, double t)
 {
     const double disc = fma(k.g2, t, -(k.c4 * M2));
     const double r = rsq64h(disc);
@@ -273,21 +279,20 @@ __device__ __forceinline__ double c2p_fast_y(const Consts<double>& k, double E, 
 }
 
 // In-sweep cons2prim (S1, S3): only v_par = M_par y and p are needed.
-template <typename T, int EOS>
-__device__ __forceinline__ void c2p_sweep(const Consts<T>& k, const T (&u)[NF], T& v, T& p)
+template <int EOS>
+__device__ __forceinline__ void c2p_sweep_d(const EosD& k, const double (&u)[NF], double& v, double& p)
 {
-    const Prim<T> o = cons2prim_general<T, EOS>(k, u[0], u[1], u[2], u[3], u[4]);
+    const Prim o = cons2prim_general<EOS>(k, u[0], u[1], u[2], u[3], u[4]);
     v = u[1] * o.y;
     p = o.p;
 }
 template <>
-__device__ __forceinline__ void c2p_sweep<double, EOS_GAMMA>(const Consts<double>& k, const double (&u)[NF],
-                                                             double& v, double& p)
+__device__ __forceinline__ void c2p_sweep_d<EOS_GAMMA>(const EosD& k, const double (&u)[NF], double& v, double& p)
 {
     const double M2 = fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3]));
     double y, e;
     if (c2p_is_vacuum(k, u[0])) {
-        const Prim<double> o = cons2prim_rare(k, u[0], u[1], u[2], u[3], u[4]);
+        const Prim o = cons2prim_rare(k, u[0], u[1], u[2], u[3], u[4]);
         y = o.y; e = o.e;
     } else {
         const double t = u[0] * u[0];
@@ -300,6 +305,16 @@ __device__ __forceinline__ void c2p_sweep<double, EOS_GAMMA>(const Consts<double
     }
     v = u[1] * y;
     p = k.gm1 * e;
+}
+template <typename T, int EOS>
+__device__ __forceinline__ void c2p_sweep(const Consts<T>& k, const T (&u)[NF], T& v, T& p)
+{
+    double ud[NF], vd, pd;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) ud[f] = (double)u[f];
+    c2p_sweep_d<EOS>(k.d, ud, vd, pd);
+    v = (T)vd;
+    p = (T)pd;
 }
 
 // eq. (21) branch-free (reading G12): A = sigma max(0, min(sigma D^_{j+1}, |A^ph|, sigma D^_{j-1}))
@@ -427,30 +442,28 @@ struct Marcher {
 };
 
 // Pi, readings G6-G8: written back to M at the end of every sweep.  E and R are never modified.
-template <typename T>
-__device__ __forceinline__ void project(const Consts<T>& k, T (&un)[NF], Cnt counts)
+__device__ __forceinline__ void project(const EosD& k, double (&un)[NF], Cnt counts)
 {
-    const T E = un[0];
-    const T M2 = t_fma(un[1], un[1], t_fma(un[2], un[2], un[3] * un[3]));
-    const T lim = k.omd * E;
-    if (!(E > T(0))) {
-        un[1] = un[2] = un[3] = T(0);
+    const double E = un[0];
+    const double M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
+    const double lim = k.omd * E;
+    if (!(E > 0.0)) {
+        un[1] = un[2] = un[3] = 0.0;
         counts.add(1);
     } else if (M2 > lim * lim) {
-        const T s = lim * t_rsqrt(M2);
+        const double s = lim * rsqrt(M2);
         un[1] *= s; un[2] *= s; un[3] *= s;
         counts.add(0);
     }
 }
 
 // primitives of one cell from its (projected) conserved state, slots permuted like the momenta
-template <typename T, int EOS>
-__device__ __forceinline__ void primitives(const Consts<T>& k, const T (&u)[NF], T (&pr)[6],
-                                           Cnt counts)
+template <int EOS>
+__device__ __forceinline__ void primitives(const EosD& k, const double (&u)[NF], double (&pr)[6], Cnt counts)
 {
-    const Prim<T> o = cons2prim_general<T, EOS>(k, u[0], u[1], u[2], u[3], u[4]);
+    const Prim o = cons2prim_general<EOS>(k, u[0], u[1], u[2], u[3], u[4]);
     pr[0] = o.e; pr[1] = o.p;
-    pr[2] = u[4] * t_sqrt(o.w);
+    pr[2] = u[4] * sqrt(o.w);
     pr[3] = u[1] * o.y; pr[4] = u[2] * o.y; pr[5] = u[3] * o.y;
     if (o.fl) {                                     // rare: diagnostics [2] e floored, [3] p floored
         if (o.fl & 1) counts.add(2);
@@ -458,24 +471,15 @@ __device__ __forceinline__ void primitives(const Consts<T>& k, const T (&u)[NF],
     }
 }
 
-__device__ __noinline__ void finish_rare(const Consts<double>& k, double (&un)[NF], double (&pr)[6], int emit,
-                                         Cnt counts)
+__device__ __noinline__ void finish_rare(const EosD& k, double (&un)[NF], double (&pr)[6], int emit, Cnt counts)
 {
-    project<double>(k, un, counts);
-    if (emit) primitives<double, EOS_GAMMA>(k, un, pr, counts);
+    project(k, un, counts);
+    if (emit) primitives<EOS_GAMMA>(k, un, pr, counts);
 }
 
-// S6 tail + S7 of one output cell: Pi on un[], and (EMIT) its primitives pr[].
-template <typename T, int EOS, bool EMIT>
-__device__ __forceinline__ void finish_cell(const Consts<T>& k, T (&un)[NF], T (&pr)[6], Cnt counts)
-{
-    project<T>(k, un, counts);
-    if (EMIT) primitives<T, EOS>(k, un, pr, counts);
-}
-// fp64 Gamma-law: Pi and the primitives share |M|^2 and E^2; everything but vacuum is inline.
 // primitives from (E, Mc^2, E^2) on the fast path: y 12 ops, e/w 3, sqrt 6, n/p/v 5
-__device__ __forceinline__ void prims_fast(const Consts<double>& k, const double (&u)[NF], double Mq, double t,
-                                           double s, double (&pr)[6])
+__device__ __forceinline__ void prims_fast(const EosD& k, const double (&u)[NF], double Mq, double t, double s,
+                                           double (&pr)[6])
 {
     double y = c2p_fast_y(k, u[0], Mq, t);
     const double e = fma(-Mq, y, u[0]);
@@ -487,49 +491,56 @@ __device__ __forceinline__ void prims_fast(const Consts<double>& k, const double
     pr[3] = u[1] * y; pr[4] = u[2] * y; pr[5] = u[3] * y;
 }
 
-template <bool EMIT>
-__device__ __forceinline__ void finish_cell_fast(const Consts<double>& k, double (&un)[NF], double (&pr)[6],
-                                                 Cnt counts)
+// S6 tail + S7 of one output cell: Pi on un[], and (EMIT) its primitives pr[].
+template <int EOS, bool EMIT>
+__device__ __forceinline__ void finish_d(const EosD& k, double (&un)[NF], double (&pr)[6], Cnt counts)
 {
-    if (c2p_is_vacuum(k, un[0])) {
-        finish_rare(k, un, pr, EMIT ? 1 : 0, counts);
-        return;
-    }
-    double M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
-    const double t = un[0] * un[0];
-    const double lim2 = k.omd2 * t;
-    double s = 1.0;
-    if (gt_nonneg(M2, lim2)) {                          // Pi fires: scale M onto |M| = (1-delta) E
-        const double sc = (k.omd * un[0]) * fast_rsqrt(M2);
-        un[1] *= sc; un[2] *= sc; un[3] *= sc;
-        counts.add(0);
-        if (EMIT) {                                     // primitives of the PROJECTED state, like the oracle
-            M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
-            if (gt_nonneg(M2, lim2)) s = (k.omd * un[0]) * fast_rsqrt(M2);
+    if (EOS == EOS_GAMMA) {
+        // Gamma-law: Pi and the primitives share |M|^2 and E^2; everything but vacuum is inline
+        if (c2p_is_vacuum(k, un[0])) {
+            finish_rare(k, un, pr, EMIT ? 1 : 0, counts);
+            return;
         }
+        double M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
+        const double t = un[0] * un[0];
+        const double lim2 = k.omd2 * t;
+        double s = 1.0;
+        if (gt_nonneg(M2, lim2)) {                          // Pi fires: scale M onto |M| = (1-delta) E
+            const double sc = (k.omd * un[0]) * fast_rsqrt(M2);
+            un[1] *= sc; un[2] *= sc; un[3] *= sc;
+            counts.add(0);
+            if (EMIT) {                                     // primitives of the PROJECTED state, like the oracle
+                M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
+                if (gt_nonneg(M2, lim2)) s = (k.omd * un[0]) * fast_rsqrt(M2);
+            }
+        }
+        if (EMIT) prims_fast(k, un, gt_nonneg(M2, lim2) ? lim2 : M2, t, s, pr);
+    } else {
+        project(k, un, counts);
+        if (EMIT) primitives<EOS>(k, un, pr, counts);
     }
-    if (EMIT) prims_fast(k, un, gt_nonneg(M2, lim2) ? lim2 : M2, t, s, pr);
 }
-template <> __device__ __forceinline__ void finish_cell<double, EOS_GAMMA, true>(
-    const Consts<double>& k, double (&un)[NF], double (&pr)[6], Cnt counts)
-{ finish_cell_fast<true>(k, un, pr, counts); }
-template <> __device__ __forceinline__ void finish_cell<double, EOS_GAMMA, false>(
-    const Consts<double>& k, double (&un)[NF], double (&pr)[6], Cnt counts)
-{ finish_cell_fast<false>(k, un, pr, counts); }
+template <typename T, int EOS, bool EMIT>
+__device__ __forceinline__ void finish_cell(const Consts<T>& k, T (&un)[NF], T (&pr)[6], Cnt counts)
+{
+    double ud[NF], pd[6];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) ud[f] = (double)un[f];
+    finish_d<EOS, EMIT>(k.d, ud, pd, counts);
+#pragma unroll
+    for (int f = 1; f < 4; ++f) un[f] = (T)ud[f];           // Pi touches M only
+    if (EMIT) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) pr[q] = (T)pd[q];
+    }
+}
 
-// primitives of an already projected cell (x sweep write-back): fast path + rare fallback
-template <typename T, int EOS>
-__device__ __forceinline__ void emit_primitives(const Consts<T>& k, const T (&u)[NF], T (&pr)[6],
-                                                Cnt counts)
+// primitives of an already projected cell (x sweep write-back, shasta_get_primitives refresh)
+template <int EOS>
+__device__ __forceinline__ void emit_d(const EosD& k, const double (&u)[NF], double (&pr)[6], Cnt counts)
 {
-    primitives<T, EOS>(k, u, pr, counts);
-}
-template <>
-__device__ __forceinline__ void emit_primitives<double, EOS_GAMMA>(const Consts<double>& k, const double (&u)[NF],
-                                                                   double (&pr)[6], Cnt counts)
-{
-    if (c2p_is_vacuum(k, u[0])) {
-        primitives<double, EOS_GAMMA>(k, u, pr, counts);
+    if (EOS != EOS_GAMMA || c2p_is_vacuum(k, u[0])) {
+        primitives<EOS>(k, u, pr, counts);
         return;
     }
     const double M2 = fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3]));
@@ -538,6 +549,16 @@ __device__ __forceinline__ void emit_primitives<double, EOS_GAMMA>(const Consts<
     const bool clamped = gt_nonneg(M2, lim2);
     const double s = clamped ? (k.omd * u[0]) * fast_rsqrt(M2) : 1.0;
     prims_fast(k, u, clamped ? lim2 : M2, t, s, pr);
+}
+template <typename T, int EOS>
+__device__ __forceinline__ void emit_primitives(const Consts<T>& k, const T (&u)[NF], T (&pr)[6], Cnt counts)
+{
+    double ud[NF], pd[6];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) ud[f] = (double)u[f];
+    emit_d<EOS>(k.d, ud, pd, counts);
+#pragma unroll
+    for (int q = 0; q < 6; ++q) pr[q] = (T)pd[q];
 }
 
 // cp.async (LDGSTS) helpers: one element per thread, global -> shared without touching registers
@@ -652,6 +673,238 @@ __global__ void __launch_bounds__(SBLOCK) sweep_strided_kernel(SweepParams P, Co
     }
     cp_async_wait<0>();
     flush_counts(c.counts, P.counts);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Warp-specialised march: the serial chain S1..S6 of one march step is cut after S3 and
+// run by TWO warps per 32 pencils, a producer P (S1-S3 + the corrector's geometry) and a consumer C
+// (S4-S6), so that twice as many warps are resident for the same register budget and each warp's
+// dependent chain is half as long.  P -> C traffic per pencil and step is four doubles through a
+// shared-memory queue: a_c = 1/2 - Q+, b_c = Q+^2/2 of the interface (i-2,i-1) at n+1/2, and the two
+// source increments -lambda Delta(p v)/2-form for E and M_par of cell i-2.
+template <typename T, int EOS>
+struct Producer {
+    T u1[NF];           // U^n_1
+    T ft[NF];           // predictor flux F~ at interface (i-2,i-1)
+    T eps1;             // (lambda/2) v_1 (time n)
+    T fE[2], fM[2];     // (p v)_1,_2 and p_1,_2 (time n)      slot (PH-k)&1
+    T epsh2;            // lambda v^{1/2}_2
+    T gE[2], gM[2];     // (p v)^{1/2}_2,_3, p^{1/2}_2,_3      slot (PH-k)&1
+
+    __device__ __forceinline__ void init()
+    {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) u1[f] = ft[f] = T(0);
+        eps1 = epsh2 = fE[0] = fE[1] = fM[0] = fM[1] = gE[0] = gE[1] = gM[0] = gM[1] = T(0);
+    }
+
+    // consumes U^n at the front cell i; msg = {a_c, b_c, sE, sM} for the consumer's step i
+    template <int PH>
+    __device__ __forceinline__ void step(const Consts<T>& k, const T (&u0)[NF], T (&msg)[4])
+    {
+        constexpr int S2 = PH & 1;              // time-n scalars _2 (new _0 takes its slot)
+        constexpr int G3 = (PH + 1) & 1;        // half-step scalars _3 (new _1 takes its slot)
+        T v0, p0;
+        c2p_sweep<T, EOS>(k, u0, v0, p0);                                   // S1
+        const T eps0 = k.hlam * v0;
+        const T fE0 = p0 * v0;
+        T ut[NF];
+        {                                                                   // S2
+            const T q = (T(0.5) - eps1) * fast_rcp(T(1) + (eps0 - eps1));   // Q+_1, eq. (15)
+            const T a = T(0.5) - q, b = (T(0.5) * q) * q;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                const T d = u0[f] - u1[f];                                  // eq. (16)
+                const T fl = t_fma(a, u1[f], -(b * d));
+                ut[f] = u1[f] - (fl - ft[f]);
+                ft[f] = fl;
+                u1[f] = u0[f];
+            }
+            ut[0] = t_fma(-k.qlam, fE0 - fE[S2], ut[0]);
+            ut[1] = t_fma(-k.qlam, p0 - fM[S2], ut[1]);
+        }
+        T vh1, ph;
+        c2p_sweep<T, EOS>(k, ut, vh1, ph);                                  // S3
+        const T epsh1 = k.lam * vh1;
+        const T gE1 = ph * vh1;
+        {                                                                   // geometry + sources of S4
+            const T q = (T(0.5) - epsh2) * fast_rcp(T(1) + (epsh1 - epsh2));
+            msg[0] = T(0.5) - q;
+            msg[1] = (T(0.5) * q) * q;
+            msg[2] = -k.hlam * (gE1 - gE[G3]);
+            msg[3] = -k.hlam * (ph - gM[G3]);
+        }
+        eps1 = eps0; fE[S2] = fE0; fM[S2] = p0;
+        epsh2 = epsh1; gE[G3] = gE1; gM[G3] = ph;
+    }
+};
+
+template <typename T>
+struct Consumer {
+    T up[NF];           // U^n_2
+    T dl[4][NF];        // Delta_2..Delta_5 (Delta_2 is formed in the step)   slot (PH-k)&3
+    T fc[NF];           // corrector flux F at interface (i-3,i-2)
+    T uh[2][NF];        // U^_3, U^_4                                         slot (PH-k)&1
+    T dh[2][NF];        // D^_4, D^_5                                         slot (PH-k)&1
+    T a5[NF];           // A_5
+
+    __device__ __forceinline__ void init()
+    {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            up[f] = dl[0][f] = dl[1][f] = dl[2][f] = dl[3][f] = fc[f] = T(0);
+            uh[0][f] = uh[1][f] = dh[0][f] = dh[1][f] = a5[f] = T(0);
+        }
+    }
+
+    // consumes U^n_{i-1} and the producer's message of step i; produces U^{n+1} of cell i-4 (before Pi)
+    template <int PH>
+    __device__ __forceinline__ void step(const T (&uj)[NF], const T (&msg)[4], T (&un)[NF])
+    {
+        constexpr int D2 = (PH + 2) & 3, D3 = (PH + 1) & 3, D4 = PH & 3, D5 = (PH + 3) & 3;
+        constexpr int H3 = (PH + 1) & 1, H4 = PH & 1;
+        constexpr int E4 = PH & 1, E5 = (PH + 1) & 1;
+        const T a = msg[0], b = msg[1];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            dl[D2][f] = uj[f] - up[f];                                           // eq. (16)
+            const T fl = t_fma(a, up[f], -(b * dl[D2][f]));                      // S4
+            T uh2 = up[f] - (fl - fc[f]);
+            if (f == 0) uh2 += msg[2];
+            if (f == 1) uh2 += msg[3];
+            fc[f] = fl;
+            const T dh3 = uh2 - uh[H3][f];                                       // eq. (18)
+            const T d2 = t_fma(T(-2), dl[D4][f], dl[D3][f] + dl[D5][f]);         // reading G14
+            const T aph = T(0.125) * t_fma(T(-0.125), d2, dh[E4][f]);            // eq. (19)
+            const T a4 = limiter<T>(aph, dh3, dh[E5][f]);                        // eqs. (20),(21)
+            un[f] = uh[H4][f] - (a4 - a5[f]);                                    // eq. (22)
+            a5[f] = a4;
+            dh[E5][f] = dh3;
+            uh[H4][f] = uh2;
+            up[f] = uj[f];
+        }
+    }
+};
+
+constexpr int WS_P = 128;         // pencils per CTA (4 producer warps + 4 consumer warps)
+constexpr int WS_R = 12;          // U ring slots per pencil
+constexpr int WS_D = WS_R - 5;    // producer prefetch distance in cells (see the slot-reuse argument below)
+constexpr int WS_Q = 4;           // message queue slots (2 chunks of 2 steps)
+
+template <typename T>
+struct WsSmem {
+    T ring[WS_R][NF][WS_P];
+    T msg[WS_Q][4][WS_P];
+    unsigned cnt[4][WS_P];
+};
+
+__device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+
+template <typename T, int EOS, bool EMIT>
+__global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(SweepParams P, Consts<T> k)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    WsSmem<T>& S = *reinterpret_cast<WsSmem<T>*>(smem_raw);
+    const int lane_p = threadIdx.x & (WS_P - 1);                // pencil slot inside the CTA
+    const bool producer = threadIdx.x < WS_P;                   // warps 0-3: P, warps 4-7: C
+    const int bar_id = 1 + ((threadIdx.x >> 5) & 3);            // one named barrier per warp pair
+    long long pen = (long long)blockIdx.x * WS_P + lane_p;
+    const bool active = pen < P.npencil;
+    if (!active) pen = P.npencil - 1;                           // idle lanes shadow a valid pencil, store nothing
+    const int sg = blockIdx.y;
+    const int j0 = sg * P.seg;
+    const int j1 = min(P.N, j0 + P.seg);
+    const long long sa = P.stride_axis;
+    const long long base = (pen % P.nx) + (pen / P.nx) * P.stride_other;
+    const int nsteps = (j1 - j0) + 2 * GH;                      // front cells j0-4 .. j1+3
+    const int nchunk = (nsteps + 1) / 2;
+    const int niter = ((nchunk + 1) + 1) & ~1;                  // P: chunks 0..nchunk-1, C one iteration behind; even
+
+    if (producer) {
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+        const T* in[NF];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) in[f] = (const T*)P.in[f] + base;
+        Producer<T, EOS> pr;
+        pr.init();
+        // prefetch state: next cell to fetch (true index ipf, ghost-mapped jpf) and its ring slot
+        int ipf = j0 - GH, jpf = ghost_index(ipf, P.N, P.periodic), pslot = 0;
+        auto prefetch = [&]() {
+            const long long o = (long long)jpf * sa;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) cp_async_elem<T>(&S.ring[pslot][f][lane_p], in[f] + o);
+            cp_async_commit();
+            pslot = (pslot + 1 == WS_R) ? 0 : pslot + 1;
+            ipf += 1;
+            if (P.periodic) { jpf = (jpf + 1 == P.N) ? 0 : jpf + 1; }
+            else            { jpf = min(max(ipf, 0), P.N - 1); }
+        };
+#pragma unroll
+        for (int d = 0; d < WS_D; ++d) prefetch();
+        int rslot = 0;
+        // Slot reuse: in iteration `it` this warp is at cells 2it+s and refills the slot of cell 2it+s+D-R
+        // = 2it+s-5 <= 2(it-1)-2, which the consumer read before the barrier that ended iteration it-1.
+#define SHK_PSTEP(PH)                                                                               \
+        {                                                                                           \
+            prefetch();                                                                             \
+            cp_async_wait<WS_D>();                                                                  \
+            T u0[NF], msg[4];                                                                       \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) u0[f] = S.ring[rslot][f][lane_p];        \
+            rslot = (rslot + 1 == WS_R) ? 0 : rslot + 1;                                            \
+            pr.template step<PH>(k, u0, msg);                                                       \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane_p] = msg[q];            \
+        }
+        for (int it = 0; it < niter; it += 2) {
+            if (it < nchunk) { SHK_PSTEP(0) SHK_PSTEP(1) }
+            pair_barrier(bar_id);
+            if (it + 1 < nchunk) { SHK_PSTEP(2) SHK_PSTEP(3) }
+            pair_barrier(bar_id);
+        }
+#undef SHK_PSTEP
+        cp_async_wait<0>();
+    } else {
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
+        T* out[NF];
+        T* prim[6];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) out[f] = (T*)P.out[f] + base;
+#pragma unroll
+        for (int q = 0; q < 6; ++q) prim[q] = (T*)P.prim[q] + base;
+        Cnt cnt;
+        cnt.p = &S.cnt[0][lane_p]; cnt.stride = WS_P;
+        cnt.zero();
+        Consumer<T> co;
+        co.init();
+        // consumer step t (front cell i = j0-4+t) reads U_{i-1}: ring slot of cell index t-1 (t = 0: the
+        // ring's last slot, never written before: a don't-care warm-up value, finite or not it is retired)
+        int cslot = WS_R - 1;
+        int i = j0 - GH;
+#define SHK_CSTEP(PH)                                                                               \
+        {                                                                                           \
+            T uj[NF], msg[4], un[NF];                                                               \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) uj[f] = S.ring[cslot][f][lane_p];        \
+            cslot = (cslot + 1 == WS_R) ? 0 : cslot + 1;                                            \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane_p];            \
+            co.template step<PH>(uj, msg, un);                                                      \
+            const int jo = i - GH;                                                                  \
+            if (jo >= j0 && jo < j1 && active) {                                                    \
+                T pv[6];                                                                            \
+                finish_cell<T, EOS, EMIT>(k, un, pv, cnt);                                          \
+                const long long o = (long long)jo * sa;                                             \
+                _Pragma("unroll") for (int f = 0; f < NF; ++f) out[f][o] = un[f];                   \
+                if (EMIT) { _Pragma("unroll") for (int q = 0; q < 6; ++q) prim[q][o] = pv[q]; }     \
+            }                                                                                       \
+            ++i;                                                                                    \
+        }
+        for (int it = 0; it < niter; it += 2) {
+            if (it >= 1 && it - 1 < nchunk) { SHK_CSTEP(2) SHK_CSTEP(3) }
+            pair_barrier(bar_id);
+            if (it < nchunk) { SHK_CSTEP(0) SHK_CSTEP(1) }
+            pair_barrier(bar_id);
+        }
+#undef SHK_CSTEP
+        flush_counts(cnt, P.counts);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
