@@ -66,9 +66,9 @@ def test_warp_specialised_variant(oracle, bc, segment):
     ref, _ = parity.run_oracle(oracle, c, steps=2)
     got, _ = parity.run_gpu(c, steps=2, variant=1, segment=segment)
     assert_kernel_parity(got, ref, f"ws variant bc {bc} segment {segment}")
+    # not bitwise the default kernel: the producer rounds the source increment before the consumer adds it
     base, _ = parity.run_gpu(c, steps=2, segment=segment)
-    for k in parity.CONS:
-        assert np.array_equal(got[k], base[k]), k
+    parity.assert_parity(got, base, 1e-13, label="ws vs default")
 
 
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
