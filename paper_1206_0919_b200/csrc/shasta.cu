@@ -92,6 +92,10 @@ int ensure_stage(shasta_t* h)
     return 0;
 }
 
+// The EOS_GAMMA kernels (closed-form fast cons2prim, shasta_kernels.cuh c2p_fast_y) need m = 0 and Gamma <= 5/3
+// (two frozen-slope Newton steps suffice while (Gamma-1)/(2-Gamma) <= 2); everything else runs the EOS_MASS kernels.
+bool use_general_eos(const shasta_t* h) { return h->mass != 0.0 || h->gamma > 5.0 / 3.0 + 1e-12; }
+
 template <typename T>
 Consts<T> make_consts(const shasta_t* h)
 {
@@ -107,9 +111,6 @@ Consts<T> make_consts(const shasta_t* h)
     k.d.omd = 1.0 - 1e-12;
     k.d.omd2 = (1.0 - 1e-12) * (1.0 - 1e-12);
     k.d.mass = h->mass;
-    // fast cons2prim path (shasta_kernels.cuh, c2p_fast_y): its frozen-slope Newton converges in two steps while
-    // (Gamma-1)/(2-Gamma) <= 2, i.e. Gamma <= 5/3; above that every cell takes the general path.
-    k.d.fast = (h->gamma <= 5.0 / 3.0 + 1e-12) ? 1 : 0;
     return k;
 }
 
@@ -290,7 +291,7 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
 
 int launch_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
 {
-    const bool general = h->mass != 0.0;
+    const bool general = use_general_eos(h);
     if (h->precision == 64) {
         if (general) return emit ? launch_sweep_t<double, EOS_MASS, true>(h, axis, st)
                                  : launch_sweep_t<double, EOS_MASS, false>(h, axis, st);
@@ -309,7 +310,7 @@ int refresh_prims_t(shasta_t* h, cudaStream_t st)
     void** U = h->U[h->cur];
     const int g = ew_grid(h, 256);
     const Consts<T> k = make_consts<T>(h);
-    if (h->mass != 0.0)
+    if (use_general_eos(h))
         cons2prim_kernel<T, EOS_MASS><<<g, 256, 0, st>>>(h->ncell, k, (T*)U[0], (T*)U[1], (T*)U[2], (T*)U[3],
             (T*)U[4], (T*)h->prim[0], (T*)h->prim[1], (T*)h->prim[2], (T*)h->prim[3], (T*)h->prim[4],
             (T*)h->prim[5], h->d_counts);

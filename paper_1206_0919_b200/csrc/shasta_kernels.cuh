@@ -47,7 +47,6 @@ struct EosD {
     double omd;     // 1 - delta, delta = 1e-12 (reading G7)
     double omd2;    // (1 - delta)^2
     double mass;    // m
-    int fast;       // 1: Gamma-law fast path usable (Gamma <= 5/3), 0: general path for every cell
 };
 
 template <typename T>
@@ -231,20 +230,14 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
     return o;
 }
 
-// out-of-line copy for the rare cells of the fp64 Gamma-law kernels (keeps the march loop small)
-__device__ __noinline__ Prim cons2prim_rare(const EosD& k, double E, double Ma, double Mb,
-                                                    double Mc, double R)
-{
-    return cons2prim_general<EOS_GAMMA>(k, E, Ma, Mb, Mc, R);
-}
-
-// Only vacuum / non-positive E (high word <= 0; also -0, NaN with the sign set) leaves the fast path for the
-// out-of-line general routine.  The causality clamp Mc = min(|M|, (1-delta) E) stays inline: Mc^2 is a
+// The EOS_GAMMA kernels have NO out-of-line path: vacuum / non-positive E (high word <= 0) is a two-line inline
+// branch (all primitives 0, M = 0), and the host instantiates them only for Gamma <= 5/3, where the frozen-slope
+// Newton of c2p_fast_y converges in two steps (larger Gamma runs the EOS_MASS kernels with m = 0).  The causality clamp Mc = min(|M|, (1-delta) E) stays inline: Mc^2 is a
 // select on the bit patterns (non-negative doubles order like integers), and only a clamped cell (~0.2 % of
 // the cells of config 4) pays the extra rsqrt for the direction-preserving scale factor.
-__device__ __forceinline__ bool c2p_is_vacuum(const EosD& k, double E)
+__device__ __forceinline__ bool c2p_is_vacuum(double E)
 {
-    return (__double2hiint(E) <= 0) | (k.fast == 0);
+    return __double2hiint(E) <= 0;
 }
 __device__ __forceinline__ bool gt_nonneg(double a, double b)      // a > b for a, b >= 0, on the integer pipe
 {
@@ -291,9 +284,8 @@ __device__ __forceinline__ void c2p_sweep_d<EOS_GAMMA>(const EosD& k, const doub
 {
     const double M2 = fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3]));
     double y, e;
-    if (c2p_is_vacuum(k, u[0])) {
-        const Prim o = cons2prim_rare(k, u[0], u[1], u[2], u[3], u[4]);
-        y = o.y; e = o.e;
+    if (c2p_is_vacuum(u[0])) {          // reading G7: all primitives 0
+        y = 0.0; e = 0.0;
     } else {
         const double t = u[0] * u[0];
         const double lim2 = k.omd2 * t;
@@ -471,12 +463,6 @@ __device__ __forceinline__ void primitives(const EosD& k, const double (&u)[NF],
     }
 }
 
-__device__ __noinline__ void finish_rare(const EosD& k, double (&un)[NF], double (&pr)[6], int emit, Cnt counts)
-{
-    project(k, un, counts);
-    if (emit) primitives<EOS_GAMMA>(k, un, pr, counts);
-}
-
 // primitives from (E, Mc^2, E^2) on the fast path: y 12 ops, e/w 3, sqrt 6, n/p/v 5
 __device__ __forceinline__ void prims_fast(const EosD& k, const double (&u)[NF], double Mq, double t, double s,
                                            double (&pr)[6])
@@ -497,8 +483,13 @@ __device__ __forceinline__ void finish_d(const EosD& k, double (&un)[NF], double
 {
     if (EOS == EOS_GAMMA) {
         // Gamma-law: Pi and the primitives share |M|^2 and E^2; everything but vacuum is inline
-        if (c2p_is_vacuum(k, un[0])) {
-            finish_rare(k, un, pr, EMIT ? 1 : 0, counts);
+        if (c2p_is_vacuum(un[0])) {                         // vacuum: M = 0, all primitives 0 (readings G7, R1)
+            un[1] = un[2] = un[3] = 0.0;
+            counts.add(1);
+            if (EMIT) {
+#pragma unroll
+                for (int q = 0; q < 6; ++q) pr[q] = 0.0;
+            }
             return;
         }
         double M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
@@ -539,8 +530,13 @@ __device__ __forceinline__ void finish_cell(const Consts<T>& k, T (&un)[NF], T (
 template <int EOS>
 __device__ __forceinline__ void emit_d(const EosD& k, const double (&u)[NF], double (&pr)[6], Cnt counts)
 {
-    if (EOS != EOS_GAMMA || c2p_is_vacuum(k, u[0])) {
+    if (EOS != EOS_GAMMA) {
         primitives<EOS>(k, u, pr, counts);
+        return;
+    }
+    if (c2p_is_vacuum(u[0])) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) pr[q] = 0.0;
         return;
     }
     const double M2 = fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3]));
@@ -801,7 +797,8 @@ struct WsSmem {
 __device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 
 template <typename T, int EOS, bool EMIT>
-__global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(SweepParams P, Consts<T> k)
+__global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __grid_constant__ SweepParams P,
+                                                                      const __grid_constant__ Consts<T> k)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WsSmem<T>& S = *reinterpret_cast<WsSmem<T>*>(smem_raw);
@@ -821,18 +818,15 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(SweepPara
     const int niter = ((nchunk + 1) + 1) & ~1;                  // P: chunks 0..nchunk-1, C one iteration behind; even
 
     if (producer) {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
-        const T* in[NF];
-#pragma unroll
-        for (int f = 0; f < NF; ++f) in[f] = (const T*)P.in[f] + base;
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
         Producer<T, EOS> pr;
         pr.init();
         // prefetch state: next cell to fetch (true index ipf, ghost-mapped jpf) and its ring slot
         int ipf = j0 - GH, jpf = ghost_index(ipf, P.N, P.periodic), pslot = 0;
         auto prefetch = [&]() {
-            const long long o = (long long)jpf * sa;
+            const long long o = base + (long long)jpf * sa;        // field pointers stay in the constant bank
 #pragma unroll
-            for (int f = 0; f < NF; ++f) cp_async_elem<T>(&S.ring[pslot][f][lane_p], in[f] + o);
+            for (int f = 0; f < NF; ++f) cp_async_elem<T>(&S.ring[pslot][f][lane_p], (const T*)P.in[f] + o);
             cp_async_commit();
             pslot = (pslot + 1 == WS_R) ? 0 : pslot + 1;
             ipf += 1;
@@ -863,13 +857,7 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(SweepPara
 #undef SHK_PSTEP
         cp_async_wait<0>();
     } else {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
-        T* out[NF];
-        T* prim[6];
-#pragma unroll
-        for (int f = 0; f < NF; ++f) out[f] = (T*)P.out[f] + base;
-#pragma unroll
-        for (int q = 0; q < 6; ++q) prim[q] = (T*)P.prim[q] + base;
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
         Cnt cnt;
         cnt.p = &S.cnt[0][lane_p]; cnt.stride = WS_P;
         cnt.zero();
@@ -890,9 +878,9 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(SweepPara
             if (jo >= j0 && jo < j1 && active) {                                                    \
                 T pv[6];                                                                            \
                 finish_cell<T, EOS, EMIT>(k, un, pv, cnt);                                          \
-                const long long o = (long long)jo * sa;                                             \
-                _Pragma("unroll") for (int f = 0; f < NF; ++f) out[f][o] = un[f];                   \
-                if (EMIT) { _Pragma("unroll") for (int q = 0; q < 6; ++q) prim[q][o] = pv[q]; }     \
+                const long long o = base + (long long)jo * sa;                                      \
+                _Pragma("unroll") for (int f = 0; f < NF; ++f) ((T*)P.out[f])[o] = un[f];           \
+                if (EMIT) { _Pragma("unroll") for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[o] = pv[q]; } \
             }                                                                                       \
             ++i;                                                                                    \
         }
