@@ -784,7 +784,7 @@ struct Consumer {
 
 constexpr int WS_P = 128;         // pencils per CTA (4 producer warps + 4 consumer warps)
 constexpr int WS_R = 12;          // U ring slots per pencil
-constexpr int WS_D = WS_R - 5;    // producer prefetch distance in cells (see the slot-reuse argument below)
+constexpr int WS_D = WS_R - 4;    // prefetch distance; D-1 copies stay in flight behind the current chunk (see below)
 constexpr int WS_Q = 4;           // message queue slots (2 chunks of 2 steps)
 
 template <typename T>
@@ -834,27 +834,37 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
             else            { jpf = min(max(ipf, 0), P.N - 1); }
         };
 #pragma unroll
-        for (int d = 0; d < WS_D; ++d) prefetch();
+        for (int d = 0; d < WS_D - 1; ++d) prefetch();
         int rslot = 0;
-        // Slot reuse: in iteration `it` this warp is at cells 2it+s and refills the slot of cell 2it+s+D-R
-        // = 2it+s-5 <= 2(it-1)-2, which the consumer read before the barrier that ended iteration it-1.
-#define SHK_PSTEP(PH)                                                                               \
+        // Copies: before chunk `it` cells 0 .. 2it+D-2 are issued; its two prefetches add cells 2it+D-1, 2it+D, and
+        // wait_group<D-1> then leaves at most the D-1 youngest pending, i.e. cells <= 2it+1 (this chunk) are complete.
+        // Slot reuse: those two refill the slots of cells 2it+D-1-R = 2it-5 and 2it-4, which the consumer read
+        // (as U_{i-1} of chunk it-2: cells <= 2it-4) before the barrier that ended iteration it-1; in iteration `it`
+        // it reads cells 2it-3, 2it-2.
+        // One chunk = two steps: both front cells are fetched first, then the two steps' arithmetic runs with no
+        // asm/memory fence in between, so the scheduler may overlap S3 of the first with S1 of the second.
+#define SHK_PCHUNK(PH)                                                                              \
         {                                                                                           \
             prefetch();                                                                             \
-            cp_async_wait<WS_D>();                                                                  \
-            T u0[NF], msg[4];                                                                       \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) u0[f] = S.ring[rslot][f][lane_p];        \
+            prefetch();                                                                             \
+            cp_async_wait<WS_D - 1>();                                                              \
+            T ua[NF], ub[NF], ma[4], mb[4];                                                         \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) ua[f] = S.ring[rslot][f][lane_p];        \
             rslot = (rslot + 1 == WS_R) ? 0 : rslot + 1;                                            \
-            pr.template step<PH>(k, u0, msg);                                                       \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane_p] = msg[q];            \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) ub[f] = S.ring[rslot][f][lane_p];        \
+            rslot = (rslot + 1 == WS_R) ? 0 : rslot + 1;                                            \
+            pr.template step<PH>(k, ua, ma);                                                        \
+            pr.template step<PH + 1>(k, ub, mb);                                                    \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane_p] = ma[q];             \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane_p] = mb[q];         \
         }
         for (int it = 0; it < niter; it += 2) {
-            if (it < nchunk) { SHK_PSTEP(0) SHK_PSTEP(1) }
+            if (it < nchunk) { SHK_PCHUNK(0) }
             pair_barrier(bar_id);
-            if (it + 1 < nchunk) { SHK_PSTEP(2) SHK_PSTEP(3) }
+            if (it + 1 < nchunk) { SHK_PCHUNK(2) }
             pair_barrier(bar_id);
         }
-#undef SHK_PSTEP
+#undef SHK_PCHUNK
         cp_async_wait<0>();
     } else {
         if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
