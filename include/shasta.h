@@ -40,9 +40,8 @@ typedef struct shasta shasta_t;   /* opaque */
 #define SHASTA_PRECISION  2   /* 64 (default) | 32: storage and transport arithmetic (before set_state) */
 #define SHASTA_STEP_INDEX 3   /* step counter s indexing the axis table (resume / tests)                */
 #define SHASTA_SEGMENT    4   /* tuning: cells marched per work item along the sweep axis (0 = auto)    */
-#define SHASTA_VARIANT    5   /* tuning: y/z sweep kernel, 0 = one marching thread per pencil (default),
-                                 1 = producer/consumer warp pair per 32 pencils (experimental, slower in
-                                 round 1: DESIGN.md 7); same arithmetic, same result                   */
+#define SHASTA_VARIANT    5   /* tuning: sweep kernels, 0 = producer/consumer warp pair per 32 pencils (default),
+                                 1 = one marching thread per pencil; same scheme, results agree to rounding */
 
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only

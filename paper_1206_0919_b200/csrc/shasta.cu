@@ -33,7 +33,7 @@ struct shasta {
     int periodic;
     int precision;          // 64 | 32
     int seg_override;
-    int variant;            // 0: single-role y/z march (default), 1: warp-specialised march (experimental)
+    int variant;            // 0: warp-specialised sweeps (producer/consumer warp pairs, default), 1: single-role march
     long long step;
     int table[64];
     int ntable;
@@ -259,11 +259,20 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
         P.stride_other = 0;
         P.seg = auto_segment(h, axis, P.N, P.npencil);
         P.nseg = (P.N + P.seg - 1) / P.seg;
-        auto kern = sweep_x_kernel<T, EOS, EMIT, ROWS>;
-        const size_t smem = sizeof(XSmem<T, ROWS>);
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        dim3 grid((unsigned)((P.npencil + ROWS - 1) / ROWS), (unsigned)P.nseg);
-        kern<<<grid, ROWS, smem, st>>>(P, k);
+        if (h->variant == 0) {
+            // warp-specialised x sweep: 128 rows per CTA, 4 producer + 4 consumer warps
+            auto kern = sweep_x_ws_kernel<T, EOS, EMIT>;
+            const size_t smem = sizeof(XvSmem<T>);
+            CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            dim3 grid((unsigned)((P.npencil + 127) / 128), (unsigned)P.nseg);
+            kern<<<grid, 256, smem, st>>>(P, k);
+        } else {
+            auto kern = sweep_x_kernel<T, EOS, EMIT, ROWS>;
+            const size_t smem = sizeof(XSmem<T, ROWS>);
+            CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            dim3 grid((unsigned)((P.npencil + ROWS - 1) / ROWS), (unsigned)P.nseg);
+            kern<<<grid, ROWS, smem, st>>>(P, k);
+        }
     } else {
         // y sweep: pencils (x,z), base = x + z*nx*ny;  z sweep: pencils (x,y), base = x + y*nx = flat
         const int other = axis == 1 ? 2 : 1;
@@ -271,8 +280,8 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
         P.stride_other = stride[other];
         P.seg = auto_segment(h, axis, P.N, P.npencil);
         P.nseg = (P.N + P.seg - 1) / P.seg;
-        if (h->variant == 1) {
-            // warp-specialised march (experimental): 128 pencils per CTA, 4 producer + 4 consumer warps
+        if (h->variant == 0) {
+            // warp-specialised march: 128 pencils per CTA, 4 producer + 4 consumer warps
             auto kern = sweep_strided_ws_kernel<T, EOS, EMIT>;
             const size_t smem = sizeof(WsSmem<T>);
             CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -646,6 +655,7 @@ long long shasta_step_index(const shasta_t* h) { return h ? h->step : -1; }
 const char* shasta_kernel_name(const shasta_t* h, int axis)
 {
     if (!h || axis < 0 || axis > 2) return "";
+    if (h->variant == 0) return axis == 0 ? "sweep_x_ws_kernel" : "sweep_strided_ws_kernel";
     return axis == 0 ? "sweep_x_kernel" : "sweep_strided_kernel";
 }
 

@@ -1030,4 +1030,163 @@ __global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> 
     flush_counts(cnt, P.counts);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Warp-specialised x sweep: the producer/consumer pair of sweep_strided_ws_kernel, with lane r marching
+// along ROW r of a 32-row strip.  The producer warp also runs the transposing loader: it copies 4-cell
+// (32 B = one sector) row pieces with cp.async into a ring of 12 cells per pair, laid out
+// ring[cell][field][row] with the cell stride padded to 168 doubles so that both the transposed fill
+// (lane -> (row, col) = (lane>>2 + 8k, lane&3)) and the marching reads (lane = row) are bank-conflict free.
+// The consumer warp stages its results in out[4 cells][field][row] and writes every finished 4-cell group
+// back as 32 B row pieces (the primitives of the last sweep are computed element-wise in that write-back).
+constexpr int XV_CH = 4;                // cells per load / store group
+constexpr int XV_R = 12;                // ring cells per pair (3 groups)
+constexpr int XV_SLOT = NF * 32 + 8;    // doubles per ring cell (168 = 8 mod 16: conflict-free transposed fill)
+
+template <typename T>
+struct XvPair {
+    T ring[XV_R][XV_SLOT];
+    T outb[XV_CH][XV_SLOT];
+    T msg[WS_Q][4][32];
+    unsigned cnt[4][32];
+};
+template <typename T>
+struct XvSmem {
+    XvPair<T> pair[4];
+};
+
+template <typename T, int EOS, bool EMIT>
+__global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constant__ SweepParams P,
+                                                            const __grid_constant__ Consts<T> k)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool producer = warp < 4;
+    XvPair<T>& S = reinterpret_cast<XvSmem<T>*>(smem_raw)->pair[warp & 3];
+    const int bar_id = 1 + (warp & 3);
+    const long long row0 = (long long)blockIdx.x * 128 + (warp & 3) * 32;
+    const bool idle = row0 >= P.npencil;                    // both warps of the pair leave together (after setmaxnreg)
+    const int nrows = (int)min(32LL, P.npencil - row0);
+    const int sg = blockIdx.y;
+    const int j0 = sg * P.seg;
+    const int j1 = min(P.N, j0 + P.seg);
+    const int ilo = j0 - GH;
+    const int N = P.N;
+    const int nsteps = (j1 - j0) + 2 * GH;                  // front cells ilo .. j1+3
+    const int nchunk = 2 * ((nsteps + 3) / 4);              // 2-step chunks, rounded to whole 4-cell groups
+    const int niter = nchunk + 2;                           // consumer runs one iteration behind; even
+    // lane -> element map of the transposed copies: col = lane & 3, rows (lane >> 2) + 8 kk
+    const int col = lane & 3, rsub = lane >> 2;
+
+    if (producer) {
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+        if (idle) return;
+        Producer<T, EOS> pr;
+        pr.init();
+        // group g = cells ilo+4g .. ilo+4g+3 -> ring cells (4g + col) % 12
+        auto load_group = [&](int g) {
+            const int i = ilo + XV_CH * g + col;
+            const int gi = ghost_index(i, N, P.periodic);
+            T* dst = &S.ring[(XV_CH * g + col) % XV_R][0];
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+                const int row = rsub + 8 * kk;
+                if (row < nrows) {
+                    const long long o = (row0 + row) * (long long)N + gi;
+#pragma unroll
+                    for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * 32 + row, (const T*)P.in[f] + o);
+                }
+            }
+            cp_async_commit();
+        };
+        load_group(0);
+        int rslot = 0, g = 0;
+        // Group g+1 is issued at the start of group g into the ring cells of group g-2, which the consumer
+        // finished (as U_{i-1}) in the iteration before: it runs one 2-step iteration behind this warp.
+#define SHK_XPCHUNK(PH, NEWGROUP)                                                                    \
+        {                                                                                           \
+            if (NEWGROUP) {                                                                         \
+                load_group(g + 1);                                                                  \
+                cp_async_wait<1>();                                                                 \
+                __syncwarp();                                                                       \
+                ++g;                                                                                \
+            }                                                                                       \
+            T ua[NF], ub[NF], ma[4], mb[4];                                                         \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) ua[f] = S.ring[rslot][f * 32 + lane];     \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) ub[f] = S.ring[rslot + 1][f * 32 + lane]; \
+            rslot = (rslot + 2 == XV_R) ? 0 : rslot + 2;                                            \
+            pr.template step<PH>(k, ua, ma);                                                        \
+            pr.template step<PH + 1>(k, ub, mb);                                                    \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane] = ma[q];               \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane] = mb[q];           \
+        }
+        for (int it = 0; it < niter; it += 2) {
+            if (it < nchunk) { SHK_XPCHUNK(0, true) }
+            pair_barrier(bar_id);
+            if (it + 1 < nchunk) { SHK_XPCHUNK(2, false) }
+            pair_barrier(bar_id);
+        }
+#undef SHK_XPCHUNK
+        cp_async_wait<0>();
+    } else {
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
+        if (idle) return;
+        Cnt cnt;
+        cnt.p = &S.cnt[0][lane]; cnt.stride = 32;
+        cnt.zero();
+        Consumer<T> co;
+        co.init();
+        int cslot = XV_R - 1;           // step t reads U of ring cell t-1 (t = 0: a don't-care warm-up value)
+        int t = 0;
+#define SHK_XCSTEP(PH)                                                                              \
+        {                                                                                           \
+            T uj[NF], msg[4], un[NF], pv[6];                                                        \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) uj[f] = S.ring[cslot][f * 32 + lane];     \
+            cslot = (cslot + 1 == XV_R) ? 0 : cslot + 1;                                            \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane];              \
+            co.template step<PH>(uj, msg, un);                                                      \
+            if (t >= 2 * GH && t < nsteps && lane < nrows) finish_cell<T, EOS, false>(k, un, pv, cnt); \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) S.outb[PH][f * 32 + lane] = un[f];       \
+            ++t;                                                                                    \
+        }
+        // write-back of the 4-cell group whose last cell was produced by step t-1: cells j0-8+4m .. +3
+        auto write_group = [&]() {
+            const int jo = ilo + (t - 4) - GH + col;
+            if (jo >= j0 && jo < j1) {
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk) {
+                    const int row = rsub + 8 * kk;
+                    if (row < nrows) {
+                        const long long o = (row0 + row) * (long long)N + jo;
+                        T u[NF];
+#pragma unroll
+                        for (int f = 0; f < NF; ++f) {
+                            u[f] = S.outb[col][f * 32 + row];
+                            ((T*)P.out[f])[o] = u[f];
+                        }
+                        if (EMIT) {
+                            T pv[6];
+                            emit_primitives<T, EOS>(k, u, pv, cnt);
+#pragma unroll
+                            for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[o] = pv[q];
+                        }
+                    }
+                }
+            }
+        };
+        for (int it = 0; it < niter; it += 2) {
+            if (it >= 1 && it - 1 < nchunk) {
+                SHK_XCSTEP(2) SHK_XCSTEP(3)
+                __syncwarp();
+                write_group();
+                __syncwarp();
+            }
+            pair_barrier(bar_id);
+            if (it < nchunk) { SHK_XCSTEP(0) SHK_XCSTEP(1) }
+            pair_barrier(bar_id);
+        }
+#undef SHK_XCSTEP
+        flush_counts(cnt, P.counts);
+    }
+}
+
 }  // namespace shk

@@ -60,15 +60,15 @@ def test_segmentation_does_not_change_the_answer(oracle, segment):
 
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
 @pytest.mark.parametrize("segment", [0, 9])
-def test_warp_specialised_variant(oracle, bc, segment):
-    # SHASTA_VARIANT 1: producer/consumer warp pairs for the y/z sweeps; same arithmetic as the default kernel
+def test_single_role_variant(oracle, bc, segment):
+    # SHASTA_VARIANT 1: one marching thread per pencil (the default, 0, is a producer/consumer warp pair)
     c = inputs.random_state(150, 21, 19, seed=31 + bc, kind="rough", boundary=bc)
     ref, _ = parity.run_oracle(oracle, c, steps=2)
     got, _ = parity.run_gpu(c, steps=2, variant=1, segment=segment)
-    assert_kernel_parity(got, ref, f"ws variant bc {bc} segment {segment}")
-    # not bitwise the default kernel: the producer rounds the source increment before the consumer adds it
+    assert_kernel_parity(got, ref, f"variant 1 bc {bc} segment {segment}")
+    # not bitwise the default kernel: there the producer rounds the source increment before the consumer adds it
     base, _ = parity.run_gpu(c, steps=2, segment=segment)
-    parity.assert_parity(got, base, 1e-13, label="ws vs default")
+    parity.assert_parity(got, base, 1e-13, label="variant 1 vs default")
 
 
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
