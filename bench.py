@@ -256,7 +256,7 @@ def ours(args):
             a = table[(3 * (base + i) + k) % len(table)]
             s.sweep(a, emit_primitives=(k == 2))
             evs[3 * i + k + 1].record(stream)
-            kinds.append((s.kernel_name(a), k == 2))
+            kinds.append((s.kernel_name(a) + ("<emit>" if k == 2 else ""), k == 2))
     barrier()
     sampler.windows.append((w0, time.perf_counter()))
     per = {}

@@ -298,7 +298,7 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
     return 0;
 }
 
-int launch_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
+int launch_sweep_raw(shasta_t* h, int axis, bool emit, cudaStream_t st)
 {
     const bool general = use_general_eos(h);
     if (h->precision == 64) {
@@ -331,6 +331,20 @@ int refresh_prims_t(shasta_t* h, cudaStream_t st)
     h->launches++;
     h->prims_valid = true;
     return 0;
+}
+
+// One sweep.  When the LAST sweep of a step runs along x, its primitives are written by the element-wise
+// cons2prim kernel instead of the sweep's write-back: in the warp-specialised x kernel the consumer warp is the
+// critical one, and computing six more fields there costs more (+0.5 ms at 256^3) than re-reading the five
+// conserved fields once (88 B/cell, ~0.3 ms).  y/z sweeps emit in place (+0.08 ms).
+int launch_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
+{
+    if (emit && axis == 0 && h->variant == 0) {
+        int rc = launch_sweep_raw(h, axis, false, st);
+        if (rc) return rc;
+        return h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
+    }
+    return launch_sweep_raw(h, axis, emit, st);
 }
 
 // copy one stored field (T) into a caller fp64 device buffer
