@@ -182,34 +182,25 @@ SEED0 = 12060919
 # ------------------------------------------------------------------------------------------------
 def ours(args):
     import torch
-    import torch.distributed as dist
     from paper_1206_0919_b200 import inputs
     from paper_1206_0919_b200.shasta import Shasta
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1206_0919_b200 import replicas
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    rank, world, local = replicas.env()
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    replicas.init(use_cuda=True)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(use_cuda=True)
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, use_cuda=True)
 
     # one independent event per rank (weak scaling, replicas: DESIGN.md 9)
     n = args.size
-    c = inputs.hotspots(n, steps=args.steps, seed=SEED0 + rank)
+    c = inputs.hotspots(n, steps=args.steps, seed=replicas.event_seed(rank))
     ncell = n ** 3
     names = ("e", "n", "vx", "vy", "vz")
     host_in = [torch.from_numpy(c[k]).pin_memory() for k in names]
@@ -241,7 +232,7 @@ def ours(args):
     sampler.windows.append((w0, time.perf_counter()))
     launches = s.launch_count - l0
     ms_total = max_over_ranks(ev0.elapsed_time(ev1))
-    value = world * ncell * K / (ms_total * 1e-3)
+    value = replicas.aggregate_rate(ncell, K, ms_total, world)
 
     # ---- region B: the same K steps sweep by sweep, CUDA events around every kernel launch
     from paper_1206_0919_b200.shasta import BRANCH as table
@@ -337,8 +328,7 @@ def ours(args):
             "roofline": roofline, "step_roofline": step_roofline, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches, "ms_step_sum_of_kernels": ms_sweeps / K, "clocks": sampler.summary(),
         }))
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.finalize()
 
 
 def main():
