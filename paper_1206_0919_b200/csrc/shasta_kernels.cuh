@@ -1032,20 +1032,20 @@ __global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> 
 
 // ------------------------------------------------------------------------------------------------
 // Warp-specialised x sweep: the producer/consumer pair of sweep_strided_ws_kernel, with lane r marching
-// along ROW r of a 32-row strip.  The producer warp also runs the transposing loader: it copies 4-cell
-// (32 B = one sector) row pieces with cp.async into a ring of 12 cells per pair, laid out
-// ring[cell][field][row] with the cell stride padded to 168 doubles so that both the transposed fill
-// (lane -> (row, col) = (lane>>2 + 8k, lane&3)) and the marching reads (lane = row) are bank-conflict free.
-// The consumer warp stages its results in out[4 cells][field][row] and writes every finished 4-cell group
-// back as 32 B row pieces (the primitives of the last sweep are computed element-wise in that write-back).
-constexpr int XV_CH = 4;                // cells per load / store group
-constexpr int XV_R = 12;                // ring cells per pair (3 groups)
-constexpr int XV_SLOT = NF * 32 + 8;    // doubles per ring cell (168 = 8 mod 16: conflict-free transposed fill)
+// along ROW r of a 32-row strip.  Global traffic moves in 4-cell groups = 32 B row pieces (one sector);
+// in shared memory a (group, field) TILE is [32 rows][4 cells], dense (1 KB) -- the layout a TMA box
+// {4, 32} produces -- with the two 16 B halves of a row swapped when bit 2 of the row is set (the 32 B
+// swizzle).  The fill (cp.async, lane -> (row, col) = (lane>>2 + 8k, lane&3)) and the write-back are then
+// contiguous 256 B per instruction, the producer reads both cells of a 2-step chunk with one conflict-free
+// LDS.128 per field, and the consumer's single-cell accesses are 2-way conflicts at worst.
+constexpr int XV_CH = 4;                // cells per group
+constexpr int XV_G = 3;                 // ring groups per pair (12 cells)
+constexpr int XV_TILE = 32 * XV_CH;     // elements per (group, field) tile
 
 template <typename T>
 struct XvPair {
-    T ring[XV_R][XV_SLOT];
-    T outb[XV_CH][XV_SLOT];
+    T ring[XV_G][NF][XV_TILE];
+    T outb[NF][XV_TILE];
     T msg[WS_Q][4][32];
     unsigned cnt[4][32];
 };
@@ -1053,6 +1053,21 @@ template <typename T>
 struct XvSmem {
     XvPair<T> pair[4];
 };
+
+// two adjacent elements with one shared-memory access (LDS.128 for fp64); p is 2-element aligned
+__device__ __forceinline__ void load2(const double* p, double& a, double& b)
+{
+    const double2 v = *reinterpret_cast<const double2*>(p);
+    a = v.x; b = v.y;
+}
+__device__ __forceinline__ void load2(const float* p, float& a, float& b)
+{
+    const float2 v = *reinterpret_cast<const float2*>(p);
+    a = v.x; b = v.y;
+}
+
+// element offset of (row, cell c in 0..3) inside a tile
+__device__ __forceinline__ int xv_off(int row, int c) { return row * 4 + 2 * ((c >> 1) ^ ((row >> 2) & 1)) + (c & 1); }
 
 template <typename T, int EOS, bool EMIT>
 __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constant__ SweepParams P,
@@ -1074,7 +1089,7 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
     const int nsteps = (j1 - j0) + 2 * GH;                  // front cells ilo .. j1+3
     const int nchunk = 2 * ((nsteps + 3) / 4);              // 2-step chunks, rounded to whole 4-cell groups
     const int niter = nchunk + 2;                           // consumer runs one iteration behind; even
-    // lane -> element map of the transposed copies: col = lane & 3, rows (lane >> 2) + 8 kk
+    // lane -> element map of the group copies: col = lane & 3, rows (lane >> 2) + 8 kk
     const int col = lane & 3, rsub = lane >> 2;
 
     if (producer) {
@@ -1082,47 +1097,47 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
         if (idle) return;
         Producer<T, EOS> pr;
         pr.init();
-        // group g = cells ilo+4g .. ilo+4g+3 -> ring cells (4g + col) % 12
+        // group g = cells ilo+4g .. ilo+4g+3 -> ring tile g % 3
         auto load_group = [&](int g) {
-            const int i = ilo + XV_CH * g + col;
-            const int gi = ghost_index(i, N, P.periodic);
-            T* dst = &S.ring[(XV_CH * g + col) % XV_R][0];
+            const int gi = ghost_index(ilo + XV_CH * g + col, N, P.periodic);
+            T* dst = &S.ring[g % XV_G][0][0];
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
                 const int row = rsub + 8 * kk;
                 if (row < nrows) {
                     const long long o = (row0 + row) * (long long)N + gi;
+                    const int so = xv_off(row, col);
 #pragma unroll
-                    for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * 32 + row, (const T*)P.in[f] + o);
+                    for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * XV_TILE + so, (const T*)P.in[f] + o);
                 }
             }
             cp_async_commit();
         };
         load_group(0);
-        int rslot = 0, g = 0;
-        // Group g+1 is issued at the start of group g into the ring cells of group g-2, which the consumer
+        int g = 0;
+        const int sw = (lane >> 2) & 1;
+        // Group g+1 is issued at the start of group g into the tile of group g-2, which the consumer
         // finished (as U_{i-1}) in the iteration before: it runs one 2-step iteration behind this warp.
-#define SHK_XPCHUNK(PH, NEWGROUP)                                                                    \
+#define SHK_XPCHUNK(PH, HALF)                                                                        \
         {                                                                                           \
-            if (NEWGROUP) {                                                                         \
+            if (HALF == 0) {                                                                        \
                 load_group(g + 1);                                                                  \
                 cp_async_wait<1>();                                                                 \
                 __syncwarp();                                                                       \
-                ++g;                                                                                \
             }                                                                                       \
             T ua[NF], ub[NF], ma[4], mb[4];                                                         \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) ua[f] = S.ring[rslot][f * 32 + lane];     \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) ub[f] = S.ring[rslot + 1][f * 32 + lane]; \
-            rslot = (rslot + 2 == XV_R) ? 0 : rslot + 2;                                            \
+            const T* src = &S.ring[g % XV_G][0][lane * 4 + 2 * (HALF ^ sw)];                        \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) load2(src + f * XV_TILE, ua[f], ub[f]);   \
+            if (HALF == 1) ++g;                                                                     \
             pr.template step<PH>(k, ua, ma);                                                        \
             pr.template step<PH + 1>(k, ub, mb);                                                    \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane] = ma[q];               \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane] = mb[q];           \
         }
         for (int it = 0; it < niter; it += 2) {
-            if (it < nchunk) { SHK_XPCHUNK(0, true) }
+            if (it < nchunk) { SHK_XPCHUNK(0, 0) }
             pair_barrier(bar_id);
-            if (it + 1 < nchunk) { SHK_XPCHUNK(2, false) }
+            if (it + 1 < nchunk) { SHK_XPCHUNK(2, 1) }
             pair_barrier(bar_id);
         }
 #undef SHK_XPCHUNK
@@ -1135,17 +1150,20 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
         cnt.zero();
         Consumer<T> co;
         co.init();
-        int cslot = XV_R - 1;           // step t reads U of ring cell t-1 (t = 0: a don't-care warm-up value)
         int t = 0;
+        int gprev = XV_G - 1;           // tile of group floor((t-1)/4); t = 0 reads a don't-care warm-up value
+        // step t (phase PH = t & 3) reads U of cell t-1 = cell (PH+3)&3 of the tile of group floor((t-1)/4)
 #define SHK_XCSTEP(PH)                                                                              \
         {                                                                                           \
             T uj[NF], msg[4], un[NF], pv[6];                                                        \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) uj[f] = S.ring[cslot][f * 32 + lane];     \
-            cslot = (cslot + 1 == XV_R) ? 0 : cslot + 1;                                            \
+            const T* src = &S.ring[gprev][0][xv_off(lane, (PH + 3) & 3)];                           \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) uj[f] = src[f * XV_TILE];                 \
+            if (PH == 0) gprev = (gprev + 1 == XV_G) ? 0 : gprev + 1;                               \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane];              \
             co.template step<PH>(uj, msg, un);                                                      \
             if (t >= 2 * GH && t < nsteps && lane < nrows) finish_cell<T, EOS, false>(k, un, pv, cnt); \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) S.outb[PH][f * 32 + lane] = un[f];       \
+            T* dst = &S.outb[0][xv_off(lane, PH)];                                                  \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) dst[f * XV_TILE] = un[f];                 \
             ++t;                                                                                    \
         }
         // write-back of the 4-cell group whose last cell was produced by step t-1: cells j0-8+4m .. +3
@@ -1157,10 +1175,11 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
                     const int row = rsub + 8 * kk;
                     if (row < nrows) {
                         const long long o = (row0 + row) * (long long)N + jo;
+                        const int so = xv_off(row, col);
                         T u[NF];
 #pragma unroll
                         for (int f = 0; f < NF; ++f) {
-                            u[f] = S.outb[col][f * 32 + row];
+                            u[f] = S.outb[f][so];
                             ((T*)P.out[f])[o] = u[f];
                         }
                         if (EMIT) {
