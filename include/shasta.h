@@ -43,6 +43,9 @@ typedef struct shasta shasta_t;   /* opaque */
 #define SHASTA_VARIANT    5   /* tuning: sweep kernels, 0 = producer/consumer warp pair per 32 pencils (default),
                                  1 = one marching thread per pencil; same scheme, results agree to rounding */
 
+#define SHASTA_NO_TMA     6   /* test hook: 1 = the x sweep fills/drains its tiles with cp.async + stores even
+                                 where TMA is usable (fp64, even nx); default 0                          */
+
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only
  * (eqs. (15)-(17)); dx enters shasta_conserved_totals.  0 < lambda <= 0.5

@@ -33,11 +33,14 @@ struct shasta {
     int periodic;
     int precision;          // 64 | 32
     int seg_override;
+    int no_tma;             // test hook: 1 = x sweep through cp.async even where TMA is possible
     int variant;            // 0: warp-specialised sweeps (producer/consumer warp pairs, default), 1: single-role march
     long long step;
     int table[64];
     int ntable;
     void* U[2][NF];         // conserved, ping-pong, natural order E,Mx,My,Mz,R
+    CUtensorMap tmap[2][NF]; // TMA maps of U (x sweep), valid when have_tmap
+    bool have_tmap;
     void* prim[6];          // e,p,n,vx,vy,vz
     double* stage;          // fp64 staging (5 fields) for host<->device and fp32 conversion
     int cur;
@@ -71,6 +74,8 @@ int fail(shasta_t* h, int code, const char* fmt, ...)
 
 size_t esize(const shasta_t* h) { return h->precision == 64 ? 8 : 4; }
 
+int make_tensor_maps(shasta_t* h);
+
 int ensure_alloc(shasta_t* h)
 {
     if (h->allocated) return 0;
@@ -83,6 +88,39 @@ int ensure_alloc(shasta_t* h)
     CK(cudaMalloc(&h->d_partial, sizeof(double) * RED_BLOCKS * NF * 2));
     CK(cudaMallocHost(&h->h_partial, sizeof(double) * RED_BLOCKS * NF * 2));
     h->allocated = true;
+    return make_tensor_maps(h);
+}
+
+// TMA tensor maps of the conserved fields for the x sweep: 2-D {nx, ny*nz}, box {4 cells, 32 rows}, 32 B swizzle
+// (the shared-memory tile layout of sweep_x_ws_kernel).  Needs 16 B row strides: fp64 and even nx; otherwise the
+// kernel's cp.async path is used.  The driver entry point is resolved at run time (libshasta.so does not link libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int make_tensor_maps(shasta_t* h)
+{
+    h->have_tmap = false;
+    if (h->precision != 64 || (h->nx % 2) != 0 || h->nx < 4) return 0;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return 0;                                   // no TMA: the cp.async path still works
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny * (cuuint64_t)h->nz};
+    const cuuint64_t strides[1] = {(cuuint64_t)h->nx * sizeof(double)};
+    const cuuint32_t box[2] = {(cuuint32_t)XV_CH, 32u};
+    const cuuint32_t estr[2] = {1u, 1u};
+    for (int b = 0; b < 2; ++b)
+        for (int f = 0; f < NF; ++f) {
+            CUresult r = ((EncodeTiledFn)fn)(&h->tmap[b][f], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, h->U[b][f], dims, strides,
+                                             box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B,
+                                             CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return 0;
+        }
+    h->have_tmap = true;
     return 0;
 }
 
@@ -261,11 +299,29 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
         P.nseg = (P.N + P.seg - 1) / P.seg;
         if (h->variant == 0) {
             // warp-specialised x sweep: 128 rows per CTA, 4 producer + 4 consumer warps
-            auto kern = sweep_x_ws_kernel<T, EOS, EMIT>;
+            XMaps maps;
+            const bool tma = h->have_tmap && sizeof(T) == 8 && !h->no_tma;
+            if (tma) {
+                maps.in[0] = h->tmap[src][0]; maps.out[0] = h->tmap[dst][0];
+                for (int c = 0; c < 3; ++c) {
+                    maps.in[1 + c] = h->tmap[src][1 + perm[axis][c]];
+                    maps.out[1 + c] = h->tmap[dst][1 + perm[axis][c]];
+                }
+                maps.in[4] = h->tmap[src][4]; maps.out[4] = h->tmap[dst][4];
+            } else {
+                memset(&maps, 0, sizeof(maps));
+            }
             const size_t smem = sizeof(XvSmem<T>);
-            CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             dim3 grid((unsigned)((P.npencil + 127) / 128), (unsigned)P.nseg);
-            kern<<<grid, 256, smem, st>>>(P, k);
+            if (tma) {
+                auto kern = sweep_x_ws_kernel<T, EOS, EMIT, true>;
+                CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                kern<<<grid, 256, smem, st>>>(P, k, maps);
+            } else {
+                auto kern = sweep_x_ws_kernel<T, EOS, EMIT, false>;
+                CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                kern<<<grid, 256, smem, st>>>(P, k, maps);
+            }
         } else {
             auto kern = sweep_x_kernel<T, EOS, EMIT, ROWS>;
             const size_t smem = sizeof(XSmem<T, ROWS>);
@@ -439,6 +495,9 @@ int shasta_set_option(shasta_t* h, int key, double value)
         if (!(value >= 0.0)) return fail(h, SHASTA_EINVAL, "SHASTA_SEGMENT must be >= 0");
         h->seg_override = (int)value;
         if (h->seg_override > 0 && h->seg_override < 8) h->seg_override = 8;
+        return 0;
+    case SHASTA_NO_TMA:
+        h->no_tma = value != 0.0;
         return 0;
     case SHASTA_VARIANT:
         if (value != 0.0 && value != 1.0) return fail(h, SHASTA_EINVAL, "SHASTA_VARIANT must be 0 or 1");

@@ -25,6 +25,7 @@
 //   * the flux limiter's min/max/sign run on the integer pipe (sign-magnitude ordering of doubles);
 //   * the register window rotates by NAME (march loop unrolled by 4, compile-time slots), not by moves.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -1044,11 +1045,55 @@ constexpr int XV_TILE = 32 * XV_CH;     // elements per (group, field) tile
 
 template <typename T>
 struct XvPair {
-    T ring[XV_G][NF][XV_TILE];
+    T ring[XV_G][NF][XV_TILE];          // tiles are 1 KB (fp64): 256 B aligned as the 32 B swizzle needs
     T outb[NF][XV_TILE];
     T msg[WS_Q][4][32];
     unsigned cnt[4][32];
+    unsigned long long bar[32];         // bar[0..2]: one mbarrier per ring tile group (TMA completion); rest: padding
 };
+
+// tensor maps of the x sweep (permuted field order like SweepParams::in/out): 2-D {nx, ny*nz}, box {4, 32},
+// CU_TENSOR_MAP_SWIZZLE_32B.  Only built for fp64 grids with even nx (TMA needs 16 B row strides).
+struct XMaps {
+    CUtensorMap in[NF];
+    CUtensorMap out[NF];
+};
+
+// ---- TMA / mbarrier PTX (sm_90+; SASS: UTMALDG / UTMASTG / SYNCS)
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int c0, int c1, const void* src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(map), "r"(c0), "r"(c1), "r"(smem_u32(src)) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 template <typename T>
 struct XvSmem {
     XvPair<T> pair[4];
@@ -1069,14 +1114,15 @@ __device__ __forceinline__ void load2(const float* p, float& a, float& b)
 // element offset of (row, cell c in 0..3) inside a tile
 __device__ __forceinline__ int xv_off(int row, int c) { return row * 4 + 2 * ((c >> 1) ^ ((row >> 2) & 1)) + (c & 1); }
 
-template <typename T, int EOS, bool EMIT>
+template <typename T, int EOS, bool EMIT, bool TMA>
 __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constant__ SweepParams P,
-                                                            const __grid_constant__ Consts<T> k)
+                                                            const __grid_constant__ Consts<T> k,
+                                                            const __grid_constant__ XMaps maps)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(1024) unsigned char smem_xv[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool producer = warp < 4;
-    XvPair<T>& S = reinterpret_cast<XvSmem<T>*>(smem_raw)->pair[warp & 3];
+    XvPair<T>& S = reinterpret_cast<XvSmem<T>*>(smem_xv)->pair[warp & 3];
     const int bar_id = 1 + (warp & 3);
     const long long row0 = (long long)blockIdx.x * 128 + (warp & 3) * 32;
     const bool idle = row0 >= P.npencil;                    // both warps of the pair leave together (after setmaxnreg)
@@ -1097,21 +1143,52 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
         if (idle) return;
         Producer<T, EOS> pr;
         pr.init();
-        // group g = cells ilo+4g .. ilo+4g+3 -> ring tile g % 3
+        // group g = cells ilo+4g .. ilo+4g+3 -> ring tile g % 3.  A group that lies inside [0, N) is one TMA box
+        // {4 cells, 32 rows} per field (rows beyond the grid are zero-filled, those lanes are idle); a group that
+        // touches a boundary needs the ghost map and goes through cp.async, element by element.
+        if (TMA) {
+            if (lane == 0) {
+#pragma unroll
+                for (int q = 0; q < XV_G; ++q) mbar_init(&S.bar[q], 1);
+            }
+            fence_proxy_async();
+            __syncwarp();
+        }
+        unsigned phase = 0;             // bit q: parity to wait for on bar[q]
+        auto group_is_tma = [&](int g) { const int x0 = ilo + XV_CH * g; return TMA && x0 >= 0 && x0 + XV_CH <= N && (x0 & 1) == 0; };   // box start 16 B aligned
         auto load_group = [&](int g) {
-            const int gi = ghost_index(ilo + XV_CH * g + col, N, P.periodic);
-            T* dst = &S.ring[g % XV_G][0][0];
+            const int q = g % XV_G;
+            if (group_is_tma(g)) {
+                if (lane == 0) {
+                    mbar_expect_tx(&S.bar[q], NF * XV_TILE * (unsigned)sizeof(T));
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk) {
-                const int row = rsub + 8 * kk;
-                if (row < nrows) {
-                    const long long o = (row0 + row) * (long long)N + gi;
-                    const int so = xv_off(row, col);
+                    for (int f = 0; f < NF; ++f)
+                        tma_load_2d(&S.ring[q][f][0], &maps.in[f], ilo + XV_CH * g, (int)row0, &S.bar[q]);
+                }
+            } else {
+                const int gi = ghost_index(ilo + XV_CH * g + col, N, P.periodic);
+                T* dst = &S.ring[q][0][0];
 #pragma unroll
-                    for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * XV_TILE + so, (const T*)P.in[f] + o);
+                for (int kk = 0; kk < 4; ++kk) {
+                    const int row = rsub + 8 * kk;
+                    if (row < nrows) {
+                        const long long o = (row0 + row) * (long long)N + gi;
+                        const int so = xv_off(row, col);
+#pragma unroll
+                        for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * XV_TILE + so, (const T*)P.in[f] + o);
+                    }
                 }
             }
-            cp_async_commit();
+            cp_async_commit();          // also for TMA groups (empty): keeps the wait_group arithmetic uniform
+        };
+        auto wait_group = [&](int g) {
+            cp_async_wait<1>();
+            if (group_is_tma(g)) {
+                const int q = g % XV_G;
+                mbar_wait(&S.bar[q], (phase >> q) & 1u);
+                phase ^= 1u << q;
+            }
+            __syncwarp();
         };
         load_group(0);
         int g = 0;
@@ -1122,8 +1199,7 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
         {                                                                                           \
             if (HALF == 0) {                                                                        \
                 load_group(g + 1);                                                                  \
-                cp_async_wait<1>();                                                                 \
-                __syncwarp();                                                                       \
+                wait_group(g);                                                                      \
             }                                                                                       \
             T ua[NF], ub[NF], ma[4], mb[4];                                                         \
             const T* src = &S.ring[g % XV_G][0][lane * 4 + 2 * (HALF ^ sw)];                        \
@@ -1192,17 +1268,40 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
                 }
             }
         };
+        // a finished group goes out as one TMA box per field when all of its cells are output cells of this
+        // segment (or are clipped by the grid edge); otherwise (and for EMIT) through the LSU write-back
+        bool store_pending = false;
         for (int it = 0; it < niter; it += 2) {
             if (it >= 1 && it - 1 < nchunk) {
                 SHK_XCSTEP(2) SHK_XCSTEP(3)
-                __syncwarp();
-                write_group();
-                __syncwarp();
+                const int jf = ilo + (t - 4) - GH;          // first cell of the finished group
+                if (TMA && !EMIT && (jf & 1) == 0 && jf >= j0 && jf < j1 && (jf + XV_CH <= j1 || j1 == N)) {
+                    fence_proxy_async();                    // generic-proxy writes of outb -> visible to the TMA engine
+                    __syncwarp();
+                    if (lane == 0) {
+#pragma unroll
+                        for (int f = 0; f < NF; ++f) tma_store_2d(&maps.out[f], jf, (int)row0, &S.outb[f][0]);
+                        tma_store_commit();
+                    }
+                    store_pending = true;
+                } else {
+                    __syncwarp();
+                    write_group();
+                    __syncwarp();
+                }
             }
             pair_barrier(bar_id);
-            if (it < nchunk) { SHK_XCSTEP(0) SHK_XCSTEP(1) }
+            if (it < nchunk) {
+                if (TMA && store_pending) {                 // outb is rewritten below: the TMA must have read it
+                    if (lane == 0) tma_store_wait_read();
+                    __syncwarp();
+                    store_pending = false;
+                }
+                SHK_XCSTEP(0) SHK_XCSTEP(1)
+            }
             pair_barrier(bar_id);
         }
+        if (TMA && lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 #undef SHK_XCSTEP
         flush_counts(cnt, P.counts);
     }

@@ -51,11 +51,11 @@ def run_oracle(oracle, c, steps=None, table=None, variant="strict"):
     return res, o
 
 
-def run_gpu(c, steps=None, table=None, precision=64, segment=0, host_io=False, variant=0):
+def run_gpu(c, steps=None, table=None, precision=64, segment=0, host_io=False, variant=0, no_tma=0):
     import torch
     from paper_1206_0919_b200.shasta import Shasta
     s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"],
-               precision=precision, segment=segment, variant=variant)
+               precision=precision, segment=segment, variant=variant, no_tma=no_tma)
     if table is not None:
         s.set_sweep_table(table)
     if host_io:

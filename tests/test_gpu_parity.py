@@ -72,6 +72,22 @@ def test_single_role_variant(oracle, bc, segment):
 
 
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("shape", [(38, 19, 23), (64, 5, 7), (130, 33, 2), (8, 40, 3)])
+@pytest.mark.parametrize("segment", [0, 8, 12, 24])
+def test_x_sweep_tma_and_cp_async_paths(oracle, bc, shape, segment):
+    # even nx: interior 4-cell groups of the x sweep move by TMA (UTMALDG/UTMASTG), boundary groups and groups that
+    # straddle a segment end by cp.async / stores; SHASTA_NO_TMA forces the latter everywhere.  Same bits either way.
+    nx, ny, nz = shape
+    c = inputs.random_state(nx, ny, nz, seed=nx + 3 * bc, kind="rough", boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=1, table=[0, 0, 0])
+    got, _ = parity.run_gpu(c, steps=1, table=[0, 0, 0], segment=segment)
+    assert_kernel_parity(got, ref, f"x sweep tma shape {shape} bc {bc} segment {segment}")
+    alt, _ = parity.run_gpu(c, steps=1, table=[0, 0, 0], segment=segment, no_tma=1)
+    for k in parity.CONS + parity.PRIM:
+        assert np.array_equal(got[k], alt[k]), k
+
+
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
 def test_general_eos_mass(oracle, bc):
     c = inputs.random_state(24, 20, 28, seed=4, kind="rough", gamma=5.0 / 3.0, mass=1.0, boundary=bc)
     ref, _ = parity.run_oracle(oracle, c, steps=6)
