@@ -795,7 +795,11 @@ struct WsSmem {
     unsigned cnt[4][WS_P];
 };
 
-__device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+// Producer/consumer hand-over of one warp pair: four named barriers (full[0..1], empty[0..1]) of 64 threads each,
+// 32 that arrive (do not wait) and 32 that sync (wait): the PTX producer/consumer pattern.  The producer may run up
+// to two 2-step chunks ahead of the consumer; chunk c uses slot c & 1.
+__device__ __forceinline__ void bar_sync64(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void bar_arrive64(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
 
 template <typename T, int EOS, bool EMIT>
 __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __grid_constant__ SweepParams P,
@@ -805,7 +809,7 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
     WsSmem<T>& S = *reinterpret_cast<WsSmem<T>*>(smem_raw);
     const int lane_p = threadIdx.x & (WS_P - 1);                // pencil slot inside the CTA
     const bool producer = threadIdx.x < WS_P;                   // warps 0-3: P, warps 4-7: C
-    const int bar_id = 1 + ((threadIdx.x >> 5) & 3);            // one named barrier per warp pair
+    const int bar_id = 4 * ((threadIdx.x >> 5) & 3);            // named barriers of this warp pair: full0, full1, empty0, empty1
     long long pen = (long long)blockIdx.x * WS_P + lane_p;
     const bool active = pen < P.npencil;
     if (!active) pen = P.npencil - 1;                           // idle lanes shadow a valid pencil, store nothing
@@ -859,11 +863,13 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane_p] = ma[q];             \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane_p] = mb[q];         \
         }
+        // lockstep: the consumer runs one 2-step iteration behind, one 64-thread barrier per iteration (the decoupled
+        // full/empty hand-over of the x kernel costs this kernel registers: ptxas spills, measured slower)
         for (int it = 0; it < niter; it += 2) {
             if (it < nchunk) { SHK_PCHUNK(0) }
-            pair_barrier(bar_id);
+            bar_sync64(bar_id);
             if (it + 1 < nchunk) { SHK_PCHUNK(2) }
-            pair_barrier(bar_id);
+            bar_sync64(bar_id);
         }
 #undef SHK_PCHUNK
         cp_async_wait<0>();
@@ -897,9 +903,9 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
         }
         for (int it = 0; it < niter; it += 2) {
             if (it >= 1 && it - 1 < nchunk) { SHK_CSTEP(2) SHK_CSTEP(3) }
-            pair_barrier(bar_id);
+            bar_sync64(bar_id);
             if (it < nchunk) { SHK_CSTEP(0) SHK_CSTEP(1) }
-            pair_barrier(bar_id);
+            bar_sync64(bar_id);
         }
 #undef SHK_CSTEP
         flush_counts(cnt, P.counts);
@@ -1123,7 +1129,7 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool producer = warp < 4;
     XvPair<T>& S = reinterpret_cast<XvSmem<T>*>(smem_xv)->pair[warp & 3];
-    const int bar_id = 1 + (warp & 3);
+    const int bar_id = 4 * (warp & 3);                      // full0, full1, empty0, empty1 of this pair
     const long long row0 = (long long)blockIdx.x * 128 + (warp & 3) * 32;
     const bool idle = row0 >= P.npencil;                    // both warps of the pair leave together (after setmaxnreg)
     const int nrows = (int)min(32LL, P.npencil - row0);
@@ -1134,7 +1140,6 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
     const int N = P.N;
     const int nsteps = (j1 - j0) + 2 * GH;                  // front cells ilo .. j1+3
     const int nchunk = 2 * ((nsteps + 3) / 4);              // 2-step chunks, rounded to whole 4-cell groups
-    const int niter = nchunk + 2;                           // consumer runs one iteration behind; even
     // lane -> element map of the group copies: col = lane & 3, rows (lane >> 2) + 8 kk
     const int col = lane & 3, rsub = lane >> 2;
 
@@ -1210,11 +1215,13 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane] = ma[q];               \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane] = mb[q];           \
         }
-        for (int it = 0; it < niter; it += 2) {
-            if (it < nchunk) { SHK_XPCHUNK(0, 0) }
-            pair_barrier(bar_id);
-            if (it + 1 < nchunk) { SHK_XPCHUNK(2, 1) }
-            pair_barrier(bar_id);
+        for (int c = 0; c < nchunk; c += 2) {                   // nchunk is even here
+            if (c >= 2) bar_sync64(bar_id + 2);
+            SHK_XPCHUNK(0, 0)
+            bar_arrive64(bar_id + 0);
+            if (c >= 1) bar_sync64(bar_id + 3);
+            SHK_XPCHUNK(2, 1)
+            bar_arrive64(bar_id + 1);
         }
 #undef SHK_XPCHUNK
         cp_async_wait<0>();
@@ -1271,35 +1278,33 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
         // a finished group goes out as one TMA box per field when all of its cells are output cells of this
         // segment (or are clipped by the grid edge); otherwise (and for EMIT) through the LSU write-back
         bool store_pending = false;
-        for (int it = 0; it < niter; it += 2) {
-            if (it >= 1 && it - 1 < nchunk) {
-                SHK_XCSTEP(2) SHK_XCSTEP(3)
-                const int jf = ilo + (t - 4) - GH;          // first cell of the finished group
-                if (TMA && !EMIT && (jf & 1) == 0 && jf >= j0 && jf < j1 && (jf + XV_CH <= j1 || j1 == N)) {
-                    fence_proxy_async();                    // generic-proxy writes of outb -> visible to the TMA engine
-                    __syncwarp();
-                    if (lane == 0) {
+        for (int c = 0; c < nchunk; c += 2) {                   // nchunk is even here
+            bar_sync64(bar_id + 0);
+            if (TMA && store_pending) {                     // outb is rewritten below: the TMA must have read it
+                if (lane == 0) tma_store_wait_read();
+                __syncwarp();
+                store_pending = false;
+            }
+            SHK_XCSTEP(0) SHK_XCSTEP(1)
+            if (c + 2 < nchunk) bar_arrive64(bar_id + 2);
+            bar_sync64(bar_id + 1);
+            SHK_XCSTEP(2) SHK_XCSTEP(3)
+            if (c + 3 < nchunk) bar_arrive64(bar_id + 3);
+            const int jf = ilo + (t - 4) - GH;              // first cell of the finished group
+            if (TMA && !EMIT && (jf & 1) == 0 && jf >= j0 && jf < j1 && (jf + XV_CH <= j1 || j1 == N)) {
+                fence_proxy_async();                        // generic-proxy writes of outb -> visible to the TMA engine
+                __syncwarp();
+                if (lane == 0) {
 #pragma unroll
-                        for (int f = 0; f < NF; ++f) tma_store_2d(&maps.out[f], jf, (int)row0, &S.outb[f][0]);
-                        tma_store_commit();
-                    }
-                    store_pending = true;
-                } else {
-                    __syncwarp();
-                    write_group();
-                    __syncwarp();
+                    for (int f = 0; f < NF; ++f) tma_store_2d(&maps.out[f], jf, (int)row0, &S.outb[f][0]);
+                    tma_store_commit();
                 }
+                store_pending = true;
+            } else {
+                __syncwarp();
+                write_group();
+                __syncwarp();
             }
-            pair_barrier(bar_id);
-            if (it < nchunk) {
-                if (TMA && store_pending) {                 // outb is rewritten below: the TMA must have read it
-                    if (lane == 0) tma_store_wait_read();
-                    __syncwarp();
-                    store_pending = false;
-                }
-                SHK_XCSTEP(0) SHK_XCSTEP(1)
-            }
-            pair_barrier(bar_id);
         }
         if (TMA && lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 #undef SHK_XCSTEP
