@@ -820,7 +820,7 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
     const long long base = (pen % P.nx) + (pen / P.nx) * P.stride_other;
     const int nsteps = (j1 - j0) + 2 * GH;                      // front cells j0-4 .. j1+3
     const int nchunk = (nsteps + 1) / 2;
-    const int niter = ((nchunk + 1) + 1) & ~1;                  // P: chunks 0..nchunk-1, C one iteration behind; even
+    const int nchunk2 = (nchunk + 1) & ~1;
 
     if (producer) {
         if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
@@ -863,13 +863,16 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane_p] = ma[q];             \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane_p] = mb[q];         \
         }
-        // lockstep: the consumer runs one 2-step iteration behind, one 64-thread barrier per iteration (the decoupled
-        // full/empty hand-over of the x kernel costs this kernel registers: ptxas spills, measured slower)
-        for (int it = 0; it < niter; it += 2) {
-            if (it < nchunk) { SHK_PCHUNK(0) }
-            bar_sync64(bar_id);
-            if (it + 1 < nchunk) { SHK_PCHUNK(2) }
-            bar_sync64(bar_id);
+        // decoupled hand-over (see bar_sync64): chunk c uses slot c & 1; nchunk is rounded up to even (a surplus
+        // chunk marches ghost cells and stores nothing)
+#pragma unroll 1
+        for (int c = 0; c < nchunk2; c += 2) {
+            if (c > 0) bar_sync64(bar_id + 2);
+            SHK_PCHUNK(0)
+            bar_arrive64(bar_id + 0);
+            if (c > 0) bar_sync64(bar_id + 3);
+            SHK_PCHUNK(2)
+            bar_arrive64(bar_id + 1);
         }
 #undef SHK_PCHUNK
         cp_async_wait<0>();
@@ -901,11 +904,14 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
             }                                                                                       \
             ++i;                                                                                    \
         }
-        for (int it = 0; it < niter; it += 2) {
-            if (it >= 1 && it - 1 < nchunk) { SHK_CSTEP(2) SHK_CSTEP(3) }
-            bar_sync64(bar_id);
-            if (it < nchunk) { SHK_CSTEP(0) SHK_CSTEP(1) }
-            bar_sync64(bar_id);
+#pragma unroll 1
+        for (int c = 0; c < nchunk2; c += 2) {
+            bar_sync64(bar_id + 0);
+            SHK_CSTEP(0) SHK_CSTEP(1)
+            if (c + 2 < nchunk2) bar_arrive64(bar_id + 2);
+            bar_sync64(bar_id + 1);
+            SHK_CSTEP(2) SHK_CSTEP(3)
+            if (c + 2 < nchunk2) bar_arrive64(bar_id + 3);
         }
 #undef SHK_CSTEP
         flush_counts(cnt, P.counts);
