@@ -681,7 +681,8 @@ __global__ void __launch_bounds__(SBLOCK) sweep_strided_kernel(SweepParams P, Co
 // source increments -lambda Delta(p v)/2-form for E and M_par of cell i-2.
 template <typename T, int EOS>
 struct Producer {
-    T u1[NF];           // U^n_1
+    // fields the producer needs: the Gamma-law pressure does not depend on R, so R's predictor is skipped there
+    static constexpr int NP = (EOS == EOS_GAMMA) ? 4 : NF;
     T ft[NF];           // predictor flux F~ at interface (i-2,i-1)
     T eps1;             // (lambda/2) v_1 (time n)
     T fE[2], fM[2];     // (p v)_1,_2 and p_1,_2 (time n)      slot (PH-k)&1
@@ -691,13 +692,15 @@ struct Producer {
     __device__ __forceinline__ void init()
     {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) u1[f] = ft[f] = T(0);
+        for (int f = 0; f < NF; ++f) ft[f] = T(0);
         eps1 = epsh2 = fE[0] = fE[1] = fM[0] = fM[1] = gE[0] = gE[1] = gM[0] = gM[1] = T(0);
     }
 
-    // consumes U^n at the front cell i; msg = {a_c, b_c, sE, sM} for the consumer's step i
+    // consumes U^n at the front cell i (u0) and at cell i-1 (u1: re-read from the ring by the caller, or the
+    // previous front cell still in registers -- never carried, so no hand-down moves);
+    // msg = {a_c, b_c, sE, sM} for the consumer's step i
     template <int PH>
-    __device__ __forceinline__ void step(const Consts<T>& k, const T (&u0)[NF], T (&msg)[4])
+    __device__ __forceinline__ void step(const Consts<T>& k, const T (&u1)[NF], const T (&u0)[NF], T (&msg)[4])
     {
         constexpr int S2 = PH & 1;              // time-n scalars _2 (new _0 takes its slot)
         constexpr int G3 = (PH + 1) & 1;        // half-step scalars _3 (new _1 takes its slot)
@@ -706,16 +709,16 @@ struct Producer {
         const T eps0 = k.hlam * v0;
         const T fE0 = p0 * v0;
         T ut[NF];
+        ut[NF - 1] = T(0);
         {                                                                   // S2
             const T q = (T(0.5) - eps1) * fast_rcp(T(1) + (eps0 - eps1));   // Q+_1, eq. (15)
             const T a = T(0.5) - q, b = (T(0.5) * q) * q;
 #pragma unroll
-            for (int f = 0; f < NF; ++f) {
+            for (int f = 0; f < NP; ++f) {
                 const T d = u0[f] - u1[f];                                  // eq. (16)
                 const T fl = t_fma(a, u1[f], -(b * d));
                 ut[f] = u1[f] - (fl - ft[f]);
                 ft[f] = fl;
-                u1[f] = u0[f];
             }
             ut[0] = t_fma(-k.qlam, fE0 - fE[S2], ut[0]);
             ut[1] = t_fma(-k.qlam, p0 - fM[S2], ut[1]);
@@ -853,13 +856,16 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
             prefetch();                                                                             \
             prefetch();                                                                             \
             cp_async_wait<WS_D - 1>();                                                              \
-            T ua[NF], ub[NF], ma[4], mb[4];                                                         \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) ua[f] = S.ring[rslot][f][lane_p];        \
+            T um[NF], ua[NF], ub[NF], ma[4], mb[4];                                                 \
+            um[NF - 1] = ua[NF - 1] = ub[NF - 1] = T(0);                                            \
+            const int mslot = (rslot == 0) ? WS_R - 1 : rslot - 1;      /* cell 2it-1 (first chunk: don't care) */ \
+            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) um[f] = S.ring[mslot][f][lane_p]; \
+            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) ua[f] = S.ring[rslot][f][lane_p]; \
             rslot = (rslot + 1 == WS_R) ? 0 : rslot + 1;                                            \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) ub[f] = S.ring[rslot][f][lane_p];        \
+            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) ub[f] = S.ring[rslot][f][lane_p]; \
             rslot = (rslot + 1 == WS_R) ? 0 : rslot + 1;                                            \
-            pr.template step<PH>(k, ua, ma);                                                        \
-            pr.template step<PH + 1>(k, ub, mb);                                                    \
+            pr.template step<PH>(k, um, ua, ma);                                                    \
+            pr.template step<PH + 1>(k, ua, ub, mb);                                                \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane_p] = ma[q];             \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane_p] = mb[q];         \
         }
@@ -1212,12 +1218,20 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
                 load_group(g + 1);                                                                  \
                 wait_group(g);                                                                      \
             }                                                                                       \
-            T ua[NF], ub[NF], ma[4], mb[4];                                                         \
-            const T* src = &S.ring[g % XV_G][0][lane * 4 + 2 * (HALF ^ sw)];                        \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) load2(src + f * XV_TILE, ua[f], ub[f]);   \
+            T um[NF], ua[NF], ub[NF], ma[4], mb[4];                                                 \
+            um[NF - 1] = ua[NF - 1] = ub[NF - 1] = T(0);                                            \
+            const int tile = g % XV_G;                                                              \
+            /* cell before the chunk: cell 1 of this tile (HALF 1) or cell 3 of the previous group's tile (HALF 0) */ \
+            const T* srm = HALF ? &S.ring[tile][0][xv_off(lane, 1)]                                 \
+                                : &S.ring[(tile + XV_G - 1) % XV_G][0][xv_off(lane, 3)];            \
+            const T* src = &S.ring[tile][0][lane * 4 + 2 * (HALF ^ sw)];                            \
+            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) {                      \
+                um[f] = srm[f * XV_TILE];                                                           \
+                load2(src + f * XV_TILE, ua[f], ub[f]);                                             \
+            }                                                                                       \
             if (HALF == 1) ++g;                                                                     \
-            pr.template step<PH>(k, ua, ma);                                                        \
-            pr.template step<PH + 1>(k, ub, mb);                                                    \
+            pr.template step<PH>(k, um, ua, ma);                                                    \
+            pr.template step<PH + 1>(k, ua, ub, mb);                                                \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane] = ma[q];               \
             _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane] = mb[q];           \
         }
