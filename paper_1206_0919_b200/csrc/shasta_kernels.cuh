@@ -741,7 +741,6 @@ struct Producer {
 
 template <typename T>
 struct Consumer {
-    T up[NF];           // U^n_2
     T dl[4][NF];        // Delta_2..Delta_5 (Delta_2 is formed in the step)   slot (PH-k)&3
     T fc[NF];           // corrector flux F at interface (i-3,i-2)
     T uh[2][NF];        // U^_3, U^_4                                         slot (PH-k)&1
@@ -752,14 +751,15 @@ struct Consumer {
     {
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-            up[f] = dl[0][f] = dl[1][f] = dl[2][f] = dl[3][f] = fc[f] = T(0);
+            dl[0][f] = dl[1][f] = dl[2][f] = dl[3][f] = fc[f] = T(0);
             uh[0][f] = uh[1][f] = dh[0][f] = dh[1][f] = a5[f] = T(0);
         }
     }
 
-    // consumes U^n_{i-1} and the producer's message of step i; produces U^{n+1} of cell i-4 (before Pi)
+    // consumes U^n_{i-2} (up), U^n_{i-1} (uj) -- both read from the ring by the caller, never carried -- and the
+    // producer's message of step i; produces U^{n+1} of cell i-4 (before Pi)
     template <int PH>
-    __device__ __forceinline__ void step(const T (&uj)[NF], const T (&msg)[4], T (&un)[NF])
+    __device__ __forceinline__ void step(const T (&up)[NF], const T (&uj)[NF], const T (&msg)[4], T (&un)[NF])
     {
         constexpr int D2 = (PH + 2) & 3, D3 = (PH + 1) & 3, D4 = PH & 3, D5 = (PH + 3) & 3;
         constexpr int H3 = (PH + 1) & 1, H4 = PH & 1;
@@ -781,14 +781,13 @@ struct Consumer {
             a5[f] = a4;
             dh[E5][f] = dh3;
             uh[H4][f] = uh2;
-            up[f] = uj[f];
         }
     }
 };
 
 constexpr int WS_P = 128;         // pencils per CTA (4 producer warps + 4 consumer warps)
 constexpr int WS_R = 12;          // U ring slots per pencil
-constexpr int WS_D = WS_R - 4;    // prefetch distance; D-1 copies stay in flight behind the current chunk (see below)
+constexpr int WS_D = WS_R - 5;    // prefetch distance; D-1 copies stay in flight behind the current chunk (see below)
 constexpr int WS_Q = 4;           // message queue slots (2 chunks of 2 steps)
 
 template <typename T>
@@ -846,9 +845,9 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
         int rslot = 0;
         // Copies: before chunk `it` cells 0 .. 2it+D-2 are issued; its two prefetches add cells 2it+D-1, 2it+D, and
         // wait_group<D-1> then leaves at most the D-1 youngest pending, i.e. cells <= 2it+1 (this chunk) are complete.
-        // Slot reuse: those two refill the slots of cells 2it+D-1-R = 2it-5 and 2it-4, which the consumer read
-        // (as U_{i-1} of chunk it-2: cells <= 2it-4) before the barrier that ended iteration it-1; in iteration `it`
-        // it reads cells 2it-3, 2it-2.
+        // Slot reuse (D = R-5): those two refill the slots of cells 2it-6 and 2it-5.  The producer enters chunk `it`
+        // only after the consumer released chunk it-2; the consumer may still be inside chunk it-1, where it reads
+        // cells 2it-4 .. 2it-2 (U_{i-2}, U_{i-1} of its two steps): all younger than the refilled ones.
         // One chunk = two steps: both front cells are fetched first, then the two steps' arithmetic runs with no
         // asm/memory fence in between, so the scheduler may overlap S3 of the first with S1 of the second.
 #define SHK_PCHUNK(PH)                                                                              \
@@ -893,33 +892,46 @@ __global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __g
         // ring's last slot, never written before: a don't-care warm-up value, finite or not it is retired)
         int cslot = WS_R - 1;
         int i = j0 - GH;
-#define SHK_CSTEP(PH)                                                                               \
+#define SHK_CSTORE(UN)                                                                              \
         {                                                                                           \
-            T uj[NF], msg[4], un[NF];                                                               \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) uj[f] = S.ring[cslot][f][lane_p];        \
-            cslot = (cslot + 1 == WS_R) ? 0 : cslot + 1;                                            \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane_p];            \
-            co.template step<PH>(uj, msg, un);                                                      \
             const int jo = i - GH;                                                                  \
             if (jo >= j0 && jo < j1 && active) {                                                    \
                 T pv[6];                                                                            \
-                finish_cell<T, EOS, EMIT>(k, un, pv, cnt);                                          \
+                finish_cell<T, EOS, EMIT>(k, UN, pv, cnt);                                          \
                 const long long o = base + (long long)jo * sa;                                      \
-                _Pragma("unroll") for (int f = 0; f < NF; ++f) ((T*)P.out[f])[o] = un[f];           \
+                _Pragma("unroll") for (int f = 0; f < NF; ++f) ((T*)P.out[f])[o] = UN[f];           \
                 if (EMIT) { _Pragma("unroll") for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[o] = pv[q]; } \
             }                                                                                       \
             ++i;                                                                                    \
         }
+        // one chunk = steps t, t+1: cells t-2, t-1, t are read from the ring (no carried U, no hand-down moves)
+#define SHK_CCHUNK(PH)                                                                              \
+        {                                                                                           \
+            T uq[NF], ua[NF], ub[NF], msg[4], un[NF];                                               \
+            const int qslot = (cslot == 0) ? WS_R - 1 : cslot - 1;                                  \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) uq[f] = S.ring[qslot][f][lane_p];        \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) ua[f] = S.ring[cslot][f][lane_p];        \
+            cslot = (cslot + 1 == WS_R) ? 0 : cslot + 1;                                            \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) ub[f] = S.ring[cslot][f][lane_p];        \
+            cslot = (cslot + 1 == WS_R) ? 0 : cslot + 1;                                            \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane_p];            \
+            co.template step<PH>(uq, ua, msg, un);                                                  \
+            SHK_CSTORE(un)                                                                          \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH + 1][q][lane_p];        \
+            co.template step<PH + 1>(ua, ub, msg, un);                                              \
+            SHK_CSTORE(un)                                                                          \
+        }
 #pragma unroll 1
         for (int c = 0; c < nchunk2; c += 2) {
             bar_sync64(bar_id + 0);
-            SHK_CSTEP(0) SHK_CSTEP(1)
+            SHK_CCHUNK(0)
             if (c + 2 < nchunk2) bar_arrive64(bar_id + 2);
             bar_sync64(bar_id + 1);
-            SHK_CSTEP(2) SHK_CSTEP(3)
+            SHK_CCHUNK(2)
             if (c + 2 < nchunk2) bar_arrive64(bar_id + 3);
         }
-#undef SHK_CSTEP
+#undef SHK_CCHUNK
+#undef SHK_CSTORE
         flush_counts(cnt, P.counts);
     }
 }
@@ -1254,20 +1266,35 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
         Consumer<T> co;
         co.init();
         int t = 0;
-        int gprev = XV_G - 1;           // tile of group floor((t-1)/4); t = 0 reads a don't-care warm-up value
-        // step t (phase PH = t & 3) reads U of cell t-1 = cell (PH+3)&3 of the tile of group floor((t-1)/4)
-#define SHK_XCSTEP(PH)                                                                              \
+        int gprev = XV_G - 1;           // tile of group floor((t-1)/4); t = 0 reads don't-care warm-up values
+        const int swc = (lane >> 2) & 1;
+#define SHK_XCFIN(UN, PH)                                                                           \
         {                                                                                           \
-            T uj[NF], msg[4], un[NF], pv[6];                                                        \
-            const T* src = &S.ring[gprev][0][xv_off(lane, (PH + 3) & 3)];                           \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) uj[f] = src[f * XV_TILE];                 \
-            if (PH == 0) gprev = (gprev + 1 == XV_G) ? 0 : gprev + 1;                               \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane];              \
-            co.template step<PH>(uj, msg, un);                                                      \
-            if (t >= 2 * GH && t < nsteps && lane < nrows) finish_cell<T, EOS, false>(k, un, pv, cnt); \
+            T pv[6];                                                                                \
+            if (t >= 2 * GH && t < nsteps && lane < nrows) finish_cell<T, EOS, false>(k, UN, pv, cnt); \
             T* dst = &S.outb[0][xv_off(lane, PH)];                                                  \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) dst[f * XV_TILE] = un[f];                 \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) dst[f * XV_TILE] = UN[f];                 \
             ++t;                                                                                    \
+        }
+        // one chunk = steps t, t+1 (t even): cells t-2, t-1 are one aligned pair (LDS.128) of the tile `gprev`,
+        // cell t is the first cell of the next pair: of the next tile when t = 0 mod 4 (PH 0), of the same tile
+        // when t = 2 mod 4 (PH 2).  Nothing of U is carried in registers.
+#define SHK_XCCHUNK(PH)                                                                             \
+        {                                                                                           \
+            T uq[NF], ua[NF], ub[NF], msg[4], un[NF];                                               \
+            const T* s2 = &S.ring[gprev][0][lane * 4 + 2 * ((PH == 0 ? 1 : 0) ^ swc)];              \
+            if (PH == 0) gprev = (gprev + 1 == XV_G) ? 0 : gprev + 1;                               \
+            const T* s1 = &S.ring[gprev][0][lane * 4 + 2 * ((PH == 0 ? 0 : 1) ^ swc)];              \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) {                                        \
+                load2(s2 + f * XV_TILE, uq[f], ua[f]);                                              \
+                ub[f] = s1[f * XV_TILE];                                                            \
+            }                                                                                       \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane];              \
+            co.template step<PH>(uq, ua, msg, un);                                                  \
+            SHK_XCFIN(un, PH)                                                                       \
+            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH + 1][q][lane];          \
+            co.template step<PH + 1>(ua, ub, msg, un);                                              \
+            SHK_XCFIN(un, PH + 1)                                                                   \
         }
         // write-back of the 4-cell group whose last cell was produced by step t-1: cells j0-8+4m .. +3
         auto write_group = [&]() {
@@ -1305,10 +1332,10 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
                 __syncwarp();
                 store_pending = false;
             }
-            SHK_XCSTEP(0) SHK_XCSTEP(1)
+            SHK_XCCHUNK(0)
             if (c + 2 < nchunk) bar_arrive64(bar_id + 2);
             bar_sync64(bar_id + 1);
-            SHK_XCSTEP(2) SHK_XCSTEP(3)
+            SHK_XCCHUNK(2)
             if (c + 3 < nchunk) bar_arrive64(bar_id + 3);
             const int jf = ilo + (t - 4) - GH;              // first cell of the finished group
             if (TMA && !EMIT && (jf & 1) == 0 && jf >= j0 && jf < j1 && (jf + XV_CH <= j1 || j1 == N)) {
@@ -1327,7 +1354,8 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
             }
         }
         if (TMA && lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-#undef SHK_XCSTEP
+#undef SHK_XCCHUNK
+#undef SHK_XCFIN
         flush_counts(cnt, P.counts);
     }
 }
