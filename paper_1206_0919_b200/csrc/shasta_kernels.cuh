@@ -151,6 +151,14 @@ __device__ __forceinline__ double fast_sqrt(double w)
     return s;
 }
 __device__ __forceinline__ float fast_sqrt(float w) { return sqrtf(w); }
+// 1/sqrt(x), normal x > 0: seed 2^-20, two Newton steps (clamped cells, general-EOS Newton loop)
+__device__ __forceinline__ double fast_rsqrt(double x)
+{
+    double r = rsq64h(x);
+    r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
+    r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
+    return r;
+}
 
 // ------------------------------------------------------------------------------------------------
 // cons2prim: relativistic correction + EOS (phases 3-4; readings G6-G10).
@@ -201,16 +209,20 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
         const double mR = k.mass * R;
         double v = lo;
         for (int it = 0; it < 48; ++it) {
+            // no library sqrt / division in the loop: w2 >= 2e-12 (v <= 1 - delta) and dg >= E - (Gamma-1)|M| v > 0
+            // are normal positive numbers, so the MUFU-seeded fast_rsqrt / fast_rcp apply (<= 2 ulp; the iteration
+            // is self-correcting and the primitives after the loop are formed from the converged v)
             const double w2 = fma(-v, v, double(1));
-            const double w = sqrt(w2);
+            const double rw = fast_rsqrt(w2);
+            const double w = w2 * rw;
             const double praw = k.gm1 * ((E - Mabs * v) - mR * w);
             const bool pos = praw > double(0);
             const double P = pos ? praw : double(0);
-            const double dP = pos ? k.gm1 * (mR * v / w - Mabs) : double(0);
+            const double dP = pos ? k.gm1 * (mR * v * rw - Mabs) : double(0);
             const double g = fma(v, E + P, -Mabs);
             const double dg = fma(v, dP, E + P);
             if (g > double(0)) hi = v; else lo = v;
-            double vn = v - g / dg;
+            double vn = v - g * fast_rcp(dg);
             if (!(vn >= lo && vn <= hi)) vn = double(0.5) * (lo + hi);
             const double dv = fabs(vn - v);
             v = vn;
@@ -243,14 +255,6 @@ __device__ __forceinline__ bool c2p_is_vacuum(double E)
 __device__ __forceinline__ bool gt_nonneg(double a, double b)      // a > b for a, b >= 0, on the integer pipe
 {
     return __double_as_longlong(a) > __double_as_longlong(b);
-}
-// 1/sqrt(x), normal x > 0: seed 2^-20, two Newton steps (only on the clamped branch)
-__device__ __forceinline__ double fast_rsqrt(double x)
-{
-    double r = rsq64h(x);
-    r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
-    r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
-    return r;
 }
 
 // Fast path, fp64, p = (Gamma-1) e.  y = 1/h, h = (b + sqrt(disc))/2 with b = Gamma E, disc = b^2 - 4 c,
