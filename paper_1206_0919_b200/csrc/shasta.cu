@@ -256,16 +256,34 @@ int ew_grid(const shasta_t* h, int threads)
 }
 
 // ---------------------------------------------------------------- sweep launch
+// Cells marched per work item.  Every segment re-marches 8 halo cells, so long segments are cheap per cell, but
+// the grid must fill the machine: a sweep kernel runs 2 CTAs of 128 pencils per SM (`slots` CTAs at once).
+// Measured on B200 (segment scan at 64^3 .. 512^3): when one layer of CTAs is already >= 3 waves the
+// whole pencil is one segment; large grids want the longest segments that still give ~3 waves (256^3: 2 x 128
+// cells); grids that fit into one wave want that wave as full as possible (128^3: 2 x 64, 64^3: 4 x 16).
 int auto_segment(const shasta_t* h, int axis, int N, long long npencil)
 {
     if (h->seg_override > 0) return h->seg_override < N ? h->seg_override : N;
-    // enough work items for ~4 waves of resident threads, segments not shorter than 32 cells
-    const long long resident = (long long)h->sm_count * 256;
-    long long nseg = (4 * resident + npencil - 1) / npencil;
-    if (nseg < 1) nseg = 1;
+    const long long slots = 2LL * h->sm_count;                     // CTAs resident at once
+    const long long base = (npencil + 127) / 128;                  // CTAs per layer of segments
+    const long long max_nseg = N / 16 > 1 ? N / 16 : 1;            // segments not shorter than 16 cells
+    long long nseg = 1;
+    if (base < 3 * slots) {
+        const long long one_wave = slots / base;                   // layers that fit one wave (0: none)
+        const long long three_waves = (3 * slots + base - 1) / base;
+        double best = 1e300;
+        const long long cand[2] = {one_wave, three_waves};
+        for (int c = 0; c < 2; ++c) {
+            long long n = cand[c] < 1 ? 0 : (cand[c] > max_nseg ? max_nseg : cand[c]);
+            if (n < 1) continue;
+            const double seg = (double)((N + n - 1) / n);
+            const double waves = (double)(base * n) / (double)slots;
+            const double t = (waves < 1.0 ? 1.0 : waves) * (seg + 8.0);
+            if (t < best) { best = t; nseg = n; }
+        }
+    }
     long long seg = (N + nseg - 1) / nseg;
-    if (seg < 32) seg = 32;
-    if (axis == 0) seg = ((seg + XCH - 1) / XCH) * XCH;   // chunk-aligned segments for the x sweep
+    if (axis == 0) seg = ((seg + XCH - 1) / XCH) * XCH;   // group-aligned segments for the x sweep
     return (int)(seg < N ? seg : N);
 }
 
