@@ -1201,6 +1201,10 @@ __global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constan
         auto group_is_tma = [&](int g) { const int x0 = ilo + XV_CH * g; return TMA && x0 >= 0 && x0 + XV_CH <= N && (x0 & 1) == 0; };   // box start 16 B aligned
         auto load_group = [&](int g) {
             const int q = g % XV_G;
+            if (2 * g >= nchunk) {      // past the last group: nothing may be left in flight when the CTA exits
+                cp_async_commit();
+                return;
+            }
             if (group_is_tma(g)) {
                 if (lane == 0) {
                     mbar_expect_tx(&S.bar[q], NF * XV_TILE * (unsigned)sizeof(T));
