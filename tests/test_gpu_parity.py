@@ -109,6 +109,18 @@ def test_uniform_state_stays_uniform_bitwise():
         assert torch.equal(before[k], after[k]), k
 
 
+@pytest.mark.parametrize("shape", [(96, 40, 24), (70, 45, 50)])
+def test_run_to_run_bitwise_reproducible(shape):
+    # the producer/consumer kernels reuse shared-memory ring and queue slots under barrier protocols: a race there
+    # would show up as run-to-run differences (compute-sanitizer is closed on this pool).  Six steps = all axis orders.
+    c = inputs.random_state(*shape, seed=99, kind="rough")
+    first, _ = parity.run_gpu(c, steps=6)
+    for _ in range(4):
+        again, _ = parity.run_gpu(c, steps=6)
+        for k in parity.CONS + parity.PRIM:
+            assert np.array_equal(first[k], again[k]), k
+
+
 def test_vacuum_and_superluminal_cells(oracle):
     # E <= 0 cells and |M| > E cells fed through set_conserved: projection + vacuum rule (P13)
     import torch
