@@ -36,6 +36,13 @@ B_SWEEP = 80.0      # algorithmic bytes per cell of one fused sweep: 5 fields re
 B_PRIM = 48.0       # + six primitive fields written by the last sweep of a step
 B_STEP = 3 * B_SWEEP + B_PRIM   # 288 B per cell-update
 HBM_FALLBACK_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+FP64_PER_CELL_SWEEP = 157.0     # fp64 instructions per cell of one Gamma-law sweep: producer 90 + consumer 67
+
+
+def sampler_clock_mhz(sampler):
+    """median SM clock seen so far by the NVML sampler (max clock if it has no samples yet)"""
+    xs = sorted(s[1] for s in sampler.samples)
+    return float(xs[len(xs) // 2]) if xs else float(getattr(sampler, "max_mhz", 1965))
 
 
 def parse_args():
@@ -274,6 +281,15 @@ def ours(args):
                 "avg_launch_ms": dom["ms"] / dom["launches"], "share_of_step": dom["ms"] / ms_sweeps,
                 "kernels": {k: {"avg_launch_ms": v["ms"] / v["launches"], "launches": v["launches"],
                                 "GB/s": v["bytes"] / (v["ms"] * 1e-3) / 1e9} for k, v in per.items()}}
+    # the second roof of this path: fp64 instructions.  157 per cell and sweep (SASS count of the
+    # Gamma-law producer 90 + consumer 67), 64 results/clk/SM measured on B200, at the SM clock sampled in this run
+    clk = sampler_clock_mhz(sampler)
+    fp64_peak = 64.0 * torch.cuda.get_device_properties(local).multi_processor_count * clk * 1e6 / 1e9
+    fp64_ach = ncell * FP64_PER_CELL_SWEEP / (dom["ms"] / dom["launches"] * 1e-3) / 1e9
+    alu_roofline = {"bound": "alu", "kernel": dom_name, "achieved": fp64_ach, "peak": fp64_peak,
+                    "unit": "G fp64 warp-lane results/s", "frac": fp64_ach / fp64_peak,
+                    "per_cell_sweep": FP64_PER_CELL_SWEEP, "clock_mhz": clk,
+                    "note": "halo re-march (+6 %) and rare-path instructions not counted in achieved"}
     step_gbs = value / world * B_STEP * (args.precision / 64.0) / 1e9
     step_roofline = {"bytes_per_cell_update": B_STEP * (args.precision / 64.0), "achieved": step_gbs,
                      "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,
@@ -325,7 +341,7 @@ def ours(args):
                        "l2": "state (2x5 fields ping-pong + 6 primitives, "
                              f"{16 * ncell * args.precision // 8 / 1e6:.0f} MB) is larger than the 126 MB L2; no flush",
                        "timing": "CUDA events on the launching stream, max over ranks"},
-            "roofline": roofline, "step_roofline": step_roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "roofline": roofline, "alu_roofline": alu_roofline, "step_roofline": step_roofline, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches, "ms_step_sum_of_kernels": ms_sweeps / K, "clocks": sampler.summary(),
         }))
     replicas.finalize()
