@@ -121,6 +121,19 @@ def test_run_to_run_bitwise_reproducible(shape):
             assert np.array_equal(first[k], again[k]), k
 
 
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("shape", [(37, 19, 23), (64, 33, 6)])
+def test_fp32_storage_kernel_level(oracle, bc, shape):
+    # fp32 storage + transport, fp64 cons2prim (row a7): ragged shapes, every axis, 2 steps: one fp32 rounding per
+    # operation, so a few 1e-7 relative; a wrong index or stride in the float instantiations would be O(1)
+    c = inputs.random_state(*shape, seed=5 + bc, kind="smooth", boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=2)
+    got, _ = parity.run_gpu(c, steps=2, precision=32)
+    errs = parity.field_errors(got, ref)
+    for k, (emax, el1) in errs.items():
+        assert emax <= 2e-5 and el1 <= 2e-6, (k, emax, el1)
+
+
 def test_vacuum_and_superluminal_cells(oracle):
     # E <= 0 cells and |M| > E cells fed through set_conserved: projection + vacuum rule (P13)
     import torch
