@@ -22,7 +22,7 @@ def _centres(n, dx):
 
 def _cfg(name, nx, ny, nz, dx, steps, bc, gamma, mass, e, n, vx, vy, vz, lam=0.4):
     shape = (nz, ny, nx)
-    f = lambda a: np.ascontiguousarray(np.broadcast_to(a, shape), dtype=np.float64)
+    f = lambda a: np.array(np.broadcast_to(a, shape), dtype=np.float64, order="C")     # writable copy
     return dict(name=name, nx=nx, ny=ny, nz=nz, dx=float(dx), lam=float(lam), steps=int(steps),
                 boundary=bc, gamma=float(gamma), mass=float(mass),
                 e=f(e), n=f(n), vx=f(vx), vy=f(vy), vz=f(vz))
