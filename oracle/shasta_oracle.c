@@ -25,12 +25,13 @@
  * Where the paper is silent the readings G1-G19 of SURVEY.md 8(c.2), restated in
  * DESIGN.md section 3, are used; each is marked "reading Gn" below.
  *
- * PARITY PINS (tests/test_oracle_*.py, -m "not gpu"): P1-P13 of DESIGN.md section 4.
- * "parity unpinned" AGAINST THE PAPER'S OWN CODE for: the predictor without
- * antidiffusion (reading G4), the causality projection Pi and its write-back
- * (G6-G8) and the ghost-extension boundary rule (G11): the paper prints no value
- * and no code for them; they are pinned only by self-consistency and by
- * convergence to the exact Riemann solution.
+ * PARITY PINS (tests/test_oracle_*.py, -m "not gpu"): P1-P15 of DESIGN.md section 4.  P14 (linear acoustic wave:
+ * observed order >= 1.8 only if v and the sources are centred at n+1/2) pins steps 3-5 of oracle_sweep_pencil,
+ * P15 (bitwise equality with a hand-extended pencil) pins ghost_index.
+ * "parity unpinned" AGAINST THE PAPER'S OWN CODE for the CHOICES the paper leaves open: the predictor
+ * without antidiffusion (reading G4; the R2 alternative is oracle_set_option key 4), the causality projection Pi
+ * and its write-back (G6-G8) and ghost extension of the sweep input as THE boundary rule (G11): the paper
+ * prints no value and no code for them; the arithmetic of each choice is pinned, the choice itself is not.
  */
 #include <math.h>
 #include <stdlib.h>
