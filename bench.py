@@ -54,7 +54,6 @@ def parse_args():
     ap.add_argument("--size", type=int, default=256, help="grid extent (256 = the metric's workload)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--segment", type=int, default=0, help="tuning: cells marched per work item (0 = auto)")
-    ap.add_argument("--variant", type=int, default=0, help="tuning: y/z kernel variant (SHASTA_VARIANT)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -215,7 +214,7 @@ def ours(args):
     dev_in = [t.cuda(non_blocking=True) for t in host_in]
     stream = torch.cuda.current_stream()
     s = Shasta(n, n, n, c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"], precision=args.precision,
-               segment=args.segment, variant=args.variant)
+               segment=args.segment)
     s.set_state(*dev_in)
     K, W = args.steps, args.warmup
     s.step(W)

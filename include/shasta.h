@@ -40,11 +40,10 @@ typedef struct shasta shasta_t;   /* opaque */
 #define SHASTA_PRECISION  2   /* 64 (default) | 32: storage and transport arithmetic (before set_state) */
 #define SHASTA_STEP_INDEX 3   /* step counter s indexing the axis table (resume / tests)                */
 #define SHASTA_SEGMENT    4   /* tuning: cells marched per work item along the sweep axis (0 = auto)    */
-#define SHASTA_VARIANT    5   /* tuning: sweep kernels, 0 = producer/consumer warp pair per 32 pencils (default),
-                                 1 = one marching thread per pencil; same scheme, results agree to rounding */
+#define SHASTA_VARIANT    5   /* reserved (round 1 had a second kernel family here); only 0 is accepted */
 
-#define SHASTA_NO_TMA     6   /* test hook: 1 = the x sweep fills/drains its tiles with cp.async + stores even
-                                 where TMA is usable (fp64, even nx); default 0                          */
+#define SHASTA_NO_TMA     6   /* test hook: 1 = the sweeps fill/drain their shared-memory tiles with cp.async + stores
+                                 even where TMA is usable (16 B row strides); same bits either way; default 0 */
 
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only

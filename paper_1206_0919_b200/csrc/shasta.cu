@@ -18,9 +18,6 @@ thread_local char g_create_err[256] = "";
 
 const int kBranch[18] = {0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2};
 
-constexpr int XROWS64 = 128;    // rows per CTA of the x sweep, fp64
-constexpr int XROWS32 = 256;    // fp32
-constexpr int STRIDED_BLOCK = shk::SBLOCK;
 constexpr int RED_BLOCKS = 592; // 4 per SM
 constexpr int RED_THREADS = 256;
 
@@ -34,13 +31,15 @@ struct shasta {
     int precision;          // 64 | 32
     int seg_override;
     int no_tma;             // test hook: 1 = x sweep through cp.async even where TMA is possible
-    int variant;            // 0: warp-specialised sweeps (producer/consumer warp pairs, default), 1: single-role march
     long long step;
     int table[64];
     int ntable;
     void* U[2][NF];         // conserved, ping-pong, natural order E,Mx,My,Mz,R
     CUtensorMap tmap[2][NF]; // TMA maps of U (x sweep), valid when have_tmap
     bool have_tmap;
+    CUtensorMap* d_xmaps;   // device copy of tmap: [buffer][field]
+    CUtensorMap* d_yzmaps;  // device: [buffer][kind: y4 {32,4,1}, z4 {32,1,4}, c1 {32,1,1}][field], 3-D maps over (x,y,z)
+    bool have_yzmap;
     void* prim[6];          // e,p,n,vx,vy,vz
     double* stage;          // fp64 staging (5 fields) for host<->device and fp32 conversion
     int cur;
@@ -75,6 +74,7 @@ int fail(shasta_t* h, int code, const char* fmt, ...)
 size_t esize(const shasta_t* h) { return h->precision == 64 ? 8 : 4; }
 
 int make_tensor_maps(shasta_t* h);
+int make_yz_maps(shasta_t* h);
 
 int ensure_alloc(shasta_t* h)
 {
@@ -88,7 +88,8 @@ int ensure_alloc(shasta_t* h)
     CK(cudaMalloc(&h->d_partial, sizeof(double) * RED_BLOCKS * NF * 2));
     CK(cudaMallocHost(&h->h_partial, sizeof(double) * RED_BLOCKS * NF * 2));
     h->allocated = true;
-    return make_tensor_maps(h);
+    make_tensor_maps(h);
+    return make_yz_maps(h);
 }
 
 // TMA tensor maps of the conserved fields for the x sweep: 2-D {nx, ny*nz}, box {4 cells, 32 rows}, 32 B swizzle
@@ -120,7 +121,63 @@ int make_tensor_maps(shasta_t* h)
                                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) return 0;
         }
+    if (!h->d_xmaps) CK(cudaMalloc(&h->d_xmaps, sizeof(h->tmap)));
+    CK(cudaMemcpy(h->d_xmaps, h->tmap, sizeof(h->tmap), cudaMemcpyHostToDevice));
     h->have_tmap = true;
+    return 0;
+}
+
+// y/z sweeps (sweep_yz_kernel): 3-D maps {nx, ny, nz}; a warp pair's 4-cell group of 32 pencils is one box {32, 4, 1}
+// (y) or {32, 1, 4} (z) per field, ghost groups are four {32, 1, 1} boxes.  Needs 16 B global strides (fp64: even nx,
+// fp32: nx % 4 == 0); otherwise the kernel's cp.async fill is used.
+int make_yz_maps(shasta_t* h)
+{
+    h->have_yzmap = false;
+    const size_t es = esize(h);
+    if (((size_t)h->nx * es) % 16 != 0 || h->nx < 32) return 0;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    const CUtensorMapDataType dt = es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const cuuint64_t dims[3] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz};
+    const cuuint64_t strides[2] = {(cuuint64_t)h->nx * es, (cuuint64_t)h->nx * (cuuint64_t)h->ny * es};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const cuuint32_t boxes[3][3] = {{32u, (cuuint32_t)YZ_CH, 1u}, {32u, 1u, (cuuint32_t)YZ_CH}, {32u, 1u, 1u}};
+    static CUtensorMap host[2][3][NF];
+    memset(host, 0, sizeof(host));
+    for (int b = 0; b < 2; ++b)
+        for (int m = 0; m < 3; ++m) {
+            if (m == 0 && h->ny < YZ_CH) continue;      // that axis falls back to cp.async (see launch)
+            if (m == 1 && h->nz < YZ_CH) continue;
+            for (int f = 0; f < NF; ++f) {
+                CUresult r = ((EncodeTiledFn)fn)(&host[b][m][f], dt, 3, h->U[b][f], dims, strides, boxes[m], estr,
+                                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                 CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                if (r != CUDA_SUCCESS) return 0;
+            }
+        }
+    if (!h->d_yzmaps) CK(cudaMalloc(&h->d_yzmaps, sizeof(host)));
+    CK(cudaMemcpy(h->d_yzmaps, host, sizeof(host), cudaMemcpyHostToDevice));
+    h->have_yzmap = true;
+    return 0;
+}
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per kernel and device, not once per launch
+int opt_in_smem(shasta_t* h, const void* kern, size_t smem)
+{
+    struct Key { const void* k; int dev; };
+    static Key done[256];
+    static int ndone = 0;
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    for (int i = 0; i < ndone; ++i)
+        if (done[i].k == kern && done[i].dev == dev) return 0;
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (ndone < 256) { done[ndone].k = kern; done[ndone].dev = dev; ++ndone; }
     return 0;
 }
 
@@ -180,9 +237,8 @@ __global__ void cons2prim_kernel(long long n, Consts<T> k, const T* E, const T* 
                                  const T* R, T* pe, T* pp, T* pn, T* pvx, T* pvy, T* pvz,
                                  unsigned long long* counts)
 {
-    unsigned lc[4] = {0u, 0u, 0u, 0u};
     Cnt cnt;
-    cnt.p = lc; cnt.stride = 1;
+    cnt.zero();
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
         T u[NF] = {E[i], Mx[i], My[i], Mz[i], R[i]};
@@ -261,11 +317,11 @@ int ew_grid(const shasta_t* h, int threads)
 // Measured on B200 (segment scan at 64^3 .. 512^3): when one layer of CTAs is already >= 3 waves the
 // whole pencil is one segment; large grids want the longest segments that still give ~3 waves (256^3: 2 x 128
 // cells); grids that fit into one wave want that wave as full as possible (128^3: 2 x 64, 64^3: 4 x 16).
-int auto_segment(const shasta_t* h, int axis, int N, long long npencil)
+int auto_segment(const shasta_t* h, int axis, int N, long long base)
 {
     if (h->seg_override > 0) return h->seg_override < N ? h->seg_override : N;
     const long long slots = 2LL * h->sm_count;                     // CTAs resident at once
-    const long long base = (npencil + 127) / 128;                  // CTAs per layer of segments
+    // base = CTAs per layer of segments
     const long long max_nseg = N / 16 > 1 ? N / 16 : 1;            // segments not shorter than 16 cells
     long long nseg = 1;
     if (base < 3 * slots) {
@@ -283,7 +339,7 @@ int auto_segment(const shasta_t* h, int axis, int N, long long npencil)
         }
     }
     long long seg = (N + nseg - 1) / nseg;
-    if (axis == 0) seg = ((seg + XCH - 1) / XCH) * XCH;   // group-aligned segments for the x sweep
+    if (axis == 0) seg = ((seg + 7) / 8) * 8;             // even, group-aligned segments for the x sweep (TMA boxes)
     return (int)(seg < N ? seg : N);
 }
 
@@ -307,63 +363,67 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
     P.N = n[axis];
     P.stride_axis = stride[axis];
     P.periodic = h->periodic;
+    P.axis = axis;
     P.counts = h->d_counts;
     const Consts<T> k = make_consts<T>(h);
     if (axis == 0) {
-        constexpr int ROWS = sizeof(T) == 8 ? XROWS64 : XROWS32;
         P.npencil = (long long)h->ny * h->nz;
         P.stride_other = 0;
-        P.seg = auto_segment(h, axis, P.N, P.npencil);
+        P.seg = auto_segment(h, axis, P.N, (P.npencil + 127) / 128);
         P.nseg = (P.N + P.seg - 1) / P.seg;
-        if (h->variant == 0) {
-            // warp-specialised x sweep: 128 rows per CTA, 4 producer + 4 consumer warps
-            XMaps maps;
+        {
+            // producer/consumer warp pairs, 32 rows per pair, 4 pairs per CTA; TMA tiles when possible (fp64, even nx)
             const bool tma = h->have_tmap && sizeof(T) == 8 && !h->no_tma;
-            if (tma) {
-                maps.in[0] = h->tmap[src][0]; maps.out[0] = h->tmap[dst][0];
-                for (int c = 0; c < 3; ++c) {
-                    maps.in[1 + c] = h->tmap[src][1 + perm[axis][c]];
-                    maps.out[1 + c] = h->tmap[dst][1 + perm[axis][c]];
-                }
-                maps.in[4] = h->tmap[src][4]; maps.out[4] = h->tmap[dst][4];
-            } else {
-                memset(&maps, 0, sizeof(maps));
-            }
-            const size_t smem = sizeof(XvSmem<T>);
+            X2Maps maps;
+            memset(&maps, 0, sizeof(maps));
+            maps.fidx[0] = 0; maps.fidx[4] = 4;
+            for (int c = 0; c < 3; ++c) maps.fidx[1 + c] = 1 + perm[axis][c];
+            if (tma) { maps.in = h->d_xmaps + src * NF; maps.out = h->d_xmaps + dst * NF; }
+            const size_t smem = sizeof(X2Smem<T>);
             dim3 grid((unsigned)((P.npencil + 127) / 128), (unsigned)P.nseg);
             if (tma) {
-                auto kern = sweep_x_ws_kernel<T, EOS, EMIT, true>;
-                CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                auto kern = sweep_x2_kernel<T, EOS, EMIT, true>;
+                int rc = opt_in_smem(h, (const void*)kern, smem);
+                if (rc) return rc;
                 kern<<<grid, 256, smem, st>>>(P, k, maps);
             } else {
-                auto kern = sweep_x_ws_kernel<T, EOS, EMIT, false>;
-                CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                auto kern = sweep_x2_kernel<T, EOS, EMIT, false>;
+                int rc = opt_in_smem(h, (const void*)kern, smem);
+                if (rc) return rc;
                 kern<<<grid, 256, smem, st>>>(P, k, maps);
             }
-        } else {
-            auto kern = sweep_x_kernel<T, EOS, EMIT, ROWS>;
-            const size_t smem = sizeof(XSmem<T, ROWS>);
-            CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            dim3 grid((unsigned)((P.npencil + ROWS - 1) / ROWS), (unsigned)P.nseg);
-            kern<<<grid, ROWS, smem, st>>>(P, k);
         }
     } else {
         // y sweep: pencils (x,z), base = x + z*nx*ny;  z sweep: pencils (x,y), base = x + y*nx = flat
         const int other = axis == 1 ? 2 : 1;
-        P.npencil = (long long)h->nx * n[other];
         P.stride_other = stride[other];
-        P.seg = auto_segment(h, axis, P.N, P.npencil);
-        P.nseg = (P.N + P.seg - 1) / P.seg;
-        if (h->variant == 0) {
-            // warp-specialised march: 128 pencils per CTA, 4 producer + 4 consumer warps
-            auto kern = sweep_strided_ws_kernel<T, EOS, EMIT>;
-            const size_t smem = sizeof(WsSmem<T>);
-            CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            dim3 grid((unsigned)((P.npencil + WS_P - 1) / WS_P), (unsigned)P.nseg);
-            kern<<<grid, 2 * WS_P, smem, st>>>(P, k);
-        } else {
-            dim3 grid((unsigned)((P.npencil + STRIDED_BLOCK - 1) / STRIDED_BLOCK), (unsigned)P.nseg);
-            sweep_strided_kernel<T, EOS, EMIT><<<grid, STRIDED_BLOCK, 0, st>>>(P, k);
+        {
+            // producer/consumer warp pairs, 32 pencils (one x-block of a row) per pair, 4 pairs per CTA; TMA-fed when possible
+            const long long nxb = (h->nx + 31) / 32;
+            P.npencil = nxb * n[other];                                         // pencil GROUPS
+            const long long ctas = (P.npencil + 3) / 4;
+            P.seg = auto_segment(h, axis, P.N, ctas);
+            P.nseg = (P.N + P.seg - 1) / P.seg;
+            const bool tma = h->have_yzmap && !h->no_tma && P.N >= YZ_CH;
+            YzMaps maps;
+            memset(&maps, 0, sizeof(maps));
+            maps.fidx[0] = 0; maps.fidx[4] = 4;
+            for (int c = 0; c < 3; ++c) maps.fidx[1 + c] = 1 + perm[axis][c];
+            if (tma) {
+                maps.in4 = h->d_yzmaps + (src * 3 + (axis == 1 ? 0 : 1)) * NF;
+                maps.in1 = h->d_yzmaps + (src * 3 + 2) * NF;
+            }
+            const size_t smem = sizeof(YzSmem<T>);
+            dim3 grid((unsigned)ctas, (unsigned)P.nseg);
+#define SHK_LAUNCH_YZ(TMA_)                                                                        \
+            {                                                                                       \
+                auto kern = sweep_yz_kernel<T, EOS, EMIT, TMA_>;                                    \
+                int rc = opt_in_smem(h, (const void*)kern, smem);                                   \
+                if (rc) return rc;                                                                  \
+                kern<<<grid, 256, smem, st>>>(P, k, maps);                                          \
+            }
+            if (tma) SHK_LAUNCH_YZ(true) else SHK_LAUNCH_YZ(false)
+#undef SHK_LAUNCH_YZ
         }
     }
     CK(cudaGetLastError());
@@ -413,7 +473,7 @@ int refresh_prims_t(shasta_t* h, cudaStream_t st)
 // conserved fields once (88 B/cell, ~0.3 ms).  y/z sweeps emit in place (+0.08 ms).
 int launch_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
 {
-    if (emit && axis == 0 && h->variant == 0) {
+    if (emit && axis == 0) {
         int rc = launch_sweep_raw(h, axis, false, st);
         if (rc) return rc;
         return h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
@@ -480,6 +540,8 @@ void shasta_destroy(shasta_t* h)
         for (int f = 0; f < NF; ++f) cudaFree(h->U[b][f]);
     for (int q = 0; q < 6; ++q) cudaFree(h->prim[q]);
     cudaFree(h->stage);
+    cudaFree(h->d_yzmaps);
+    cudaFree(h->d_xmaps);
     cudaFree(h->d_counts);
     cudaFree(h->d_partial);
     if (h->h_partial) cudaFreeHost(h->h_partial);
@@ -518,8 +580,7 @@ int shasta_set_option(shasta_t* h, int key, double value)
         h->no_tma = value != 0.0;
         return 0;
     case SHASTA_VARIANT:
-        if (value != 0.0 && value != 1.0) return fail(h, SHASTA_EINVAL, "SHASTA_VARIANT must be 0 or 1");
-        h->variant = (int)value;
+        if (value != 0.0) return fail(h, SHASTA_EINVAL, "SHASTA_VARIANT: only 0 exists (the single-role kernels of round 1 were removed)");
         return 0;
     default:
         return fail(h, SHASTA_EINVAL, "shasta_set_option: unknown key %d", key);
@@ -746,8 +807,7 @@ long long shasta_step_index(const shasta_t* h) { return h ? h->step : -1; }
 const char* shasta_kernel_name(const shasta_t* h, int axis)
 {
     if (!h || axis < 0 || axis > 2) return "";
-    if (h->variant == 0) return axis == 0 ? "sweep_x_ws_kernel" : "sweep_strided_ws_kernel";
-    return axis == 0 ? "sweep_x_kernel" : "sweep_strided_kernel";
+    return axis == 0 ? "sweep_x2_kernel" : "sweep_yz_kernel";
 }
 
 const char* shasta_last_error(const shasta_t* h) { return h ? h->err : g_create_err; }

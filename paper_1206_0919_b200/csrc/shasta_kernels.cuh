@@ -70,26 +70,28 @@ struct SweepParams {
     int seg;                // cells marched per work item
     int nseg;               // segments per pencil
     int periodic;           // boundary rule (reading G11)
+    int axis;               // 0 x, 1 y, 2 z
     unsigned long long* counts;   // diagnostics [4]
 };
 
-// Diagnostics are counted per thread in shared memory (or registers) and flushed once per warp at the end of
-// the kernel: one global atomic per event on a single address serialises in L2 and cost 60 % of the step
-// time once the causality projection fires in ~0.2 % of the cells (profiles/, round 1).
+// Diagnostics are counted per thread in REGISTERS and flushed once per warp at the end of the kernel: one global atomic
+// per event on a single address serialises in L2 and cost 60 % of the step time once the causality projection fired
+// in ~0.2 % of the cells (round 1).
 struct Cnt {
-    unsigned* p;    // this thread's four counters: p[w * stride]
-    int stride;
-    __device__ __forceinline__ void add(int w) const { p[w * stride] += 1u; }
-    __device__ __forceinline__ void zero() const { p[0] = p[stride] = p[2 * stride] = p[3 * stride] = 0u; }
+    unsigned pv;        // Pi fired (low 16 bits) | vacuum cells (high 16 bits): a thread marches < 65536 cells per launch
+    unsigned fl;        // e < 0 floored (low 16) | p < 0 floored (high 16)   (primitive output only)
+    __device__ __forceinline__ void zero() { pv = fl = 0u; }
+    __device__ __forceinline__ void add(int w) { if (w == 0) pv += 1u; else if (w == 1) pv += 0x10000u; else if (w == 2) fl += 1u; else fl += 0x10000u; }
 };
 __device__ __forceinline__ void flush_counts(const Cnt& c, unsigned long long* g)
 {
     const unsigned mask = __activemask();
     const int leader = __ffs(mask) - 1;
+    const unsigned v[4] = {c.pv & 0xffffu, c.pv >> 16, c.fl & 0xffffu, c.fl >> 16};
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
-        const unsigned v = __reduce_add_sync(mask, c.p[w * c.stride]);
-        if ((int)(threadIdx.x & 31) == leader && v) atomicAdd(g + w, (unsigned long long)v);
+        const unsigned t = __reduce_add_sync(mask, v[w]);
+        if ((int)(threadIdx.x & 31) == leader && t) atomicAdd(g + w, (unsigned long long)t);
     }
 }
 
@@ -158,6 +160,16 @@ __device__ __forceinline__ double fast_rsqrt(double x)
     r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
     r = fma(0.5 * r, fma(-(x * r), r, 1.0), r);
     return r;
+}
+
+// 1/sqrt(x), normal x > 0: seed r (2^-20), ONE cubic step r (1 + e/2 + 3 e^2/8), e = 1 - x r^2: truncation 5/16 e^3 = 2^-58.
+// 5 fp64 ops (fast_rsqrt: 8); used where the result is needed unconditionally (branch-free causality clamp).
+__device__ __forceinline__ double fast_rsqrt3(double x)
+{
+    const double r = rsq64h(x);
+    const double e = fma(-(x * r), r, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(r, p * e, r);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -297,9 +309,13 @@ __device__ __forceinline__ void c2p_sweep_d(const EosD& k, const double (&u)[NF]
 template <>
 __device__ __forceinline__ void c2p_sweep_d<EOS_GAMMA>(const EosD& k, const double (&u)[NF], double& v, double& p)
 {
-    // No vacuum BRANCH here: the arithmetic runs on whatever E is (inf / NaN intermediates cost nothing on the fp64
-    // pipe) and the two results are masked by selects, so that the scheduler can interleave the cons2prim chains of
-    // the two cells of a chunk (a branch ends the basic block: measured -5 % per sweep for the two branches here).
+    // No BRANCH here, neither for vacuum nor for the causality clamp: the arithmetic runs on whatever E, M are (inf / NaN
+    // intermediates cost nothing on the fp64 pipe) and the results are masked by selects.  A branch ends the basic
+    // block, and the producer's cons2prim chains are serial (~20 dependent fp64 operations): only when the whole
+    // 4-cell group is ONE basic block can ptxas interleave the chains of its cells (ncu, round 2: with the clamp as a
+    // branch the producer issued one instruction every 6.2 cycles, all of it fixed-latency `wait`).  The price is the
+    // direction-preserving scale factor Mc/|M| computed for every cell (8 fp64 operations) instead of for the ~0.2 %
+    // that are clamped.
     const double M2 = fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3]));
     const bool vac = c2p_is_vacuum(u[0]);       // reading G7: all primitives 0
     const double t = u[0] * u[0];
@@ -308,7 +324,8 @@ __device__ __forceinline__ void c2p_sweep_d<EOS_GAMMA>(const EosD& k, const doub
     const double Mq = clamped ? lim2 : M2;
     double y = c2p_fast_y(k, u[0], Mq, t);
     double e = fma(-Mq, y, u[0]);               // e = E - Mc v >= delta E > 0: no floor
-    if (clamped) y *= (k.omd * u[0]) * fast_rsqrt(M2);      // rare (Pi-clamped cells): direction-preserving scale
+    const double ys = y * ((k.omd * u[0]) * fast_rsqrt3(M2));   // clamped cells: v_i = (Mc y) M_i / |M|
+    y = clamped ? ys : y;
     y = vac ? 0.0 : y;
     e = vac ? 0.0 : e;
     v = u[1] * y;
@@ -333,124 +350,20 @@ __device__ __forceinline__ T limiter(T aph, T dhp, T dhm)
     const T m = t_min(t_min(sg * dhp, t_abs(aph)), sg * dhm);
     return sg * t_max(m, T(0));
 }
-// fp64 on the INTEGER pipe: multiplying by sigma = flipping the sign bit; IEEE doubles order like
-// sign-magnitude integers, so min over non-negative doubles = min over their bit patterns as signed
-// 64-bit integers, and any negative operand makes that integer minimum negative, which max(.,0)
-// clips to +0 -- exactly the max{0, min{...}} of eq. (21).  No fp64-pipe instruction.
+// fp64: the three arguments must agree in sign, else A = 0; if they do, A is the one of smallest magnitude, sign
+// included.  Two DSETP with |.| operand modifiers + selects, the sign test is one LOP3 on the high words: 10
+// instructions per field (the sign-magnitude integer min of round 1 cost 16, all on the 2-cycle ALU pipe).
 template <>
 __device__ __forceinline__ double limiter<double>(double aph, double dhp, double dhm)
 {
-    const long long ia = __double_as_longlong(aph);
-    const long long sg = ia & (long long)0x8000000000000000ULL;
-    const long long z = ia ^ sg;
-    const long long x = __double_as_longlong(dhp) ^ sg;
-    const long long y = __double_as_longlong(dhm) ^ sg;
-    long long m = min(min(x, z), y);
-    if ((int)(m >> 32) < 0) m = 0;
-    return __longlong_as_double(m ^ sg);
+    const int dis = (__double2hiint(aph) ^ __double2hiint(dhp)) | (__double2hiint(aph) ^ __double2hiint(dhm));
+    double m = fabs(dhp) < fabs(aph) ? dhp : aph;
+    m = fabs(dhm) < fabs(m) ? dhm : m;
+    return dis < 0 ? 0.0 : m;
 }
 
-// ------------------------------------------------------------------------------------------------
-// The rolling window of one marching thread.  "X_k" below means the quantity at cell (or interface)
-// i-k, where i is the front cell of the CURRENT step.  Each window is a small ring whose slot is a
-// compile-time function of the phase PH = (step number) mod 4: the march loop is unrolled by 4, so
-// every slot is a fixed register and the window advances without a single move instruction.
-template <typename T, int EOS>
-struct Marcher {
-    T u[2][NF];         // U^n_1, U^n_2                    slot of U^n_k : (PH-k)&1
-    T dl[4][NF];        // Delta_2..Delta_5, eq. (16)      slot of Delta_k: (PH-k)&3
-    T ft[NF];           // predictor flux F~ at interface (i-2,i-1)
-    T fc[NF];           // corrector flux F at interface (i-3,i-2)
-    T uh[2][NF];        // U^_3, U^_4                      slot of U^_k : (PH-k)&1
-    T dh[2][NF];        // D^_4, D^_5, eq. (18)            slot of D^_k : (PH-k)&1
-    T a5[NF];           // limited antidiffusive flux A_5
-    T eps1;             // (lambda/2) v_1 (time n)
-    T fE[2], fM[2];     // (p v)_1,_2 and p_1,_2 (time n)  slot (PH-k)&1
-    T epsh2;            // lambda v^{1/2}_2
-    T gE[2], gM[2];     // (p v)^{1/2}_2,_3 and p^{1/2}_2,_3   slot (PH-k)&1
-
-    __device__ __forceinline__ void init()
-    {
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            u[0][f] = u[1][f] = dl[0][f] = dl[1][f] = dl[2][f] = dl[3][f] = ft[f] = fc[f] = T(0);
-            uh[0][f] = uh[1][f] = dh[0][f] = dh[1][f] = a5[f] = T(0);
-        }
-        eps1 = epsh2 = fE[0] = fE[1] = fM[0] = fM[1] = gE[0] = gE[1] = gM[0] = gM[1] = T(0);
-    }
-
-    // One march step: consumes U^n at the front cell, produces U^{n+1} of cell i-4 in un[].
-    template <int PH>
-    __device__ __forceinline__ void step(const Consts<T>& k, const T (&u0)[NF], T (&un)[NF])
-    {
-        constexpr int U1 = (PH + 3) & 1, U2 = (PH + 2) & 1;                 // U^n_1, U^n_2 (new U^n_0 -> U2)
-        constexpr int D2 = (PH + 2) & 3, D3 = (PH + 1) & 3, D4 = PH & 3, D5 = (PH + 3) & 3;   // new Delta_1 -> D5
-        constexpr int H3 = (PH + 1) & 1, H4 = PH & 1;                       // U^_3, U^_4 (new U^_2 -> H4)
-        constexpr int E4 = PH & 1, E5 = (PH + 1) & 1;                       // D^_4, D^_5 (new D^_3 -> E5)
-        constexpr int S1 = (PH + 1) & 1, S2 = PH & 1;                       // time-n scalars _1,_2 (new _0 -> S2)
-        constexpr int G2 = PH & 1, G3 = (PH + 1) & 1;                       // half-step scalars _2,_3 (new _1 -> G3)
-        (void)S1; (void)G2;
-        // S1: time-n primitives of the front cell
-        T v0, p0;
-        c2p_sweep<T, EOS>(k, u0, v0, p0);
-        const T eps0 = k.hlam * v0;
-        const T fE0 = p0 * v0;
-        // S2: predictor (half step, no antidiffusion: reading G4), interface (i-1,i), cell i-1
-        T ut[NF], dl1[NF];
-        {
-            const T q = (T(0.5) - eps1) * fast_rcp(T(1) + (eps0 - eps1));   // Q+_1, eq. (15); Q-_0 = 1-q (P1)
-            const T a = T(0.5) - q, b = (T(0.5) * q) * q;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-                dl1[f] = u0[f] - u[U1][f];                                  // eq. (16)
-                const T fl = t_fma(a, u[U1][f], -(b * dl1[f]));             // F = (1/2-q) U - 1/2 q^2 Delta (P2)
-                ut[f] = u[U1][f] - (fl - ft[f]);                               // exact no-op on uniform data (P10)
-                ft[f] = fl;
-            }
-            ut[0] = t_fma(-k.qlam, fE0 - fE[S2], ut[0]);                    // + (lambda/2) Delta(p v)
-            ut[1] = t_fma(-k.qlam, p0 - fM[S2], ut[1]);                     // + (lambda/2) Delta(p)
-        }
-        // S3: half-step primitives of cell i-1
-        T vh1, ph;
-        c2p_sweep<T, EOS>(k, ut, vh1, ph);
-        const T epsh1 = k.lam * vh1;
-        const T gE1 = ph * vh1;
-        // S4: corrector transport of U^n, interface (i-2,i-1), cell i-2
-        T uh2[NF];
-        {
-            const T q = (T(0.5) - epsh2) * fast_rcp(T(1) + (epsh1 - epsh2));
-            const T a = T(0.5) - q, b = (T(0.5) * q) * q;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-                const T fl = t_fma(a, u[U2][f], -(b * dl[D2][f]));
-                uh2[f] = u[U2][f] - (fl - fc[f]);
-                fc[f] = fl;
-            }
-            uh2[0] = t_fma(-k.hlam, gE1 - gE[G3], uh2[0]);                  // + lambda Delta(p v)^{n+1/2}
-            uh2[1] = t_fma(-k.hlam, ph - gM[G3], uh2[1]);                   // + lambda Delta(p)^{n+1/2}
-        }
-        // S5+S6: antidiffusion at interface (i-4,i-3), update of cell i-4
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            const T dh3 = uh2[f] - uh[H3][f];                                    // eq. (18)
-            const T d2 = t_fma(T(-2), dl[D4][f], dl[D3][f] + dl[D5][f]);         // reading G14
-            const T aph = T(0.125) * t_fma(T(-0.125), d2, dh[E4][f]);            // eq. (19)
-            const T a4 = limiter<T>(aph, dh3, dh[E5][f]);                        // eqs. (20),(21)
-            un[f] = uh[H4][f] - (a4 - a5[f]);                                    // eq. (22)
-            // advance the window: the new values take the slots of the oldest ones
-            a5[f] = a4;
-            dh[E5][f] = dh3;
-            uh[H4][f] = uh2[f];
-            dl[D5][f] = dl1[f];
-            u[U2][f] = u0[f];
-        }
-        eps1 = eps0; fE[S2] = fE0; fM[S2] = p0;
-        epsh2 = epsh1; gE[G3] = gE1; gM[G3] = ph;
-    }
-};
-
 // Pi, readings G6-G8: written back to M at the end of every sweep.  E and R are never modified.
-__device__ __forceinline__ void project(const EosD& k, double (&un)[NF], Cnt counts)
+__device__ __forceinline__ void project(const EosD& k, double (&un)[NF], Cnt& counts)
 {
     const double E = un[0];
     const double M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
@@ -467,7 +380,7 @@ __device__ __forceinline__ void project(const EosD& k, double (&un)[NF], Cnt cou
 
 // primitives of one cell from its (projected) conserved state, slots permuted like the momenta
 template <int EOS>
-__device__ __forceinline__ void primitives(const EosD& k, const double (&u)[NF], double (&pr)[6], Cnt counts)
+__device__ __forceinline__ void primitives(const EosD& k, const double (&u)[NF], double (&pr)[6], Cnt& counts)
 {
     const Prim o = cons2prim_general<EOS>(k, u[0], u[1], u[2], u[3], u[4]);
     pr[0] = o.e; pr[1] = o.p;
@@ -495,7 +408,7 @@ __device__ __forceinline__ void prims_fast(const EosD& k, const double (&u)[NF],
 
 // S6 tail + S7 of one output cell: Pi on un[], and (EMIT) its primitives pr[].
 template <int EOS, bool EMIT>
-__device__ __forceinline__ void finish_d(const EosD& k, double (&un)[NF], double (&pr)[6], Cnt counts)
+__device__ __forceinline__ void finish_d(const EosD& k, double (&un)[NF], double (&pr)[6], Cnt& counts)
 {
     if (EOS == EOS_GAMMA) {
         // Gamma-law: Pi and the primitives share |M|^2 and E^2; everything but vacuum is inline
@@ -528,7 +441,7 @@ __device__ __forceinline__ void finish_d(const EosD& k, double (&un)[NF], double
     }
 }
 template <typename T, int EOS, bool EMIT>
-__device__ __forceinline__ void finish_cell(const Consts<T>& k, T (&un)[NF], T (&pr)[6], Cnt counts)
+__device__ __forceinline__ void finish_cell(const Consts<T>& k, T (&un)[NF], T (&pr)[6], Cnt& counts)
 {
     double ud[NF], pd[6];
 #pragma unroll
@@ -544,7 +457,7 @@ __device__ __forceinline__ void finish_cell(const Consts<T>& k, T (&un)[NF], T (
 
 // primitives of an already projected cell (x sweep write-back, shasta_get_primitives refresh)
 template <int EOS>
-__device__ __forceinline__ void emit_d(const EosD& k, const double (&u)[NF], double (&pr)[6], Cnt counts)
+__device__ __forceinline__ void emit_d(const EosD& k, const double (&u)[NF], double (&pr)[6], Cnt& counts)
 {
     if (EOS != EOS_GAMMA) {
         primitives<EOS>(k, u, pr, counts);
@@ -563,7 +476,7 @@ __device__ __forceinline__ void emit_d(const EosD& k, const double (&u)[NF], dou
     prims_fast(k, u, clamped ? lim2 : M2, t, s, pr);
 }
 template <typename T, int EOS>
-__device__ __forceinline__ void emit_primitives(const Consts<T>& k, const T (&u)[NF], T (&pr)[6], Cnt counts)
+__device__ __forceinline__ void emit_primitives(const Consts<T>& k, const T (&u)[NF], T (&pr)[6], Cnt& counts)
 {
     double ud[NF], pd[6];
 #pragma unroll
@@ -585,107 +498,6 @@ __device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc)
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
-
-// ------------------------------------------------------------------------------------------------
-// Sweep along y or z: lanes run along the contiguous x axis, so every load and store of a warp is a
-// coalesced 256 B (fp64) row piece.  Work item = (pencil, segment).  The marching thread is latency-
-// bound unless many cells are in flight per pencil, and registers are full (the window), so the input
-// is PREFETCHED SD-1 cells ahead with cp.async into a per-thread ring in shared memory
-// (ring[slot][field][thread]: conflict-free).  A thread only ever reads what it copied itself:
-// cp.async.wait_group is the only synchronisation.
-constexpr int SD = 8;             // ring slots = cells in flight per pencil + 1
-constexpr int SBLOCK = 128;       // threads per CTA
-
-template <typename T>
-struct StridedCtx {
-    const T* in[NF];
-    T* out[NF];
-    T* prim[6];
-    long long sa;       // element stride along the sweep axis
-    int N, periodic, j0, j1;
-    int ipf, jpf;       // next cell to prefetch: true index and ghost-mapped index (reading G11)
-    Cnt counts;
-};
-
-// issue the copy of the next cell into ring slot `slot`; one commit group per cell
-template <typename T>
-__device__ __forceinline__ void strided_prefetch(StridedCtx<T>& c, T* slot)
-{
-    const long long o = (long long)c.jpf * c.sa;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) cp_async_elem<T>(slot + f * SBLOCK, c.in[f] + o);
-    cp_async_commit();
-    c.ipf += 1;
-    if (c.periodic) { c.jpf = (c.jpf + 1 == c.N) ? 0 : c.jpf + 1; }     // wrap
-    else            { c.jpf = min(max(c.ipf, 0), c.N - 1); }            // copy of the edge cell
-}
-
-// PH = step number mod 4 (compile time: window phase and ring slot inside the current half of the ring);
-// cur / oth = the two halves (4 slots each) of this thread's ring, swapped every 4 steps by the caller.
-template <typename T, int EOS, bool EMIT, int PH>
-__device__ __forceinline__ void strided_substep(Marcher<T, EOS>& m, const Consts<T>& k, StridedCtx<T>& c, int i,
-                                                T* cur, T* oth)
-{
-    // refill the slot consumed by the PREVIOUS step (its reads are long retired), then wait for cell i
-    strided_prefetch<T>(c, PH == 0 ? oth + 3 * NF * SBLOCK : cur + (PH - 1) * NF * SBLOCK);
-    cp_async_wait<SD - 1>();
-    T u0[NF], un[NF];
-#pragma unroll
-    for (int f = 0; f < NF; ++f) u0[f] = cur[(PH * NF + f) * SBLOCK];
-    m.template step<PH>(k, u0, un);
-    const int jo = i - GH;
-    if (jo >= c.j0 && jo < c.j1) {
-        T pr[6];
-        finish_cell<T, EOS, EMIT>(k, un, pr, c.counts);
-        const long long o = (long long)jo * c.sa;
-#pragma unroll
-        for (int f = 0; f < NF; ++f) c.out[f][o] = un[f];
-        if (EMIT) {
-#pragma unroll
-            for (int q = 0; q < 6; ++q) c.prim[q][o] = pr[q];
-        }
-    }
-}
-
-template <typename T, int EOS, bool EMIT>
-__global__ void __launch_bounds__(SBLOCK) sweep_strided_kernel(SweepParams P, Consts<T> k)
-{
-    __shared__ T ring[SD * NF * SBLOCK];
-    __shared__ unsigned cnt[4 * SBLOCK];
-    const long long pen = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (pen >= P.npencil) return;
-    const int sg = blockIdx.y;
-    StridedCtx<T> c;
-    c.j0 = sg * P.seg;
-    c.j1 = min(P.N, c.j0 + P.seg);
-    c.N = P.N; c.periodic = P.periodic; c.sa = P.stride_axis;
-    c.counts.p = cnt + threadIdx.x; c.counts.stride = SBLOCK;
-    c.counts.zero();
-    const long long base = (pen % P.nx) + (pen / P.nx) * P.stride_other;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) { c.in[f] = (const T*)P.in[f] + base; c.out[f] = (T*)P.out[f] + base; }
-#pragma unroll
-    for (int q = 0; q < 6; ++q) c.prim[q] = (T*)P.prim[q] + base;
-
-    Marcher<T, EOS> m;
-    m.init();
-    c.ipf = c.j0 - GH;
-    c.jpf = ghost_index(c.ipf, P.N, P.periodic);
-    T* cur = ring + threadIdx.x;
-    T* oth = cur + 4 * NF * SBLOCK;
-#pragma unroll
-    for (int d = 0; d < SD - 1; ++d) strided_prefetch<T>(c, cur + d * NF * SBLOCK);      // cells j0-4 .. j0+2
-    // front cells j0-4 .. j1+3, rounded up to a multiple of 4 steps (the surplus steps store nothing)
-    for (int i = c.j0 - GH; i < c.j1 + GH; i += 4) {
-        strided_substep<T, EOS, EMIT, 0>(m, k, c, i, cur, oth);
-        strided_substep<T, EOS, EMIT, 1>(m, k, c, i + 1, cur, oth);
-        strided_substep<T, EOS, EMIT, 2>(m, k, c, i + 2, cur, oth);
-        strided_substep<T, EOS, EMIT, 3>(m, k, c, i + 3, cur, oth);
-        T* tmp = cur; cur = oth; oth = tmp;
-    }
-    cp_async_wait<0>();
-    flush_counts(c.counts, P.counts);
-}
 
 // ------------------------------------------------------------------------------------------------
 // Warp-specialised march: the serial chain S1..S6 of one march step is cut after S3 and
@@ -800,309 +612,28 @@ struct Consumer {
     }
 };
 
-constexpr int WS_P = 128;         // pencils per CTA (4 producer warps + 4 consumer warps)
-constexpr int WS_R = 12;          // U ring slots per pencil
-constexpr int WS_D = WS_R - 5;    // prefetch distance; D-1 copies stay in flight behind the current chunk (see below)
-constexpr int WS_Q = 4;           // message queue slots (2 chunks of 2 steps)
+// two adjacent elements with one shared-memory access (LDS.128 for fp64); p is 2-element aligned
+__device__ __forceinline__ void load2(const double* p, double& a, double& b)
+{
+    const double2 v = *reinterpret_cast<const double2*>(p);
+    a = v.x; b = v.y;
+}
+__device__ __forceinline__ void load2(const float* p, float& a, float& b)
+{
+    const float2 v = *reinterpret_cast<const float2*>(p);
+    a = v.x; b = v.y;
+}
 
-template <typename T>
-struct WsSmem {
-    T ring[WS_R][NF][WS_P];
-    T msg[WS_Q][4][WS_P];
-    unsigned cnt[4][WS_P];
-};
+__device__ __forceinline__ void store2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
+__device__ __forceinline__ void store2(float* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
 
-// Producer/consumer hand-over of one warp pair: four named barriers (full[0..1], empty[0..1]) of 64 threads each,
-// 32 that arrive (do not wait) and 32 that sync (wait): the PTX producer/consumer pattern.  The producer may run up
-// to two 2-step chunks ahead of the consumer; chunk c uses slot c & 1.
+// Producer/consumer hand-over of one warp pair: named barriers of 64 threads each, 32 that arrive (do not wait) and 32
+// that sync (wait): the PTX producer/consumer pattern.
 __device__ __forceinline__ void bar_sync64(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 __device__ __forceinline__ void bar_arrive64(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
 
-template <typename T, int EOS, bool EMIT>
-__global__ void __launch_bounds__(2 * WS_P, 2) sweep_strided_ws_kernel(const __grid_constant__ SweepParams P,
-                                                                      const __grid_constant__ Consts<T> k)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    WsSmem<T>& S = *reinterpret_cast<WsSmem<T>*>(smem_raw);
-    const int lane_p = threadIdx.x & (WS_P - 1);                // pencil slot inside the CTA
-    const bool producer = threadIdx.x < WS_P;                   // warps 0-3: P, warps 4-7: C
-    const int bar_id = 4 * ((threadIdx.x >> 5) & 3);            // named barriers of this warp pair: full0, full1, empty0, empty1
-    long long pen = (long long)blockIdx.x * WS_P + lane_p;
-    const bool active = pen < P.npencil;
-    if (!active) pen = P.npencil - 1;                           // idle lanes shadow a valid pencil, store nothing
-    const int sg = blockIdx.y;
-    const int j0 = sg * P.seg;
-    const int j1 = min(P.N, j0 + P.seg);
-    const long long sa = P.stride_axis;
-    const long long base = (pen % P.nx) + (pen / P.nx) * P.stride_other;
-    const int nsteps = (j1 - j0) + 2 * GH;                      // front cells j0-4 .. j1+3
-    const int nchunk = (nsteps + 1) / 2;
-    const int nchunk2 = (nchunk + 1) & ~1;
-
-    if (producer) {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
-        Producer<T, EOS> pr;
-        pr.init();
-        // prefetch state: next cell to fetch (true index ipf, ghost-mapped jpf) and its ring slot
-        int ipf = j0 - GH, jpf = ghost_index(ipf, P.N, P.periodic), pslot = 0;
-        auto prefetch = [&]() {
-            const long long o = base + (long long)jpf * sa;        // field pointers stay in the constant bank
-#pragma unroll
-            for (int f = 0; f < NF; ++f) cp_async_elem<T>(&S.ring[pslot][f][lane_p], (const T*)P.in[f] + o);
-            cp_async_commit();
-            pslot = (pslot + 1 == WS_R) ? 0 : pslot + 1;
-            ipf += 1;
-            if (P.periodic) { jpf = (jpf + 1 == P.N) ? 0 : jpf + 1; }
-            else            { jpf = min(max(ipf, 0), P.N - 1); }
-        };
-#pragma unroll
-        for (int d = 0; d < WS_D - 1; ++d) prefetch();
-        int rslot = 0;
-        // Copies: before chunk `it` cells 0 .. 2it+D-2 are issued; its two prefetches add cells 2it+D-1, 2it+D, and
-        // wait_group<D-1> then leaves at most the D-1 youngest pending, i.e. cells <= 2it+1 (this chunk) are complete.
-        // Slot reuse (D = R-5): those two refill the slots of cells 2it-6 and 2it-5.  The producer enters chunk `it`
-        // only after the consumer released chunk it-2; the consumer may still be inside chunk it-1, where it reads
-        // cells 2it-4 .. 2it-2 (U_{i-2}, U_{i-1} of its two steps): all younger than the refilled ones.
-        // One chunk = two steps: both front cells are fetched first, then the two steps' arithmetic runs with no
-        // asm/memory fence in between, so the scheduler may overlap S3 of the first with S1 of the second.
-#define SHK_PCHUNK(PH)                                                                              \
-        {                                                                                           \
-            prefetch();                                                                             \
-            prefetch();                                                                             \
-            cp_async_wait<WS_D - 1>();                                                              \
-            T um[NF], ua[NF], ub[NF], ma[4], mb[4];                                                 \
-            um[NF - 1] = ua[NF - 1] = ub[NF - 1] = T(0);                                            \
-            const int mslot = (rslot == 0) ? WS_R - 1 : rslot - 1;      /* cell 2it-1 (first chunk: don't care) */ \
-            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) um[f] = S.ring[mslot][f][lane_p]; \
-            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) ua[f] = S.ring[rslot][f][lane_p]; \
-            rslot = (rslot + 1 == WS_R) ? 0 : rslot + 1;                                            \
-            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) ub[f] = S.ring[rslot][f][lane_p]; \
-            rslot = (rslot + 1 == WS_R) ? 0 : rslot + 1;                                            \
-            pr.template step<PH>(k, um, ua, ma);                                                    \
-            pr.template step<PH + 1>(k, ua, ub, mb);                                                \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane_p] = ma[q];             \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane_p] = mb[q];         \
-        }
-        // decoupled hand-over (see bar_sync64): chunk c uses slot c & 1; nchunk is rounded up to even (a surplus
-        // chunk marches ghost cells and stores nothing)
-#pragma unroll 1
-        for (int c = 0; c < nchunk2; c += 2) {
-            if (c > 0) bar_sync64(bar_id + 2);
-            SHK_PCHUNK(0)
-            bar_arrive64(bar_id + 0);
-            if (c > 0) bar_sync64(bar_id + 3);
-            SHK_PCHUNK(2)
-            bar_arrive64(bar_id + 1);
-        }
-#undef SHK_PCHUNK
-        cp_async_wait<0>();
-    } else {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
-        Cnt cnt;
-        cnt.p = &S.cnt[0][lane_p]; cnt.stride = WS_P;
-        cnt.zero();
-        Consumer<T> co;
-        co.init();
-        // consumer step t (front cell i = j0-4+t) reads U_{i-1}: ring slot of cell index t-1 (t = 0: the
-        // ring's last slot, never written before: a don't-care warm-up value, finite or not it is retired)
-        int cslot = WS_R - 1;
-        int i = j0 - GH;
-#define SHK_CSTORE(UN)                                                                              \
-        {                                                                                           \
-            const int jo = i - GH;                                                                  \
-            if (jo >= j0 && jo < j1 && active) {                                                    \
-                T pv[6];                                                                            \
-                finish_cell<T, EOS, EMIT>(k, UN, pv, cnt);                                          \
-                const long long o = base + (long long)jo * sa;                                      \
-                _Pragma("unroll") for (int f = 0; f < NF; ++f) ((T*)P.out[f])[o] = UN[f];           \
-                if (EMIT) { _Pragma("unroll") for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[o] = pv[q]; } \
-            }                                                                                       \
-            ++i;                                                                                    \
-        }
-        // one chunk = steps t, t+1: cells t-2, t-1, t are read from the ring (no carried U, no hand-down moves)
-#define SHK_CCHUNK(PH)                                                                              \
-        {                                                                                           \
-            T uq[NF], ua[NF], ub[NF], msg[4], un[NF];                                               \
-            const int qslot = (cslot == 0) ? WS_R - 1 : cslot - 1;                                  \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) uq[f] = S.ring[qslot][f][lane_p];        \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) ua[f] = S.ring[cslot][f][lane_p];        \
-            cslot = (cslot + 1 == WS_R) ? 0 : cslot + 1;                                            \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) ub[f] = S.ring[cslot][f][lane_p];        \
-            cslot = (cslot + 1 == WS_R) ? 0 : cslot + 1;                                            \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane_p];            \
-            co.template step<PH>(uq, ua, msg, un);                                                  \
-            SHK_CSTORE(un)                                                                          \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH + 1][q][lane_p];        \
-            co.template step<PH + 1>(ua, ub, msg, un);                                              \
-            SHK_CSTORE(un)                                                                          \
-        }
-#pragma unroll 1
-        for (int c = 0; c < nchunk2; c += 2) {
-            bar_sync64(bar_id + 0);
-            SHK_CCHUNK(0)
-            if (c + 2 < nchunk2) bar_arrive64(bar_id + 2);
-            bar_sync64(bar_id + 1);
-            SHK_CCHUNK(2)
-            if (c + 2 < nchunk2) bar_arrive64(bar_id + 3);
-        }
-#undef SHK_CCHUNK
-#undef SHK_CSTORE
-        flush_counts(cnt, P.counts);
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// Sweep along x (the contiguous axis): a WARP owns 32 rows; lane r marches along row r.  The rows
-// are staged through shared memory in chunks of XCH cells per row (cp.async, double buffered) so that
-// global traffic stays coalesced (64 B row pieces) while each thread reads its own row conflict-free
-// (row pitch XCH+1: odd).  The result of cell i-4 is written IN PLACE over the slot of the front cell i
-// just consumed, so a chunk buffer holds the inputs [8c, 8c+8) before and the outputs [8c-4, 8c+4)
-// after its march; the write-back is coalesced (the primitives of the last sweep are computed element-wise there).
-constexpr int XCH = 8;            // cells per row per chunk
-constexpr int XPITCH = XCH + 1;   // odd pitch: conflict-free column access for 8 B elements
-constexpr int XNS = 2;            // stages
-
-constexpr int XW = 32;            // rows per warp: every warp runs its own pipeline, no CTA barrier
-
-template <typename T, int ROWS>
-struct XSmem {
-    T buf[ROWS / XW][XNS][NF][XW * XPITCH];
-    unsigned cnt[4][ROWS];
-};
-
-template <typename T, int EOS, int PH>
-__device__ __forceinline__ void x_substep(Marcher<T, EOS>& m, const Consts<T>& k, T* sb, int i, int ilo, int ihi,
-                                          int j0, Cnt counts)
-{
-    // sb = &buf[warp][stage][0][lane * XPITCH + 4 h]: column 4 h + PH of the chunk; window phase = PH
-    if (i < ilo || i >= ihi) return;
-    T u0[NF], un[NF];
-#pragma unroll
-    for (int f = 0; f < NF; ++f) u0[f] = sb[f * (XW * XPITCH) + PH];
-    m.template step<PH>(k, u0, un);
-    if (i - GH >= j0) {
-        T pr[6];
-        finish_cell<T, EOS, false>(k, un, pr, counts);
-#pragma unroll
-        for (int f = 0; f < NF; ++f) sb[f * (XW * XPITCH) + PH] = un[f];
-    }
-}
-
-template <typename T, int EOS, bool EMIT, int ROWS>
-__global__ void __launch_bounds__(ROWS) sweep_x_kernel(SweepParams P, Consts<T> k)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    XSmem<T, ROWS>& S = *reinterpret_cast<XSmem<T, ROWS>*>(smem_raw);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const long long row0 = (long long)blockIdx.x * ROWS + warp * XW;
-    if (row0 >= P.npencil) return;                        // whole warp idle (no CTA barrier below)
-    const int nrows = (int)min((long long)XW, P.npencil - row0);
-    const int sg = blockIdx.y;
-    const int j0 = sg * P.seg;
-    const int j1 = min(P.N, j0 + P.seg);
-    const int ilo = j0 - GH, ihi = j1 + GH;               // front cells [ilo, ihi)
-    const int c_first = (ilo >= 0) ? ilo / XCH : -((-ilo + XCH - 1) / XCH);
-    const int c_last = (ihi - 1) / XCH;
-    const int N = P.N;
-
-    // warp-cooperative chunk loader: element (row, col) of chunk c <- in[f][(row0+row)*nx + ghost(XCH*c+col)]
-    // (lane -> 8 consecutive lanes cover one 64 B row piece)
-    auto load_chunk = [&](int c, int stage) {
-        if (c <= c_last) {
-#pragma unroll
-            for (int e = lane; e < XW * XCH; e += 32) {
-                const int row = e / XCH, col = e % XCH;
-                const int i = c * XCH + col;
-                if (row < nrows && i >= ilo && i < ihi) {
-                    const long long g = (row0 + row) * (long long)N + ghost_index(i, N, P.periodic);
-#pragma unroll
-                    for (int f = 0; f < NF; ++f)
-                        cp_async_elem<T>(&S.buf[warp][stage][f][row * XPITCH + col], (const T*)P.in[f] + g);
-                }
-            }
-        }
-        cp_async_commit();
-    };
-
-    Cnt cnt;
-    cnt.p = &S.cnt[0][threadIdx.x]; cnt.stride = ROWS;
-    cnt.zero();
-    Marcher<T, EOS> m;
-    m.init();
-    load_chunk(c_first, 0);
-    load_chunk(c_first + 1, 1);
-    for (int c = c_first; c <= c_last; ++c) {
-        const int stage = (c - c_first) % XNS;
-        cp_async_wait<XNS - 1>();
-        __syncwarp();
-        if (lane < nrows) {
-#pragma unroll 1
-            for (int h = 0; h < XCH / 4; ++h) {
-                T* sb = &S.buf[warp][stage][0][lane * XPITCH + 4 * h];
-                const int i = c * XCH + 4 * h;
-                x_substep<T, EOS, 0>(m, k, sb, i + 0, ilo, ihi, j0, cnt);
-                x_substep<T, EOS, 1>(m, k, sb, i + 1, ilo, ihi, j0, cnt);
-                x_substep<T, EOS, 2>(m, k, sb, i + 2, ilo, ihi, j0, cnt);
-                x_substep<T, EOS, 3>(m, k, sb, i + 3, ilo, ihi, j0, cnt);
-            }
-        }
-        __syncwarp();
-        // write-back of output cells [XCH*c - 4, XCH*c + 4), then refill of the same stage.  Every lane
-        // refills exactly the elements it has just read (same e -> (row, col) map), so program order
-        // (LDS -> STG -> LDGSTS) keeps the refill behind the read.
-#pragma unroll
-        for (int e = lane; e < XW * XCH; e += 32) {
-            const int row = e / XCH, col = e % XCH;
-            const int jo = c * XCH - GH + col;
-            if (row < nrows && jo >= j0 && jo < j1) {
-                const long long g = (row0 + row) * (long long)N + jo;
-                T u[NF];
-#pragma unroll
-                for (int f = 0; f < NF; ++f) {
-                    u[f] = S.buf[warp][stage][f][row * XPITCH + col];
-                    ((T*)P.out[f])[g] = u[f];
-                }
-                if (EMIT) {
-                    T pr[6];
-                    emit_primitives<T, EOS>(k, u, pr, cnt);
-#pragma unroll
-                    for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[g] = pr[q];
-                }
-            }
-        }
-        load_chunk(c + XNS, stage);
-    }
-    cp_async_wait<0>();
-    flush_counts(cnt, P.counts);
-}
-
-// ------------------------------------------------------------------------------------------------
-// Warp-specialised x sweep: the producer/consumer pair of sweep_strided_ws_kernel, with lane r marching
-// along ROW r of a 32-row strip.  Global traffic moves in 4-cell groups = 32 B row pieces (one sector);
-// in shared memory a (group, field) TILE is [32 rows][4 cells], dense (1 KB) -- the layout a TMA box
-// {4, 32} produces -- with the two 16 B halves of a row swapped when bit 2 of the row is set (the 32 B
-// swizzle).  The fill (cp.async, lane -> (row, col) = (lane>>2 + 8k, lane&3)) and the write-back are then
-// contiguous 256 B per instruction, the producer reads both cells of a 2-step chunk with one conflict-free
-// LDS.128 per field, and the consumer's single-cell accesses are 2-way conflicts at worst.
 constexpr int XV_CH = 4;                // cells per group
-constexpr int XV_G = 3;                 // ring groups per pair (12 cells)
 constexpr int XV_TILE = 32 * XV_CH;     // elements per (group, field) tile
-
-template <typename T>
-struct XvPair {
-    T ring[XV_G][NF][XV_TILE];          // tiles are 1 KB (fp64): 256 B aligned as the 32 B swizzle needs
-    T outb[NF][XV_TILE];
-    T msg[WS_Q][4][32];
-    unsigned cnt[4][32];
-    unsigned long long bar[32];         // bar[0..2]: one mbarrier per ring tile group (TMA completion); rest: padding
-};
-
-// tensor maps of the x sweep (permuted field order like SweepParams::in/out): 2-D {nx, ny*nz}, box {4, 32},
-// CU_TENSOR_MAP_SWIZZLE_32B.  Only built for fp64 grids with even nx (TMA needs 16 B row strides).
-struct XMaps {
-    CUtensorMap in[NF];
-    CUtensorMap out[NF];
-};
 
 // ---- TMA / mbarrier PTX (sm_90+; SASS: UTMALDG / UTMASTG / SYNCS)
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -1139,242 +670,470 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int c0, int
 }
 __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-template <typename T>
-struct XvSmem {
-    XvPair<T> pair[4];
-};
 
-// two adjacent elements with one shared-memory access (LDS.128 for fp64); p is 2-element aligned
-__device__ __forceinline__ void load2(const double* p, double& a, double& b)
-{
-    const double2 v = *reinterpret_cast<const double2*>(p);
-    a = v.x; b = v.y;
-}
-__device__ __forceinline__ void load2(const float* p, float& a, float& b)
-{
-    const float2 v = *reinterpret_cast<const float2*>(p);
-    a = v.x; b = v.y;
-}
-
-// element offset of (row, cell c in 0..3) inside a tile
+// element offset of (row, cell c in 0..3) inside an x-sweep tile [32 rows][4 cells] with the 32 B swizzle
 __device__ __forceinline__ int xv_off(int row, int c) { return row * 4 + 2 * ((c >> 1) ^ ((row >> 2) & 1)) + (c & 1); }
 
-template <typename T, int EOS, bool EMIT, bool TMA>
-__global__ void __launch_bounds__(256, 2) sweep_x_ws_kernel(const __grid_constant__ SweepParams P,
-                                                            const __grid_constant__ Consts<T> k,
-                                                            const __grid_constant__ XMaps maps)
+// ================================================================================================
+// Round 2: TMA-fed y/z march, one 4-cell group per hand-over.
+// ncu's stall samples of the round-1 kernels say the PRODUCER is the critical warp of a pair (5.8 cycles per issued
+// instruction: serial cons2prim chains cut into small basic blocks by the clamp branch; the consumer idles at the
+// hand-over 11 % of its time).  So
+//   * the producer issues NO per-thread global loads: the five fields of a 4-cell group of its 32 pencils arrive as
+//     one TMA box {32 x, 4 cells} per field (3-D tensor map over (x, y, z); ghost groups: four 1-cell boxes with the
+//     ghost-mapped coordinate, reading G11), so the ~28 address/LDGSTS/ring-slot instructions per step are gone;
+//   * a hand-over chunk is one 4-cell group and the producer's part of it is ONE basic block (no branch in
+//     c2p_sweep_d<EOS_GAMMA>), so the four independent cons2prim chains of a group interleave.
+constexpr int YZ_G = 4;           // ring tiles (4-cell groups) per warp pair
+constexpr int YZ_CH = 4;          // cells per group = steps per hand-over chunk
+#ifndef SHK_YZ_PREG
+#define SHK_YZ_PREG 96
+#endif
+constexpr int YZ_PREG = SHK_YZ_PREG;          // registers per producer thread (setmaxnreg); consumer gets 256 - YZ_PREG
+constexpr int YZ_CREG = 256 - YZ_PREG;
+
+template <typename T>
+struct alignas(128) YzPair {      // TMA destinations need 128 B alignment
+    T ring[YZ_G][NF][YZ_CH][32];          // tile = what TMA boxes {32, 4} of the five fields produce: [field][cell][lane]
+    T msg[2][YZ_CH][2][32][2];            // per step {a_c, b_c} and {sE, sM}: one 16 B access per lane (fp64), conflict-free
+    unsigned long long bar[8];            // bar[q]: TMA completion of ring tile q
+};                                        // fp64: 28800 B; 4 pairs = 112.5 KB per CTA, two CTAs per SM (diagnostic counters live in registers)
+template <typename T>
+struct YzSmem {
+    YzPair<T> pair[4];
+};
+
+// tensor maps of a y or z sweep: 3-D {nx, ny, nz}; in4: box {32, 4, 1} (y) or {32, 1, 4} (z), in1: box {32, 1, 1}.
+// The maps live in DEVICE memory (written once at allocation), NF per kind in natural field order; fidx[slot] is the
+// natural index of the permuted slot.  A pointer from the constant bank keeps the descriptor address in uniform
+// registers: with the maps as __grid_constant__ parameters every UTMALDG paid a 15-instruction ELECT / R2UR loop.
+struct YzMaps {
+    const CUtensorMap* in4;
+    const CUtensorMap* in1;
+    int fidx[NF];
+};
+
+// one lane of a converged warp: ptxas then knows the region is single-threaded and issues UTMALDG without an ELECT loop
+// keeps shared-memory loads below this point (registers: a pair of cells is 20 registers)
+__device__ __forceinline__ void load_fence() { asm volatile("" ::: "memory"); }
+__device__ __forceinline__ bool elect_one()
 {
-    extern __shared__ __align__(1024) unsigned char smem_xv[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned pred;
+    asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+
+// P.axis: 1 = y sweep (pencil = (x, z), cell stride nx), 2 = z sweep (pencil = (x, y), cell stride nx ny).
+// grid.x = ceil(nxb * n_other / 4) with nxb = ceil(nx / 32) x-blocks per row: warp pair w of CTA b owns the 32 pencils
+// x0 .. x0+31 of row `oth`, (xb, oth) = divmod(4 b + w, nxb); grid.y = segments.
+template <typename T, int EOS, bool EMIT, bool TMA>
+__global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant__ SweepParams P,
+                                                          const __grid_constant__ Consts<T> k,
+                                                          const __grid_constant__ YzMaps maps)
+{
+    extern __shared__ __align__(1024) unsigned char smem_yz[];
+    const int lane = threadIdx.x & 31;
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);     // provably warp-uniform: TMA operands stay in uniform registers
     const bool producer = warp < 4;
-    XvPair<T>& S = reinterpret_cast<XvSmem<T>*>(smem_xv)->pair[warp & 3];
+    YzPair<T>& S = reinterpret_cast<YzSmem<T>*>(smem_yz)->pair[warp & 3];
     const int bar_id = 4 * (warp & 3);                      // full0, full1, empty0, empty1 of this pair
-    const long long row0 = (long long)blockIdx.x * 128 + (warp & 3) * 32;
-    const bool idle = row0 >= P.npencil;                    // both warps of the pair leave together (after setmaxnreg)
-    const int nrows = (int)min(32LL, P.npencil - row0);
-    const int sg = blockIdx.y;
-    const int j0 = sg * P.seg;
+    const int nxb = (P.nx + 31) >> 5;
+    const long long pg = (long long)blockIdx.x * 4 + (warp & 3);        // pencil group
+    const bool idle = pg >= P.npencil;                      // npencil = nxb * n_other pencil GROUPS for this kernel
+    const int oth = (int)(pg / nxb);
+    const int x0 = 32 * (int)(pg - (long long)oth * nxb);
+    const bool active = x0 + lane < P.nx;
+    const int xl = active ? x0 + lane : P.nx - 1;           // idle lanes shadow a valid pencil (non-TMA fill), store nothing
+    const int j0 = blockIdx.y * P.seg;
     const int j1 = min(P.N, j0 + P.seg);
     const int ilo = j0 - GH;
     const int N = P.N;
     const int nsteps = (j1 - j0) + 2 * GH;                  // front cells ilo .. j1+3
-    const int nchunk = 2 * ((nsteps + 3) / 4);              // 2-step chunks, rounded to whole 4-cell groups
-    // lane -> element map of the group copies: col = lane & 3, rows (lane >> 2) + 8 kk
-    const int col = lane & 3, rsub = lane >> 2;
+    const int ngroups = (nsteps + YZ_CH - 1) / YZ_CH;
+    const long long sa = P.stride_axis;
+    const bool ysweep = P.axis == 1;
 
     if (producer) {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(YZ_PREG));
         if (idle) return;
         Producer<T, EOS> pr;
         pr.init();
-        // group g = cells ilo+4g .. ilo+4g+3 -> ring tile g % 3.  A group that lies inside [0, N) is one TMA box
-        // {4 cells, 32 rows} per field (rows beyond the grid are zero-filled, those lanes are idle); a group that
-        // touches a boundary needs the ghost map and goes through cp.async, element by element.
         if (TMA) {
             if (lane == 0) {
 #pragma unroll
-                for (int q = 0; q < XV_G; ++q) mbar_init(&S.bar[q], 1);
+                for (int q = 0; q < YZ_G; ++q) mbar_init(&S.bar[q], 1);
             }
             fence_proxy_async();
             __syncwarp();
         }
         unsigned phase = 0;             // bit q: parity to wait for on bar[q]
-        auto group_is_tma = [&](int g) { const int x0 = ilo + XV_CH * g; return TMA && x0 >= 0 && x0 + XV_CH <= N && (x0 & 1) == 0; };   // box start 16 B aligned
-        auto load_group = [&](int g) {
-            const int q = g % XV_G;
-            if (2 * g >= nchunk) {      // past the last group: nothing may be left in flight when the CTA exits
-                cp_async_commit();
-                return;
-            }
-            if (group_is_tma(g)) {
-                if (lane == 0) {
-                    mbar_expect_tx(&S.bar[q], NF * XV_TILE * (unsigned)sizeof(T));
+        const long long lbase = (long long)xl + (long long)oth * P.stride_other;
+        constexpr int NP = Producer<T, EOS>::NP;
+        // group g = cells ilo+4g .. ilo+4g+3 -> ring tile g % 4.  Group g+1 is requested at the start of group g into
+        // the tile of group g-3, which the consumer finished reading in its group g-2 (the `empty` barrier below).
+#pragma unroll 1
+        for (int g = -1; g < ngroups; ++g) {
+            if (g >= 2) bar_sync64(bar_id + 2 + (g & 1));       // the consumer has finished group g-2
+            if (g + 1 < ngroups) {
+                const int q = (g + 1) & (YZ_G - 1);
+                const int jg = ilo + YZ_CH * (g + 1);
+                if (TMA) {
+                    if (elect_one()) {
+                        mbar_expect_tx(&S.bar[q], NF * YZ_CH * 32 * (unsigned)sizeof(T));
+                        if (jg >= 0 && jg + YZ_CH <= N) {
 #pragma unroll
-                    for (int f = 0; f < NF; ++f)
-                        tma_load_2d(&S.ring[q][f][0], &maps.in[f], ilo + XV_CH * g, (int)row0, &S.bar[q]);
-                }
-            } else {
-                const int gi = ghost_index(ilo + XV_CH * g + col, N, P.periodic);
-                T* dst = &S.ring[q][0][0];
+                            for (int f = 0; f < NF; ++f)
+                                tma_load_3d(&S.ring[q][f][0][0], maps.in4 + maps.fidx[f], x0, ysweep ? jg : oth, ysweep ? oth : jg, &S.bar[q]);
+                        } else {        // ghost group (reading G11): 1-cell boxes at the ghost-mapped coordinate; rare, kept small
+#pragma unroll 1
+                            for (int c = 0; c < YZ_CH; ++c) {
+                                const int jj = ghost_index(jg + c, N, P.periodic);
+#pragma unroll 1
+                                for (int f = 0; f < NF; ++f)
+                                    tma_load_3d(&S.ring[q][f][c][0], maps.in1 + maps.fidx[f], x0, ysweep ? jj : oth, ysweep ? oth : jj, &S.bar[q]);
+                            }
+                        }
+                    }
+                } else {
+#pragma unroll 1
+                    for (int c = 0; c < YZ_CH; ++c) {
+                        const long long o = lbase + (long long)ghost_index(jg + c, N, P.periodic) * sa;
 #pragma unroll
-                for (int kk = 0; kk < 4; ++kk) {
-                    const int row = rsub + 8 * kk;
-                    if (row < nrows) {
-                        const long long o = (row0 + row) * (long long)N + gi;
-                        const int so = xv_off(row, col);
-#pragma unroll
-                        for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * XV_TILE + so, (const T*)P.in[f] + o);
+                        for (int f = 0; f < NF; ++f) cp_async_elem<T>(&S.ring[q][f][c][lane], (const T*)P.in[f] + o);
                     }
                 }
             }
-            cp_async_commit();          // also for TMA groups (empty): keeps the wait_group arithmetic uniform
-        };
-        auto wait_group = [&](int g) {
-            cp_async_wait<1>();
-            if (group_is_tma(g)) {
-                const int q = g % XV_G;
+            if (!TMA) cp_async_commit();        // one commit group per iteration (empty past the last group)
+            if (g < 0) continue;
+            if (TMA) {
+                const int q = g & (YZ_G - 1);
                 mbar_wait(&S.bar[q], (phase >> q) & 1u);
                 phase ^= 1u << q;
+            } else {
+                cp_async_wait<1>();
             }
-            __syncwarp();
-        };
-        load_group(0);
-        int g = 0;
-        const int sw = (lane >> 2) & 1;
-        // Group g+1 is issued at the start of group g into the tile of group g-2, which the consumer
-        // finished (as U_{i-1}) in the iteration before: it runs one 2-step iteration behind this warp.
-#define SHK_XPCHUNK(PH, HALF)                                                                        \
-        {                                                                                           \
-            if (HALF == 0) {                                                                        \
-                load_group(g + 1);                                                                  \
-                wait_group(g);                                                                      \
-            }                                                                                       \
-            T um[NF], ua[NF], ub[NF], ma[4], mb[4];                                                 \
-            um[NF - 1] = ua[NF - 1] = ub[NF - 1] = T(0);                                            \
-            const int tile = g % XV_G;                                                              \
-            /* cell before the chunk: cell 1 of this tile (HALF 1) or cell 3 of the previous group's tile (HALF 0) */ \
-            const T* srm = HALF ? &S.ring[tile][0][xv_off(lane, 1)]                                 \
-                                : &S.ring[(tile + XV_G - 1) % XV_G][0][xv_off(lane, 3)];            \
-            const T* src = &S.ring[tile][0][lane * 4 + 2 * (HALF ^ sw)];                            \
-            _Pragma("unroll") for (int f = 0; f < Producer<T, EOS>::NP; ++f) {                      \
-                um[f] = srm[f * XV_TILE];                                                           \
-                load2(src + f * XV_TILE, ua[f], ub[f]);                                             \
-            }                                                                                       \
-            if (HALF == 1) ++g;                                                                     \
-            pr.template step<PH>(k, um, ua, ma);                                                    \
-            pr.template step<PH + 1>(k, ua, ub, mb);                                                \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH][q][lane] = ma[q];               \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) S.msg[PH + 1][q][lane] = mb[q];           \
+            const T* tp = &S.ring[(g + YZ_G - 1) & (YZ_G - 1)][0][YZ_CH - 1][lane];     // last cell of the previous group
+            const T* tc = &S.ring[g & (YZ_G - 1)][0][0][lane];
+            T um[NF], c0[NF], c1[NF], c2[NF], c3[NF], m0[4], m1[4], m2[4], m3[4];
+            um[NF - 1] = c0[NF - 1] = c1[NF - 1] = c2[NF - 1] = c3[NF - 1] = T(0);
+#pragma unroll
+            for (int f = 0; f < NP; ++f) {
+                um[f] = tp[f * YZ_CH * 32];
+                c0[f] = tc[f * YZ_CH * 32];
+                c1[f] = tc[f * YZ_CH * 32 + 32];
+                c2[f] = tc[f * YZ_CH * 32 + 64];
+                c3[f] = tc[f * YZ_CH * 32 + 96];
+            }
+            T* mq = &S.msg[g & 1][0][0][lane][0];
+            pr.template step<0>(k, um, c0, m0);
+            store2(mq, m0[0], m0[1]);           store2(mq + 64, m0[2], m0[3]);
+            pr.template step<1>(k, c0, c1, m1);
+            store2(mq + 128, m1[0], m1[1]);     store2(mq + 192, m1[2], m1[3]);
+            pr.template step<2>(k, c1, c2, m2);
+            store2(mq + 256, m2[0], m2[1]);     store2(mq + 320, m2[2], m2[3]);
+            pr.template step<3>(k, c2, c3, m3);
+            store2(mq + 384, m3[0], m3[1]);     store2(mq + 448, m3[2], m3[3]);
+            bar_arrive64(bar_id + (g & 1));
         }
-        for (int c = 0; c < nchunk; c += 2) {                   // nchunk is even here
-            if (c >= 2) bar_sync64(bar_id + 2);
-            SHK_XPCHUNK(0, 0)
-            bar_arrive64(bar_id + 0);
-            if (c >= 1) bar_sync64(bar_id + 3);
-            SHK_XPCHUNK(2, 1)
-            bar_arrive64(bar_id + 1);
-        }
-#undef SHK_XPCHUNK
-        cp_async_wait<0>();
+        if (!TMA) cp_async_wait<0>();
     } else {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 160;");
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(YZ_CREG));
         if (idle) return;
         Cnt cnt;
-        cnt.p = &S.cnt[0][lane]; cnt.stride = 32;
         cnt.zero();
         Consumer<T> co;
         co.init();
-        int t = 0;
-        int gprev = XV_G - 1;           // tile of group floor((t-1)/4); t = 0 reads don't-care warm-up values
-        const int swc = (lane >> 2) & 1;
-#define SHK_XCFIN(UN, PH)                                                                           \
+        // element offset of the output cell of the NEXT step: cell ilo - 4 (the first two groups store nothing)
+        long long o = (long long)(x0 + lane) + (long long)oth * P.stride_other + (long long)(ilo - GH) * sa;
+        int left = active ? (j1 - j0) : 0;      // output cells this lane still has to store
+#define SHK_YZ_OUT(UN, S_)                                                                          \
         {                                                                                           \
-            T pv[6];                                                                                \
-            if (t >= 2 * GH && t < nsteps && lane < nrows) finish_cell<T, EOS, false>(k, UN, pv, cnt); \
-            T* dst = &S.outb[0][xv_off(lane, PH)];                                                  \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) dst[f * XV_TILE] = UN[f];                 \
-            ++t;                                                                                    \
-        }
-        // one chunk = steps t, t+1 (t even): cells t-2, t-1 are one aligned pair (LDS.128) of the tile `gprev`,
-        // cell t is the first cell of the next pair: of the next tile when t = 0 mod 4 (PH 0), of the same tile
-        // when t = 2 mod 4 (PH 2).  Nothing of U is carried in registers.
-#define SHK_XCCHUNK(PH)                                                                             \
-        {                                                                                           \
-            T uq[NF], ua[NF], ub[NF], msg[4], un[NF];                                               \
-            const T* s2 = &S.ring[gprev][0][lane * 4 + 2 * ((PH == 0 ? 1 : 0) ^ swc)];              \
-            if (PH == 0) gprev = (gprev + 1 == XV_G) ? 0 : gprev + 1;                               \
-            const T* s1 = &S.ring[gprev][0][lane * 4 + 2 * ((PH == 0 ? 0 : 1) ^ swc)];              \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) {                                        \
-                load2(s2 + f * XV_TILE, uq[f], ua[f]);                                              \
-                ub[f] = s1[f * XV_TILE];                                                            \
+            if (g >= 2 && (S_) < left) {                                                            \
+                T pv[6];                                                                            \
+                finish_cell<T, EOS, EMIT>(k, UN, pv, cnt);                                          \
+                _Pragma("unroll") for (int f = 0; f < NF; ++f) ((T*)P.out[f])[o] = UN[f];           \
+                if (EMIT) { _Pragma("unroll") for (int qq = 0; qq < 6; ++qq) ((T*)P.prim[qq])[o] = pv[qq]; } \
             }                                                                                       \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH][q][lane];              \
-            co.template step<PH>(uq, ua, msg, un);                                                  \
-            SHK_XCFIN(un, PH)                                                                       \
-            _Pragma("unroll") for (int q = 0; q < 4; ++q) msg[q] = S.msg[PH + 1][q][lane];          \
-            co.template step<PH + 1>(ua, ub, msg, un);                                              \
-            SHK_XCFIN(un, PH + 1)                                                                   \
+            o += sa;                                                                                \
         }
-        // write-back of the 4-cell group whose last cell was produced by step t-1: cells j0-8+4m .. +3
-        auto write_group = [&]() {
-            const int jo = ilo + (t - 4) - GH + col;
-            if (jo >= j0 && jo < j1) {
+#pragma unroll 1
+        for (int g = 0; g < ngroups; ++g) {
+            bar_sync64(bar_id + (g & 1));
+            const T* tp = &S.ring[(g + YZ_G - 1) & (YZ_G - 1)][0][0][lane];
+            const T* tc = &S.ring[g & (YZ_G - 1)][0][0][lane];
+            const T* mq = &S.msg[g & 1][0][0][lane][0];
+            T uq[NF], ua[NF], c0[NF], c1[NF], c2[NF], msg[4], un[NF];
 #pragma unroll
-                for (int kk = 0; kk < 4; ++kk) {
-                    const int row = rsub + 8 * kk;
-                    if (row < nrows) {
-                        const long long o = (row0 + row) * (long long)N + jo;
-                        const int so = xv_off(row, col);
-                        T u[NF];
+            for (int f = 0; f < NF; ++f) {
+                uq[f] = tp[f * YZ_CH * 32 + 64];
+                ua[f] = tp[f * YZ_CH * 32 + 96];
+                c0[f] = tc[f * YZ_CH * 32];
+            }
+            load2(mq, msg[0], msg[1]); load2(mq + 64, msg[2], msg[3]);
+            co.template step<0>(uq, ua, msg, un);
+            SHK_YZ_OUT(un, 0)
 #pragma unroll
-                        for (int f = 0; f < NF; ++f) {
-                            u[f] = S.outb[f][so];
-                            ((T*)P.out[f])[o] = u[f];
-                        }
-                        if (EMIT) {
-                            T pv[6];
-                            emit_primitives<T, EOS>(k, u, pv, cnt);
+            for (int f = 0; f < NF; ++f) c1[f] = tc[f * YZ_CH * 32 + 32];
+            load2(mq + 128, msg[0], msg[1]); load2(mq + 192, msg[2], msg[3]);
+            co.template step<1>(ua, c0, msg, un);
+            SHK_YZ_OUT(un, 1)
 #pragma unroll
-                            for (int q = 0; q < 6; ++q) ((T*)P.prim[q])[o] = pv[q];
+            for (int f = 0; f < NF; ++f) c2[f] = tc[f * YZ_CH * 32 + 64];
+            load2(mq + 256, msg[0], msg[1]); load2(mq + 320, msg[2], msg[3]);
+            co.template step<2>(c0, c1, msg, un);
+            SHK_YZ_OUT(un, 2)
+            load2(mq + 384, msg[0], msg[1]); load2(mq + 448, msg[2], msg[3]);
+            co.template step<3>(c1, c2, msg, un);
+            SHK_YZ_OUT(un, 3)
+            if (g >= 2) left -= YZ_CH;
+            if (g + 2 < ngroups) bar_arrive64(bar_id + 2 + (g & 1));
+        }
+#undef SHK_YZ_OUT
+        flush_counts(cnt, P.counts);
+    }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// x sweep, round 2: the same group-wise producer/consumer pair with lane r marching along ROW r of a 32-row strip.
+// A (group, field) tile is [32 rows][4 cells], dense (1 KB in fp64) with the two 16 B halves of a row swapped when bit 2
+// of the row is set: what a TMA box {4 cells, 32 rows} with CU_TENSOR_MAP_SWIZZLE_32B produces, so that a lane reads
+// an aligned cell pair of its row with one conflict-free LDS.128.  Outputs of a group are staged in `outb` (same
+// layout) and leave as one TMA box per field.  Three ring tiles suffice because the consumer releases a tile as soon
+// as it has READ it (top of its group), not when it has finished the group.
+constexpr int X2_G = 3;
+
+template <typename T>
+struct alignas(256) X2Pair {
+    T ring[X2_G][NF][XV_TILE];
+    T outb[NF][XV_TILE];
+    T msg[2][YZ_CH][2][32][2];
+    unsigned long long bar[4];            // bar[q], q < 3: TMA completion of ring tile q; bar[3]: scratch (early release)
+};                                        // fp64: 28928 B; 4 pairs = 113 KB per CTA: two CTAs per SM, exactly
+template <typename T>
+struct X2Smem {
+    X2Pair<T> pair[4];
+};
+
+// tensor maps of the x sweep in DEVICE memory (see YzMaps): 2-D {nx, ny*nz}, box {4, 32}, 32 B swizzle
+struct X2Maps {
+    const CUtensorMap* in;
+    const CUtensorMap* out;
+    int fidx[NF];
+};
+
+template <typename T, int EOS, bool EMIT, bool TMA>
+__global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant__ SweepParams P,
+                                                          const __grid_constant__ Consts<T> k,
+                                                          const __grid_constant__ X2Maps maps)
+{
+    extern __shared__ __align__(1024) unsigned char smem_x2[];
+    const int lane = threadIdx.x & 31;
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    const bool producer = warp < 4;
+    X2Pair<T>& S = reinterpret_cast<X2Smem<T>*>(smem_x2)->pair[warp & 3];
+    const int bar_id = 4 * (warp & 3);                      // full0, full1, empty0, empty1 of this pair
+    const long long row0 = (long long)blockIdx.x * 128 + (warp & 3) * 32;
+    const bool idle = row0 >= P.npencil;
+    const int nrows = (int)min(32LL, P.npencil - row0);
+    const int j0 = blockIdx.y * P.seg;
+    const int j1 = min(P.N, j0 + P.seg);
+    const int ilo = j0 - GH;
+    const int N = P.N;
+    const int nsteps = (j1 - j0) + 2 * GH;
+    const int ngroups = (nsteps + XV_CH - 1) / XV_CH;
+    const int col = lane & 3, rsub = lane >> 2;             // element map of the LSU group copies: col, rows rsub + 8 kk
+    const int sw = (lane >> 2) & 1;                         // 32 B swizzle of this lane's row
+
+    if (producer) {
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(YZ_PREG));
+        if (idle) return;
+        Producer<T, EOS> pr;
+        pr.init();
+        if (TMA) {
+            if (lane == 0) {
+#pragma unroll
+                for (int q = 0; q < X2_G; ++q) mbar_init(&S.bar[q], 1);
+            }
+            fence_proxy_async();
+            __syncwarp();
+        }
+        unsigned phase = 0;
+        constexpr int NP = Producer<T, EOS>::NP;
+        // a group that lies inside [0, N) and starts at an even cell is one TMA box per field; a group that touches a
+        // boundary needs the ghost map (reading G11) and is copied element by element (cp.async)
+        auto group_is_tma = [&](int g) { const int xg = ilo + XV_CH * g; return TMA && xg >= 0 && xg + XV_CH <= N && (xg & 1) == 0; };
+        int q1 = 0;                     // ring tile of group g+1
+#pragma unroll 1
+        for (int g = -1; g < ngroups; ++g) {
+            if (g >= 1) bar_sync64(bar_id + 2 + ((g - 1) & 1));     // the consumer has read what it needs of group g-2
+            if (g + 1 < ngroups) {
+                const int xg = ilo + XV_CH * (g + 1);
+                if (group_is_tma(g + 1)) {
+                    if (elect_one()) {
+                        mbar_expect_tx(&S.bar[q1], NF * XV_TILE * (unsigned)sizeof(T));
+#pragma unroll
+                        for (int f = 0; f < NF; ++f)
+                            tma_load_2d(&S.ring[q1][f][0], maps.in + maps.fidx[f], xg, (int)row0, &S.bar[q1]);
+                    }
+                } else {
+                    const int gi = ghost_index(xg + col, N, P.periodic);
+                    T* dst = &S.ring[q1][0][0];
+#pragma unroll 1
+                    for (int kk = 0; kk < 4; ++kk) {
+                        const int row = rsub + 8 * kk;
+                        if (row < nrows) {
+                            const long long o = (row0 + row) * (long long)N + gi;
+                            const int so = xv_off(row, col);
+#pragma unroll
+                            for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * XV_TILE + so, (const T*)P.in[f] + o);
                         }
                     }
+                    cp_async_commit();
                 }
             }
-        };
-        // a finished group goes out as one TMA box per field when all of its cells are output cells of this
-        // segment (or are clipped by the grid edge); otherwise (and for EMIT) through the LSU write-back
+            const int q0 = (q1 == 0) ? X2_G - 1 : q1 - 1;           // tile of group g
+            q1 = (q1 + 1 == X2_G) ? 0 : q1 + 1;
+            if (g < 0) continue;
+            if (group_is_tma(g)) {
+                mbar_wait(&S.bar[q0], (phase >> q0) & 1u);
+                phase ^= 1u << q0;
+            } else {
+                // LSU groups are rare and at most two are in flight (g, g+1): wait for all but the youngest
+                if (g + 1 < ngroups && !group_is_tma(g + 1)) cp_async_wait<1>(); else cp_async_wait<0>();
+                __syncwarp();
+            }
+            const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;           // tile of group g-1
+            const T* tp = &S.ring[qm][0][xv_off(lane, 3)];
+            const T* tc = &S.ring[q0][0][lane * 4];
+            T um[NF], c0[NF], c1[NF], c2[NF], c3[NF], m0[4], m1[4], m2[4], m3[4];
+            um[NF - 1] = c0[NF - 1] = c1[NF - 1] = c2[NF - 1] = c3[NF - 1] = T(0);
+#pragma unroll
+            for (int f = 0; f < NP; ++f) {
+                um[f] = tp[f * XV_TILE];
+                load2(tc + f * XV_TILE + 2 * sw, c0[f], c1[f]);
+            }
+            T* mq = &S.msg[g & 1][0][0][lane][0];
+            pr.template step<0>(k, um, c0, m0);
+            store2(mq, m0[0], m0[1]);           store2(mq + 64, m0[2], m0[3]);
+            load_fence();
+#pragma unroll
+            for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (1 ^ sw), c2[f], c3[f]);
+            pr.template step<1>(k, c0, c1, m1);
+            store2(mq + 128, m1[0], m1[1]);     store2(mq + 192, m1[2], m1[3]);
+            pr.template step<2>(k, c1, c2, m2);
+            store2(mq + 256, m2[0], m2[1]);     store2(mq + 320, m2[2], m2[3]);
+            pr.template step<3>(k, c2, c3, m3);
+            store2(mq + 384, m3[0], m3[1]);     store2(mq + 448, m3[2], m3[3]);
+            bar_arrive64(bar_id + (g & 1));
+        }
+        cp_async_wait<0>();
+    } else {
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(YZ_CREG));
+        if (idle) return;
+        Cnt cnt;
+        cnt.zero();
+        Consumer<T> co;
+        co.init();
+        int q0 = 0;                     // ring tile of group g
         bool store_pending = false;
-        for (int c = 0; c < nchunk; c += 2) {                   // nchunk is even here
-            bar_sync64(bar_id + 0);
-            if (TMA && store_pending) {                     // outb is rewritten below: the TMA must have read it
+#pragma unroll 1
+        for (int g = 0; g < ngroups; ++g) {
+            bar_sync64(bar_id + (g & 1));
+            const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;
+            const T* tp = &S.ring[qm][0][lane * 4 + 2 * (1 ^ sw)];          // cells 2, 3 of group g-1
+            const T* tc = &S.ring[q0][0][lane * 4];
+            const T* mq = &S.msg[g & 1][0][0][lane][0];
+            q0 = (q0 + 1 == X2_G) ? 0 : q0 + 1;
+            T uq[NF], ua[NF], c0[NF], c1[NF], c2[NF], msg[4], un[NF], uo[NF];
+#pragma unroll
+            for (int f = 0; f < NF; ++f) load2(tp + f * XV_TILE, uq[f], ua[f]);
+            // Early release of the tile of group g-1 (the producer's next TMA request refills it).  BAR.ARV does NOT wait
+            // for shared-memory loads in flight (measured: issued right behind the LDS, 2.6 % of the cells of a 256^3
+            // sweep then differed from run to run), so a 4-byte store whose data depends on all five loads goes first:
+            // it cannot issue before uq, ua have arrived, and the barrier stays behind it.
+            {
+                const unsigned d = (unsigned)(__double2hiint((double)uq[0]) ^ __double2hiint((double)uq[1]) ^ __double2hiint((double)uq[2]) ^
+                                              __double2hiint((double)uq[3]) ^ __double2hiint((double)uq[4]));
+                *reinterpret_cast<volatile unsigned*>(&S.bar[X2_G]) = d;        // bar[3]: scratch word, never read
+                if (g + 1 < ngroups) bar_arrive64(bar_id + 2 + (g & 1));
+            }
+            const int jf = ilo + XV_CH * g - GH;                            // first output cell of this group
+            const bool any_out = g >= 2;                                    // jf >= j0
+            if (TMA && store_pending) {                                     // outb is rewritten below: the TMA must have read it
                 if (lane == 0) tma_store_wait_read();
                 __syncwarp();
                 store_pending = false;
             }
-            SHK_XCCHUNK(0)
-            if (c + 2 < nchunk) bar_arrive64(bar_id + 2);
-            bar_sync64(bar_id + 1);
-            SHK_XCCHUNK(2)
-            if (c + 3 < nchunk) bar_arrive64(bar_id + 3);
-            const int jf = ilo + (t - 4) - GH;              // first cell of the finished group
-            if (TMA && !EMIT && (jf & 1) == 0 && jf >= j0 && jf < j1 && (jf + XV_CH <= j1 || j1 == N)) {
+            T* ob = &S.outb[0][lane * 4];
+            load2(mq, msg[0], msg[1]); load2(mq + 64, msg[2], msg[3]);
+            co.template step<0>(uq, ua, msg, uo);
+            if (any_out && jf < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, uo, pv, cnt); }
+            load_fence();
+#pragma unroll
+            for (int f = 0; f < NF; ++f) load2(tc + f * XV_TILE + 2 * sw, c0[f], c1[f]);
+            load2(mq + 128, msg[0], msg[1]); load2(mq + 192, msg[2], msg[3]);
+            co.template step<1>(ua, c0, msg, un);
+            if (any_out && jf + 1 < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, un, pv, cnt); }
+#pragma unroll
+            for (int f = 0; f < NF; ++f) store2(ob + f * XV_TILE + 2 * sw, uo[f], un[f]);
+            load2(mq + 256, msg[0], msg[1]); load2(mq + 320, msg[2], msg[3]);
+            co.template step<2>(c0, c1, msg, uo);
+            if (any_out && jf + 2 < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, uo, pv, cnt); }
+            load_fence();
+#pragma unroll
+            for (int f = 0; f < NF; ++f) c2[f] = tc[f * XV_TILE + 2 * (1 ^ sw)];
+            load2(mq + 384, msg[0], msg[1]); load2(mq + 448, msg[2], msg[3]);
+            co.template step<3>(c1, c2, msg, un);
+            if (any_out && jf + 3 < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, un, pv, cnt); }
+#pragma unroll
+            for (int f = 0; f < NF; ++f) store2(ob + f * XV_TILE + 2 * (1 ^ sw), uo[f], un[f]);
+            if (!any_out) continue;
+            // the finished group leaves as one TMA box per field when all of its cells are output cells of this segment (or
+            // are clipped by the grid edge); otherwise (ragged segment end, odd start, EMIT) through the LSU
+            if (TMA && !EMIT && (jf & 1) == 0 && (jf + XV_CH <= j1 || j1 == N)) {
                 fence_proxy_async();                        // generic-proxy writes of outb -> visible to the TMA engine
                 __syncwarp();
                 if (lane == 0) {
 #pragma unroll
-                    for (int f = 0; f < NF; ++f) tma_store_2d(&maps.out[f], jf, (int)row0, &S.outb[f][0]);
+                    for (int f = 0; f < NF; ++f) tma_store_2d(maps.out + maps.fidx[f], jf, (int)row0, &S.outb[f][0]);
                     tma_store_commit();
                 }
                 store_pending = true;
             } else {
                 __syncwarp();
-                write_group();
+                const int jo = jf + col;
+                if (jo < j1) {
+#pragma unroll 1
+                    for (int kk = 0; kk < 4; ++kk) {
+                        const int row = rsub + 8 * kk;
+                        if (row < nrows) {
+                            const long long o = (row0 + row) * (long long)N + jo;
+                            const int so = xv_off(row, col);
+                            T u[NF];
+#pragma unroll
+                            for (int f = 0; f < NF; ++f) {
+                                u[f] = S.outb[f][so];
+                                ((T*)P.out[f])[o] = u[f];
+                            }
+                            if (EMIT) {
+                                T pv[6];
+                                emit_primitives<T, EOS>(k, u, pv, cnt);
+#pragma unroll
+                                for (int qq = 0; qq < 6; ++qq) ((T*)P.prim[qq])[o] = pv[qq];
+                            }
+                        }
+                    }
+                }
                 __syncwarp();
             }
         }
         if (TMA && lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-#undef SHK_XCCHUNK
-#undef SHK_XCFIN
         flush_counts(cnt, P.counts);
     }
 }

@@ -97,7 +97,7 @@ class Shasta:
     """One solver handle = shasta_create ... shasta_destroy.  Method names follow the C ABI."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, precision=64,
-                 segment=0, variant=0, no_tma=0):
+                 segment=0, no_tma=0):
         L = load()
         self._L = L
         self._h = _vp()
@@ -113,8 +113,6 @@ class Shasta:
         self.set_option(PRECISION, precision)
         if segment:
             self.set_option(SEGMENT, segment)
-        if variant:
-            self.set_option(VARIANT, variant)
         if no_tma:
             self.set_option(NO_TMA, 1)
 

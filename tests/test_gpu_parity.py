@@ -36,7 +36,8 @@ def test_single_axis_sweeps_ragged(oracle, axis, bc, kind):
     ref, o = parity.run_oracle(oracle, c, steps=1, table=[axis] * 3)
     got, s = parity.run_gpu(c, steps=1, table=[axis] * 3)
     assert_kernel_parity(got, ref, f"axis {axis} bc {bc} {kind}")
-    assert abs(s.diagnostics()[0] - o.diagnostics()[0]) <= max(2, o.diagnostics()[0] // 50)
+    # Pi fires in the same cells up to those sitting within rounding of the limit |M| = (1-1e-12) E
+    assert abs(s.diagnostics()[0] - o.diagnostics()[0]) <= max(2, o.diagnostics()[0] // 200)
 
 
 @pytest.mark.parametrize("shape", [(1, 1, 50), (1, 40, 1), (64, 1, 1), (5, 1, 9), (2, 3, 4), (3, 3, 3), (130, 2, 1),
@@ -59,19 +60,6 @@ def test_segmentation_does_not_change_the_answer(oracle, segment):
 
 
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
-@pytest.mark.parametrize("segment", [0, 9])
-def test_single_role_variant(oracle, bc, segment):
-    # SHASTA_VARIANT 1: one marching thread per pencil (the default, 0, is a producer/consumer warp pair)
-    c = inputs.random_state(150, 21, 19, seed=31 + bc, kind="rough", boundary=bc)
-    ref, _ = parity.run_oracle(oracle, c, steps=2)
-    got, _ = parity.run_gpu(c, steps=2, variant=1, segment=segment)
-    assert_kernel_parity(got, ref, f"variant 1 bc {bc} segment {segment}")
-    # not bitwise the default kernel: there the producer rounds the source increment before the consumer adds it
-    base, _ = parity.run_gpu(c, steps=2, segment=segment)
-    parity.assert_parity(got, base, 1e-13, label="variant 1 vs default")
-
-
-@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
 @pytest.mark.parametrize("shape", [(38, 19, 23), (64, 5, 7), (130, 33, 2), (8, 40, 3)])
 @pytest.mark.parametrize("segment", [0, 8, 12, 24])
 def test_x_sweep_tma_and_cp_async_paths(oracle, bc, shape, segment):
@@ -83,6 +71,22 @@ def test_x_sweep_tma_and_cp_async_paths(oracle, bc, shape, segment):
     got, _ = parity.run_gpu(c, steps=1, table=[0, 0, 0], segment=segment)
     assert_kernel_parity(got, ref, f"x sweep tma shape {shape} bc {bc} segment {segment}")
     alt, _ = parity.run_gpu(c, steps=1, table=[0, 0, 0], segment=segment, no_tma=1)
+    for k in parity.CONS + parity.PRIM:
+        assert np.array_equal(got[k], alt[k]), k
+
+
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("shape", [(38, 19, 23), (64, 9, 7), (130, 6, 5), (96, 40, 3), (32, 4, 4)])
+@pytest.mark.parametrize("segment", [0, 8, 12])
+def test_yz_sweeps_tma_and_cp_async_paths(oracle, bc, shape, segment):
+    # nx >= 32 and even: the y/z sweeps are fed by 3-D TMA boxes {32, 4 cells} (ghost groups: four 1-cell boxes at the
+    # ghost-mapped coordinate, partial x-blocks zero-filled and never stored); SHASTA_NO_TMA forces the cp.async fill.
+    nx, ny, nz = shape
+    c = inputs.random_state(nx, ny, nz, seed=nx + 5 * bc, kind="rough", boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=1, table=[1, 2, 1])
+    got, s = parity.run_gpu(c, steps=1, table=[1, 2, 1], segment=segment)
+    assert_kernel_parity(got, ref, f"y/z sweeps tma shape {shape} bc {bc} segment {segment}")
+    alt, _ = parity.run_gpu(c, steps=1, table=[1, 2, 1], segment=segment, no_tma=1)
     for k in parity.CONS + parity.PRIM:
         assert np.array_equal(got[k], alt[k]), k
 
@@ -190,13 +194,37 @@ def test_conserved_totals_periodic(oracle):
 
 
 # ------------------------------------------------------------------ T2: the configs
+# Bars (north_star): fp64 err_max <= 1e-10 per field, err_L1 reported (expected <= 1e-12).  Configs 3 and 4
+# amplify rounding noise: two equally valid fp64 evaluations of the ORACLE (strict vs FMA-contracted build) already
+# differ by more than 1e-10 in some primitive fields there, so for those fields the bar is max(1e-10, 4 x that floor);
+# the CONSERVED fields are held to 1e-10 outright.  Every achieved number goes to gpurun_out/parity_r2.json.
+CONS_OUTRIGHT = 1e-10
+
+
+def _check_config(oracle, name, c, got, ref, s=None, o=None, floor=True, l1=True, **meta):
+    fl = parity.noise_floor(oracle, c, ref, steps=meta.get("steps")) if floor else None
+    errs = parity.field_errors(got, ref)
+    bar = {k: (max(TOL64, 4.0 * fl[k][0]) if fl else TOL64) for k in errs}
+    for k in parity.CONS:
+        bar[k] = CONS_OUTRIGHT
+    rep = parity.field_report(got, ref, fl, bar)
+    if s is not None and o is not None:
+        meta["pi_fired_gpu_oracle"] = [s.diagnostics()[0], o.diagnostics()[0]]
+    parity.record(name, rep, **meta)
+    bad = {k: (v, bar[k]) for k, v in errs.items() if not v[0] <= bar[k]}
+    assert not bad, f"{name}: (err_max, err_L1), bar: {bad}; all: {rep}"
+    if l1:
+        badl = {k: v for k, v in errs.items() if not v[1] <= max(1e-12, 4.0 * (fl[k][1] if fl else 0.0))}
+        assert not badl, f"{name}: err_L1 above max(1e-12, 4 x floor): {badl}; all: {rep}"
+    return rep
+
+
 def test_config1_shock_tube(oracle):
     for e_right in (0.01, 1e-8):
         c = inputs.shock_tube(400, e_right)
         ref, o = parity.run_oracle(oracle, c)
         got, s = parity.run_gpu(c)
-        errs = parity.assert_parity(got, ref, TOL64, label=f"config1 eR={e_right}")
-        print("config1", e_right, errs)
+        _check_config(oracle, f"config1 eR={e_right}", c, got, ref, s, o, floor=False, steps=c["steps"], grid=[400, 1, 1])
         assert s.diagnostics()[0] == o.diagnostics()[0]
 
 
@@ -210,10 +238,9 @@ def test_config1_along_y_and_z(oracle):
 
 def test_config2_fireball(oracle):
     c = inputs.fireball(64, steps=100)
-    ref, _ = parity.run_oracle(oracle, c)
-    got, _ = parity.run_gpu(c)
-    errs = parity.assert_parity(got, ref, TOL64, label="config2")
-    print("config2", errs)
+    ref, o = parity.run_oracle(oracle, c)
+    got, s = parity.run_gpu(c)
+    _check_config(oracle, "config2 fireball 64^3", c, got, ref, s, o, floor=False, steps=100, grid=[64, 64, 64])
 
 
 def test_config3_spherical_riemann(oracle):
@@ -221,10 +248,8 @@ def test_config3_spherical_riemann(oracle):
     ref, o = parity.run_oracle(oracle, c)
     got, s = parity.run_gpu(c)
     # strong spherical shock: the rounding-noise floor of the step map itself reaches ~1e-10 in p
-    # (p = (Gamma-1)(e - n) cancels); bar = max(1e-10, 4 x floor), DESIGN.md 4
-    floor = parity.noise_floor(oracle, c, ref)
-    errs = parity.assert_parity_noise(got, ref, floor, TOL64, label="config3")
-    print("config3", errs, "floor", floor, o.diagnostics(), s.diagnostics())
+    # (p = (Gamma-1)(e - n) cancels)
+    _check_config(oracle, "config3 spherical riemann 128^3", c, got, ref, s, o, steps=100, grid=[128, 128, 128])
     t = np.array(s.conserved_totals())
     t0 = np.array(parity.run_gpu(c, steps=0)[1].conserved_totals())
     assert abs(t[0] - t0[0]) <= 1e-12 * t0[0] and abs(t[4] - t0[4]) <= 1e-12 * t0[4]
@@ -232,54 +257,105 @@ def test_config3_spherical_riemann(oracle):
 
 
 def test_config4_hotspots_reduced(oracle):
-    # same box, flow and hotspots on 96^3 for the full 200 steps (the 256^3 run is sampled below)
+    # same box, flow and hotspots on 96^3 for the full 200 steps (the 256^3 runs are below)
     c = inputs.hotspots(96, steps=200)
-    ref, _ = parity.run_oracle(oracle, c)
-    got, _ = parity.run_gpu(c)
-    floor = parity.noise_floor(oracle, c, ref)
-    errs = parity.assert_parity_noise(got, ref, floor, TOL64, label="config4@96")
-    print("config4@96", errs, "floor", floor)
-    for k, v in errs.items():
-        assert v[1] <= max(1e-12, 4 * floor[k][1]), (k, v, floor[k])
+    ref, o = parity.run_oracle(oracle, c)
+    got, s = parity.run_gpu(c)
+    _check_config(oracle, "config4 hotspots 96^3 (dx=0.267)", c, got, ref, s, o, steps=200, grid=[96, 96, 96])
 
 
 def test_config4_hotspots_crop_at_full_resolution(oracle):
     # the 256^3 state at its own dx = 0.1 fm on the 96^3 sub-box touching the +z face (gamma up to 12 at
     # the outflow boundary), 100 steps
     c = inputs.hotspots_crop(96, steps=100)
-    ref, _ = parity.run_oracle(oracle, c)
-    got, _ = parity.run_gpu(c)
-    floor = parity.noise_floor(oracle, c, ref)
-    errs = parity.assert_parity_noise(got, ref, floor, TOL64, label="config4 crop")
-    print("config4 crop", errs, "floor", floor)
+    ref, o = parity.run_oracle(oracle, c)
+    got, s = parity.run_gpu(c)
+    _check_config(oracle, "config4 crop 96^3 of 256^3 at +z face", c, got, ref, s, o, steps=100, grid=[96, 96, 96])
 
 
-def test_config4_hotspots_fp32(oracle):
-    # fp32 storage + transport, fp64 cons2prim ("fp32 bar").  north_star: err_L1 <= 1e-4 vs the fp64
-    # oracle.  That holds while the scheme's own amplification of rounding noise allows it: the fp64 noise floor of
-    # this config (strict vs FMA-contracted oracle) grows to ~1e-12 by step 200, and fp32 rounding is 2^29 times
-    # coarser, so any fp32 evaluation sits near floor64 * 2^29 ~ 5e-4 there.  Hard bar 1e-4 at 48 steps; at 200 steps
-    # the bar is max(1e-4, floor64_L1 * 2^29) per field.
-    c = inputs.hotspots(96, steps=48)
+FP32_STEPS = (12, 24, 48, 96, 200)
+
+
+def _fp32_study(oracle, name, c):
+    """f3: err_L1 of the fp32-storage path (fp32 transport, fp64 cons2prim) vs the fp64 oracle as the run proceeds."""
+    out = {}
+    for st in FP32_STEPS:
+        if st > c["steps"]:
+            break
+        ref, _ = parity.run_oracle(oracle, c, steps=st)
+        got, _ = parity.run_gpu(c, steps=st, precision=32)
+        rep = parity.field_report(got, ref)
+        parity.record(f"{name} fp32 {st} steps", rep, steps=st, precision=32, grid=[c["nx"], c["ny"], c["nz"]])
+        out[st] = {k: v["err_L1"] for k, v in rep.items()}
+    return out
+
+
+def test_config4_hotspots_fp32_48_steps(oracle):
+    # fp32 storage + transport, fp64 cons2prim.  north_star: err_L1 <= 1e-4 vs the fp64 oracle: holds through 48 steps
+    # (and through 96: recorded); the error grows with the step count exactly as the fp64 rounding noise does
+    l1 = _fp32_study(oracle, "config4 hotspots 96^3", inputs.hotspots(96, steps=48))
+    for st, d in l1.items():
+        for k, v in d.items():
+            assert v <= 1e-4, (st, k, v)
+
+
+@pytest.mark.xfail(strict=True, reason="north_star's fp32 bar (err_L1 <= 1e-4) at config 4's own 200 steps is NOT met: "
+                   "measured 2.8e-4 in E; the scheme amplifies one fp32 rounding (2^29 coarser than fp64) exactly as it "
+                   "amplifies fp64 rounding (floor64 x 2^29 ~ 5e-4 at 200 steps).  DESIGN.md 4, row a7: bar not met.")
+def test_config4_hotspots_fp32_200_steps_north_star_bar(oracle):
+    c = inputs.hotspots(96, steps=200)
     ref, _ = parity.run_oracle(oracle, c)
     got, _ = parity.run_gpu(c, precision=32)
-    errs = parity.field_errors(got, ref)
-    print("config4@96 fp32, 48 steps", errs)
-    for k, (emax, el1) in errs.items():
-        assert el1 <= 1e-4, (k, emax, el1)
+    rep = parity.field_report(got, ref)
+    parity.record("config4 hotspots 96^3 fp32 200 steps", rep, steps=200, precision=32, grid=[96, 96, 96])
+    for k, v in rep.items():
+        assert v["err_L1"] <= 1e-4, (k, v)
+
+
+def test_config4_hotspots_fp32_200_steps_stays_at_the_noise_scaled_level(oracle):
+    # what CAN be asserted at 200 steps: the fp32 path is no worse than fp64 rounding noise scaled by 2^29
     c = inputs.hotspots(96, steps=200)
     ref, _ = parity.run_oracle(oracle, c)
     got, _ = parity.run_gpu(c, precision=32)
     errs = parity.field_errors(got, ref)
     floor = parity.noise_floor(oracle, c, ref)
-    print("config4@96 fp32, 200 steps", errs, "floor64", floor)
     for k, (emax, el1) in errs.items():
         assert el1 <= max(1e-4, floor[k][1] * 2.0 ** 29), (k, emax, el1, floor[k])
 
 
+def test_config5_slabs_fp32_study(oracle):
+    # f3 at high gamma: the slab column (1x1x512 = config 5 by pin P11), fp32 transport vs the fp64 oracle
+    _fp32_study(oracle, "config5 slabs 1x1x512", inputs.slabs(512, steps=100, nxy=1))
+
+
+def test_config4_full_size_every_cell_24_steps(oracle):
+    # the metric's own configuration: 256^3, dx = 0.1 fm, in the launch configuration bench.py times, EVERY cell compared
+    # after 24 steps (four cycles of the six axis orders); the oracle runs on all host cores (~1 min on 16); fp32 too
+    c = inputs.hotspots(256, steps=24)
+    ref, o = parity.run_oracle(oracle, c)
+    got, s = parity.run_gpu(c)
+    _check_config(oracle, "config4 hotspots 256^3 (full size), 24 steps", c, got, ref, s, o, steps=24, grid=[256] * 3)
+    del got
+    got32, _ = parity.run_gpu(c, precision=32)
+    rep = parity.field_report(got32, ref)
+    parity.record("config4 hotspots 256^3 (full size) fp32 24 steps", rep, steps=24, precision=32, grid=[256] * 3)
+    for k, v in rep.items():
+        assert v["err_L1"] <= 1e-4, (k, v)
+
+
+@pytest.mark.slow
+def test_config4_full_size_every_cell_200_steps(oracle):
+    # config 4 exactly as BASELINE.json states it: 256^3 x 200 steps, every cell (oracle: ~7 min on 16 cores, twice
+    # for the noise floor).  Opt-in: SHASTA_SLOW=1 or -m "gpu and slow".
+    c = inputs.hotspots(256, steps=200)
+    ref, o = parity.run_oracle(oracle, c)
+    got, s = parity.run_gpu(c)
+    _check_config(oracle, "config4 hotspots 256^3 (full size), 200 steps", c, got, ref, s, o, steps=200, grid=[256] * 3)
+
+
 def test_config4_full_size_sampled(oracle):
     # 256^3 in the launch configuration bench.py times; the oracle recomputes sampled sub-boxes:
-    # after s steps a cell depends on +-12 s cells... per axis only +-4 s (one sweep per axis per step)
+    # after s steps a cell depends on +-4 s cells per axis (one sweep per axis per step)
     steps, w = 6, 16
     halo = 4 * steps
     c = inputs.hotspots(256, steps=steps)
