@@ -41,7 +41,8 @@
 #endif
 
 #define NF 5          /* E, Mx, My, Mz, R  (R is the paper's N, eq. (9)) */
-#define G  4          /* ghost depth of one sweep: dependency radius */
+#define G  4          /* ghost depth of one sweep: dependency radius of the default scheme (R1) */
+#define G2 6          /* same for the R2 predictor (half step WITH antidiffusion, reading G4 alternative) */
 #define PI_DELTA 1e-12            /* reading G7 */
 #define FP_TOL   1e-15            /* reading G9 */
 #define FP_MAXIT 200              /* reading G9 */
@@ -52,6 +53,8 @@ typedef struct oracle_shasta {
     int nx, ny, nz;
     double dx, lambda, gamma, mass;
     int bc;
+    int predictor;                /* 0 = R1 (reading G4): predictor = eq. (17) alone; 1 = R2: predictor = eqs. (17)-(22) */
+    double diff;                  /* Listing 1 'diff': factor on A^ph; 1 = paper default, 0 = "n/af" */
     long long step_index;
     int table[64];
     int ntable;
@@ -212,67 +215,92 @@ static int ghost_index(int j, int N, int bc)
 
 /* ---------------------------------------------------------- one pencil --- */
 /* One full sweep (phases 1-4) of one pencil along axis a (0=x,1=y,2=z).
-   U[f][0..N-1] is updated in place.  counts (may be NULL): [0] Pi fired, [1] vacuum. */
-void oracle_sweep_pencil(int N, double *U[NF], int a, double lambda, double gamma,
-                         double mass, int bc, unsigned long long counts[2])
+   U[f][0..N-1] is updated in place.  counts (may be NULL): [0] Pi fired, [1] vacuum.
+   Scheme variants the paper describes as selectable:
+     diff       factor on the antidiffusive flux A^ph ("fine controlled application of numerical viscosity",
+                PAPER.md:159; `const float diff = 1.0f`); diff = 0 is the "n/af" mode of Fig. 7
+                (no anti-flux);
+     predictor  0 = R1 (reading G4, the default): half step = eq. (17) alone with lambda/2;
+                1 = R2: half step = the complete kernel with lambda/2, i.e. eq. (17) AND eqs. (18)-(22), which is what
+                Listing 2 suggests (the ordinary prop kernels run after half_cfl).  Radius 6. */
+void oracle_sweep_pencil_ex(int N, double *U[NF], int a, double lambda, double gamma,
+                            double mass, int bc, unsigned long long counts[2], double diff, int predictor)
 {
-    const int NE = N + 2 * G;                 /* extended length, j = -G .. N+G-1 at offset +G */
-    double *buf = (double *)malloc(sizeof(double) * (size_t)NE * (4 * NF + 8));
-    double *Ue[NF], *Ut[NF], *Uh[NF], *Un[NF];
+    const int g = predictor ? G2 : G;         /* ghost depth */
+    const int NE = N + 2 * g;                 /* extended length, j = -g .. N+g-1 at offset +g */
+    double *buf = (double *)malloc(sizeof(double) * (size_t)NE * (5 * NF + 8));
+    double *Ue[NF], *Ut[NF], *Uh[NF], *Un[NF], *Up[NF];
     double *p = buf;
     for (int f = 0; f < NF; ++f) { Ue[f] = p; p += NE; }
     for (int f = 0; f < NF; ++f) { Ut[f] = p; p += NE; }
     for (int f = 0; f < NF; ++f) { Uh[f] = p; p += NE; }
     for (int f = 0; f < NF; ++f) { Un[f] = p; p += NE; }
+    for (int f = 0; f < NF; ++f) { Up[f] = p; p += NE; }
     double *v = p;  p += NE;  double *pr = p; p += NE;  double *pv = p; p += NE;
     double *eps = p; p += NE; double *vh = p; p += NE;  double *ph = p; p += NE;
     double *pvh = p; p += NE; double *epsh = p; p += NE;
+    /* index of cell j in the extended arrays is j + g; lo/hi below are extended indices.  The half-step state is
+       needed at j = -3 .. N+2, the corrector transport at j = -2 .. N+1 */
+    const int h_lo = g - 3, h_hi = g + N + 3;
 
-    /* 1. extend j = -4 .. N+3 */
+    /* 1. extend j = -g .. N+g-1 */
     for (int i = 0; i < NE; ++i) {
-        int src = ghost_index(i - G, N, bc);
+        int src = ghost_index(i - g, N, bc);
         for (int f = 0; f < NF; ++f) Ue[f][i] = U[f][src];
     }
-    /* 2. time-n primitives, j = -4 .. N+3 */
+    /* 2. time-n primitives on the whole extended pencil */
     for (int i = 0; i < NE; ++i) {
         double o[7];
         oracle_cons2prim(Ue[0][i], Ue[1][i], Ue[2][i], Ue[3][i], Ue[4][i], gamma, mass, o, NULL);
         v[i] = o[3 + a]; pr[i] = o[1]; pv[i] = o[1] * o[3 + a];
     }
-    /* 3. predictor (readings G4, G5): eq. (17) with lambda/2, time-n v and p, no antidiffusion;
-          j = -3 .. N+2 */
+    /* 3. predictor (readings G4, G5): eq. (17) with lambda/2, time-n v and p */
     const double h = 0.5 * lambda;
     for (int i = 0; i < NE; ++i) eps[i] = h * v[i];
     for (int f = 0; f < NF; ++f) {
         const double *src = (f == 0) ? pv : (f == 1 + a ? pr : NULL);
-        oracle_transport(NE, Ue[f], eps, src, h, Ut[f], 1, NE - 1);
+        if (!predictor) {
+            /* R1: no antidiffusion; j = -3 .. N+2 */
+            oracle_transport(NE, Ue[f], eps, src, h, Ut[f], h_lo, h_hi);
+        } else {
+            /* R2: transport j = -5 .. N+4, then eqs. (18)-(22) j = -3 .. N+2 */
+            oracle_transport(NE, Ue[f], eps, src, h, Up[f], h_lo - 2, h_hi + 2);
+            oracle_antidiffuse(NE, Ue[f], Up[f], diff, Ut[f], h_lo, h_hi);
+        }
     }
     /* 4. half-step primitives, j = -3 .. N+2 */
-    for (int i = 1; i < NE - 1; ++i) {
+    for (int i = h_lo; i < h_hi; ++i) {
         double o[7];
         oracle_cons2prim(Ut[0][i], Ut[1][i], Ut[2][i], Ut[3][i], Ut[4][i], gamma, mass, o, NULL);
         vh[i] = o[3 + a]; ph[i] = o[1]; pvh[i] = o[1] * o[3 + a];
     }
     /* 5. corrector transport: eq. (17) with lambda, half-step v and p, transports U^n;
           j = -2 .. N+1 */
-    for (int i = 1; i < NE - 1; ++i) epsh[i] = lambda * vh[i];
+    for (int i = h_lo; i < h_hi; ++i) epsh[i] = lambda * vh[i];
     for (int f = 0; f < NF; ++f) {
         const double *src = (f == 0) ? pvh : (f == 1 + a ? ph : NULL);
-        oracle_transport(NE, Ue[f], epsh, src, lambda, Uh[f], 2, NE - 2);
+        oracle_transport(NE, Ue[f], epsh, src, lambda, Uh[f], h_lo + 1, h_hi - 1);
     }
     /* 6.+7. antidiffusion, limiter, update: j = 0 .. N-1 */
     for (int f = 0; f < NF; ++f)
-        oracle_antidiffuse(NE, Ue[f], Uh[f], 1.0, Un[f], G, G + N);
+        oracle_antidiffuse(NE, Ue[f], Uh[f], diff, Un[f], g, g + N);
     /* 8. relativistic correction Pi written back (reading G8) */
     for (int j = 0; j < N; ++j) {
-        double M[3] = { Un[1][G + j], Un[2][G + j], Un[3][G + j] };
-        int r = oracle_project(Un[0][G + j], M);
+        double M[3] = { Un[1][g + j], Un[2][g + j], Un[3][g + j] };
+        int r = oracle_project(Un[0][g + j], M);
         if (counts) { if (r == 1) counts[0]++; else if (r == 2) counts[1]++; }
-        U[0][j] = Un[0][G + j];
+        U[0][j] = Un[0][g + j];
         U[1][j] = M[0]; U[2][j] = M[1]; U[3][j] = M[2];
-        U[4][j] = Un[4][G + j];
+        U[4][j] = Un[4][g + j];
     }
     free(buf);
+}
+
+/* the default scheme: diff = 1, predictor R1 */
+void oracle_sweep_pencil(int N, double *U[NF], int a, double lambda, double gamma,
+                         double mass, int bc, unsigned long long counts[2])
+{
+    oracle_sweep_pencil_ex(N, U, a, lambda, gamma, mass, bc, counts, 1.0, 0);
 }
 
 /* P5 pin helper: advect ONE source-free field with a PRESCRIBED velocity (cons2prim
@@ -305,7 +333,7 @@ oracle_t *oracle_create(int nx, int ny, int nz, double dx, double lambda, double
         !(eos_gamma > 1.0)) return NULL;
     oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
     o->nx = nx; o->ny = ny; o->nz = nz; o->dx = dx; o->lambda = lambda; o->gamma = eos_gamma;
-    o->mass = 0.0; o->bc = BC_OUTFLOW; o->step_index = 0;
+    o->mass = 0.0; o->bc = BC_OUTFLOW; o->step_index = 0; o->predictor = 0; o->diff = 1.0;
     memcpy(o->table, kBranch, sizeof(kBranch)); o->ntable = 18;
     size_t n = (size_t)nx * ny * nz;
     for (int f = 0; f < NF; ++f) o->U[f] = (double *)calloc(n, sizeof(double));
@@ -317,7 +345,7 @@ void oracle_destroy(oracle_t *o)
     for (int f = 0; f < NF; ++f) free(o->U[f]);
     free(o);
 }
-/* keys: 0 boundary (0 outflow, 1 periodic), 1 EOS mass m, 3 step index */
+/* keys: 0 boundary (0 outflow, 1 periodic), 1 EOS mass m, 3 step index, 4 predictor (0 = R1, 1 = R2), 5 diff >= 0 */
 int oracle_set_option(oracle_t *o, int key, double value)
 {
     if (!o) return -1;
@@ -325,6 +353,8 @@ int oracle_set_option(oracle_t *o, int key, double value)
     case 0: if (value != 0.0 && value != 1.0) return -1; o->bc = (int)value; return 0;
     case 1: if (value < 0.0) return -1; o->mass = value; return 0;
     case 3: if (value < 0.0) return -1; o->step_index = (long long)value; return 0;
+    case 4: if (value != 0.0 && value != 1.0) return -1; o->predictor = (int)value; return 0;
+    case 5: if (!(value >= 0.0)) return -1; o->diff = value; return 0;
     default: return -1;
     }
 }
@@ -389,7 +419,7 @@ static void sweep_grid(oracle_t *o, int a)
             for (int j = 0; j < N; ++j) P[f][j] = o->U[f][base + j * stride[a]];
         }
         unsigned long long cnt[2] = { 0, 0 };
-        oracle_sweep_pencil(N, P, a, o->lambda, o->gamma, o->mass, o->bc, cnt);
+        oracle_sweep_pencil_ex(N, P, a, o->lambda, o->gamma, o->mass, o->bc, cnt, o->diff, o->predictor);
         for (int f = 0; f < NF; ++f)
             for (int j = 0; j < N; ++j) o->U[f][base + j * stride[a]] = P[f][j];
         c0 += cnt[0]; c1 += cnt[1];

@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "shasta_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle_shasta.so")
 
-BOUNDARY, EOS_MASS, STEP_INDEX = 0, 1, 3
+BOUNDARY, EOS_MASS, STEP_INDEX, PREDICTOR, DIFF = 0, 1, 3, 4, 5
+R1, R2 = 0, 1
 OUTFLOW, PERIODIC = 0, 1
 BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 
@@ -75,6 +76,8 @@ def lib(variant: str = "strict"):
         L.oracle_project.argtypes = [C.c_double, _dp]
         L.oracle_sweep_pencil.argtypes = [C.c_int, C.POINTER(_dp), C.c_int, C.c_double, C.c_double,
                                           C.c_double, C.c_int, C.POINTER(C.c_ulonglong)]
+        L.oracle_sweep_pencil_ex.argtypes = [C.c_int, C.POINTER(_dp), C.c_int, C.c_double, C.c_double,
+                                             C.c_double, C.c_int, C.POINTER(C.c_ulonglong), C.c_double, C.c_int]
         L.oracle_advect_pencil.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_int, C.c_int, _dp]
         L.oracle_set_threads(_threads[0])
         _libs[variant] = L
@@ -152,13 +155,16 @@ def project(E, M):
     return m, r
 
 
-def sweep_pencil(U5, axis, lam, gamma, mass=0.0, bc=OUTFLOW):
+def sweep_pencil(U5, axis, lam, gamma, mass=0.0, bc=OUTFLOW, diff=1.0, predictor=R1):
     """U5: (5, N) array; returns the swept copy and the counts [Pi fired, vacuum]."""
     U5 = np.array(U5, dtype=np.float64, order="C")
     N = U5.shape[1]
     ptrs = (_dp * 5)(*[_p(U5[f]) for f in range(5)])
     cnt = (C.c_ulonglong * 2)(0, 0)
-    lib().oracle_sweep_pencil(N, ptrs, axis, lam, gamma, mass, bc, cnt)
+    if diff == 1.0 and predictor == R1:
+        lib().oracle_sweep_pencil(N, ptrs, axis, lam, gamma, mass, bc, cnt)
+    else:
+        lib().oracle_sweep_pencil_ex(N, ptrs, axis, lam, gamma, mass, bc, cnt, diff, predictor)
     return U5, (cnt[0], cnt[1])
 
 
@@ -175,7 +181,8 @@ def advect_pencil(U, vel, lam, bc, nsteps):
 class Oracle:
     """Same call sequence as the product's C ABI (include/shasta.h) with host arrays."""
 
-    def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, variant="strict"):
+    def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, variant="strict",
+                 predictor=R1, diff=1.0):
         self._L = lib(variant)
         self.shape = (nz, ny, nx)
         self._h = self._L.oracle_create(nx, ny, nz, dx, lam, eos_gamma)
@@ -183,6 +190,10 @@ class Oracle:
             raise ValueError("oracle_create: bad argument")
         self.set_option(BOUNDARY, boundary)
         self.set_option(EOS_MASS, eos_mass)
+        if predictor != R1:
+            self.set_option(PREDICTOR, predictor)
+        if diff != 1.0:
+            self.set_option(DIFF, diff)
 
     def __del__(self):
         if getattr(self, "_h", None):

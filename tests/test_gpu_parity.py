@@ -196,17 +196,19 @@ def test_conserved_totals_periodic(oracle):
 # ------------------------------------------------------------------ T2: the configs
 # Bars (north_star): fp64 err_max <= 1e-10 per field, err_L1 reported (expected <= 1e-12).  Configs 3 and 4
 # amplify rounding noise: two equally valid fp64 evaluations of the ORACLE (strict vs FMA-contracted build) already
-# differ by more than 1e-10 in some primitive fields there, so for those fields the bar is max(1e-10, 4 x that floor);
-# the CONSERVED fields are held to 1e-10 outright.  Every achieved number goes to gpurun_out/parity_r2.json.
-CONS_OUTRIGHT = 1e-10
+# differ by more than 1e-10 in some fields there (R and the primitives of config 4, p of config 3), so the bar is
+# max(1e-10, 2 x that floor): the GPU path is one more valid evaluation and must sit at the floor, not above it.
+# E and the momenta are held to 1e-10 outright.  Every achieved number goes to gpurun_out/parity_r2.json.
+OUTRIGHT = ("E", "Mx", "My", "Mz")
+FLOOR_FACTOR = 2.0
 
 
 def _check_config(oracle, name, c, got, ref, s=None, o=None, floor=True, l1=True, **meta):
     fl = parity.noise_floor(oracle, c, ref, steps=meta.get("steps")) if floor else None
     errs = parity.field_errors(got, ref)
-    bar = {k: (max(TOL64, 4.0 * fl[k][0]) if fl else TOL64) for k in errs}
-    for k in parity.CONS:
-        bar[k] = CONS_OUTRIGHT
+    bar = {k: (max(TOL64, FLOOR_FACTOR * fl[k][0]) if fl else TOL64) for k in errs}
+    for k in OUTRIGHT:
+        bar[k] = TOL64
     rep = parity.field_report(got, ref, fl, bar)
     if s is not None and o is not None:
         meta["pi_fired_gpu_oracle"] = [s.diagnostics()[0], o.diagnostics()[0]]
@@ -214,8 +216,8 @@ def _check_config(oracle, name, c, got, ref, s=None, o=None, floor=True, l1=True
     bad = {k: (v, bar[k]) for k, v in errs.items() if not v[0] <= bar[k]}
     assert not bad, f"{name}: (err_max, err_L1), bar: {bad}; all: {rep}"
     if l1:
-        badl = {k: v for k, v in errs.items() if not v[1] <= max(1e-12, 4.0 * (fl[k][1] if fl else 0.0))}
-        assert not badl, f"{name}: err_L1 above max(1e-12, 4 x floor): {badl}; all: {rep}"
+        badl = {k: v for k, v in errs.items() if not v[1] <= max(1e-12, FLOOR_FACTOR * (fl[k][1] if fl else 0.0))}
+        assert not badl, f"{name}: err_L1 above max(1e-12, 2 x floor): {badl}; all: {rep}"
     return rep
 
 
