@@ -44,6 +44,14 @@ typedef struct shasta shasta_t;   /* opaque */
 
 #define SHASTA_NO_TMA     6   /* test hook: 1 = the sweeps fill/drain their shared-memory tiles with cp.async + stores
                                  even where TMA is usable (16 B row strides); same bits either way; default 0 */
+#define SHASTA_PREDICTOR  7   /* scheme variant: 0 = R1 (default, reading G4): half step = eq. (17)
+                                 alone with lambda/2; 1 = R2: half step = the complete kernel with lambda/2, eq. (17)
+                                 and eqs. (18)-(22).  R2 runs the per-cell kernels (one thread per
+                                 cell, the paper's own decomposition), fp64 only                      */
+#define SHASTA_DIFF       8   /* factor on the antidiffusive flux A^ph of eq. (19) (Listing 1 `diff`);
+                                 1 = paper default, 0 = the "n/af" mode; 0 <= diff <= 8            */
+#define SHASTA_CELL_PATH  9   /* 1 = per-cell kernels for the default scheme too (A/B datapoint "the paper's design on
+                                 this GPU", tests); default 0 = fused sweep kernels                                    */
 
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only

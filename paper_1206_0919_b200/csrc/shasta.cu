@@ -27,6 +27,9 @@ struct shasta {
     int nx, ny, nz;
     long long ncell;
     double dx, lambda, gamma, mass;
+    double diff;            // factor on the antidiffusive flux; 1 by default
+    int cell_path;          // 1 = run the per-cell kernels also for the default scheme (A/B datapoint, tests)
+    int predictor;          // 0 = R1 (eq. (17) alone), 1 = R2 (complete kernel at lambda/2): per-cell kernels
     int periodic;
     int precision;          // 64 | 32
     int seg_override;
@@ -198,6 +201,7 @@ Consts<T> make_consts(const shasta_t* h)
     k.lam = (T)h->lambda;
     k.hlam = (T)(0.5 * h->lambda);
     k.qlam = (T)(0.25 * h->lambda);
+    k.aq = (T)(0.125 * h->diff);
     k.d.gam = h->gamma;
     k.d.gm1 = h->gamma - 1.0;
     k.d.g2 = h->gamma * h->gamma;
@@ -432,9 +436,43 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
     return 0;
 }
 
+// per-cell kernels (sweep_cell_kernel): the paper's own decomposition, used for the R2 predictor
+template <int EOS>
+int launch_cell_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
+{
+    const int n[3] = {h->nx, h->ny, h->nz};
+    const long long stride[3] = {1, h->nx, (long long)h->nx * h->ny};
+    const int perm[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};
+    SweepParams P;
+    memset(&P, 0, sizeof(P));
+    const int src = h->cur, dst = 1 - h->cur;
+    P.in[0] = h->U[src][0]; P.out[0] = h->U[dst][0];
+    for (int c = 0; c < 3; ++c) {
+        P.in[1 + c] = h->U[src][1 + perm[axis][c]];
+        P.out[1 + c] = h->U[dst][1 + perm[axis][c]];
+        P.prim[3 + c] = h->prim[3 + perm[axis][c]];
+    }
+    P.in[4] = h->U[src][4]; P.out[4] = h->U[dst][4];
+    P.prim[0] = h->prim[0]; P.prim[1] = h->prim[1]; P.prim[2] = h->prim[2];
+    P.nx = h->nx; P.N = n[axis]; P.stride_axis = stride[axis]; P.periodic = h->periodic; P.axis = axis;
+    P.counts = h->d_counts;
+    const Consts<double> k = make_consts<double>(h);
+    const unsigned blocks = (unsigned)((h->ncell + 127) / 128);
+    if (h->predictor) sweep_cell_kernel<EOS, true><<<blocks, 128, 0, st>>>(P, k, h->ncell, h->diff, emit ? 1 : 0);
+    else              sweep_cell_kernel<EOS, false><<<blocks, 128, 0, st>>>(P, k, h->ncell, h->diff, emit ? 1 : 0);
+    CK(cudaGetLastError());
+    h->launches++;
+    h->cur = dst;
+    return 0;
+}
+
 int launch_sweep_raw(shasta_t* h, int axis, bool emit, cudaStream_t st)
 {
     const bool general = use_general_eos(h);
+    if (h->predictor || h->cell_path) {
+        if (h->precision != 64) return fail(h, SHASTA_ESTATE, "the per-cell kernels (R2 predictor) run in fp64 only");
+        return general ? launch_cell_sweep<EOS_MASS>(h, axis, emit, st) : launch_cell_sweep<EOS_GAMMA>(h, axis, emit, st);
+    }
     if (h->precision == 64) {
         if (general) return emit ? launch_sweep_t<double, EOS_MASS, true>(h, axis, st)
                                  : launch_sweep_t<double, EOS_MASS, false>(h, axis, st);
@@ -473,7 +511,7 @@ int refresh_prims_t(shasta_t* h, cudaStream_t st)
 // conserved fields once (88 B/cell, ~0.3 ms).  y/z sweeps emit in place (+0.08 ms).
 int launch_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
 {
-    if (emit && axis == 0) {
+    if (emit && axis == 0 && !h->predictor && !h->cell_path) {
         int rc = launch_sweep_raw(h, axis, false, st);
         if (rc) return rc;
         return h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
@@ -526,6 +564,7 @@ int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lamb
     h->ncell = (long long)nx * ny * nz;
     h->dx = dx; h->lambda = lambda; h->gamma = eos_gamma; h->mass = 0.0;
     h->precision = 64;
+    h->diff = 1.0;
     memcpy(h->table, kBranch, sizeof(kBranch));
     h->ntable = 18;
     h->sm_count = prop.multiProcessorCount;
@@ -578,6 +617,18 @@ int shasta_set_option(shasta_t* h, int key, double value)
         return 0;
     case SHASTA_NO_TMA:
         h->no_tma = value != 0.0;
+        return 0;
+    case SHASTA_DIFF:
+        if (!(value >= 0.0) || value > 8.0) return fail(h, SHASTA_EINVAL, "SHASTA_DIFF must be in [0, 8]");
+        h->diff = value;
+        return 0;
+    case SHASTA_CELL_PATH:
+        h->cell_path = value != 0.0;
+        return 0;
+    case SHASTA_PREDICTOR:
+        if (value != 0.0 && value != 1.0) return fail(h, SHASTA_EINVAL, "SHASTA_PREDICTOR must be 0 (R1) or 1 (R2)");
+        if (value == 1.0 && h->precision != 64) return fail(h, SHASTA_EINVAL, "SHASTA_PREDICTOR 1 runs in fp64 only");
+        h->predictor = (int)value;
         return 0;
     case SHASTA_VARIANT:
         if (value != 0.0) return fail(h, SHASTA_EINVAL, "SHASTA_VARIANT: only 0 exists (the single-role kernels of round 1 were removed)");
@@ -807,6 +858,7 @@ long long shasta_step_index(const shasta_t* h) { return h ? h->step : -1; }
 const char* shasta_kernel_name(const shasta_t* h, int axis)
 {
     if (!h || axis < 0 || axis > 2) return "";
+    if (h->predictor || h->cell_path) return "sweep_cell_kernel";
     return axis == 0 ? "sweep_x2_kernel" : "sweep_yz_kernel";
 }
 

@@ -55,6 +55,7 @@ struct Consts {
     T lam;      // lambda = dt/dx
     T hlam;     // lambda/2 (predictor; corrector source factor)
     T qlam;     // lambda/4 (predictor source factor 1/2 * lambda/2)
+    T aq;       // diff / 8: outer factor of eq. (19) times the paper's `diff`; 1/8 by default
     EosD d;
 };
 
@@ -573,9 +574,11 @@ struct Consumer {
     T uh[2][NF];        // U^_3, U^_4                                         slot (PH-k)&1
     T dh[2][NF];        // D^_4, D^_5                                         slot (PH-k)&1
     T a5[NF];           // A_5
+    T aq;               // diff / 8
 
-    __device__ __forceinline__ void init()
+    __device__ __forceinline__ void init(T aq_)
     {
+        aq = aq_;
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
             dl[0][f] = dl[1][f] = dl[2][f] = dl[3][f] = fc[f] = T(0);
@@ -602,7 +605,7 @@ struct Consumer {
             fc[f] = fl;
             const T dh3 = uh2 - uh[H3][f];                                       // eq. (18)
             const T d2 = t_fma(T(-2), dl[D4][f], dl[D3][f] + dl[D5][f]);         // reading G14
-            const T aph = T(0.125) * t_fma(T(-0.125), d2, dh[E4][f]);            // eq. (19)
+            const T aph = aq * t_fma(T(-0.125), d2, dh[E4][f]);                  // eq. (19) (x diff: exact scaling, same bits as the oracle)
             const T a4 = limiter<T>(aph, dh3, dh[E5][f]);                        // eqs. (20),(21)
             un[f] = uh[H4][f] - (a4 - a5[f]);                                    // eq. (22)
             a5[f] = a4;
@@ -847,7 +850,7 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
         Cnt cnt;
         cnt.zero();
         Consumer<T> co;
-        co.init();
+        co.init(k.aq);
         // element offset of the output cell of the NEXT step: cell ilo - 4 (the first two groups store nothing)
         long long o = (long long)(x0 + lane) + (long long)oth * P.stride_other + (long long)(ilo - GH) * sa;
         int left = active ? (j1 - j0) : 0;      // output cells this lane still has to store
@@ -1039,7 +1042,7 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
         Cnt cnt;
         cnt.zero();
         Consumer<T> co;
-        co.init();
+        co.init(k.aq);
         int q0 = 0;                     // ring tile of group g
         bool store_pending = false;
 #pragma unroll 1
@@ -1136,6 +1139,147 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
         if (TMA && lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
         flush_counts(cnt, P.counts);
     }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// Per-cell path: one thread per cell and sweep, everything recomputed from a window of U^n -- the decomposition of the
+// paper's own kernels (one work-item per cell, U-hat recomputed for every neighbour, Listing 1).  It
+// exists for the scheme variants the fused kernels do not implement -- the R2 predictor (half step = the complete kernel
+// with lambda/2, eqs. (17)-(22); dependency radius 6) -- and as the A/B datapoint "the paper's design
+// on this GPU".  It follows the eight steps of DESIGN.md 1 literally on a (2W+1)-cell window; fp64 only.
+template <int W>
+struct CellWin {
+    double u[NF][2 * W + 1];        // U^n at j-W .. j+W (ghost-mapped, reading G11)
+    double v[2 * W + 1], p[2 * W + 1];
+};
+
+// eq. (17) for one field at window slot m: eps, U at m-1..m+1; src = f_{m+1} - f_{m-1} (0 for source-free fields)
+__device__ __forceinline__ double cell_transport(double um, double u0, double up, double em, double e0, double ep,
+                                                 double lam, double fm, double fp)
+{
+    const double Qp = (0.5 - e0) / (1.0 + (ep - e0));            // eq. (15), upper signs (G1)
+    const double Qm = (0.5 + e0) / (1.0 - (em - e0));            // lower signs
+    const double Dj = up - u0, Djm = u0 - um;                    // eq. (16)
+    double uh = 0.5 * Qp * Qp * Dj - 0.5 * Qm * Qm * Djm + (Qp + Qm) * u0;
+    uh += lam * (-0.5 * (fp - fm));                              // + lambda Delta(f)
+    return uh;
+}
+// eqs. (18)-(21): limited antidiffusive flux at interface (i, i+1); uh at i-1..i+2, u at i-1..i+2
+__device__ __forceinline__ double cell_antiflux(double hm, double h0, double h1, double h2, double um, double u0, double u1,
+                                                double u2, double diff)
+{
+    const double Dh = h1 - h0, Dhp = h2 - h1, Dhm = h0 - hm;     // eq. (18)
+    const double Di = u1 - u0, Dip = u2 - u1, Dim = u0 - um;
+    const double aph = diff * (0.125 * (Dh - 0.125 * ((Dip + Dim) - 2.0 * Di)));     // eq. (19), G14
+    const double sg = (aph > 0.0) - (aph < 0.0);                 // eq. (20)
+    double m = fmin(fmin(sg * Dhp, fabs(aph)), sg * Dhm);
+    return sg * fmax(m, 0.0);                                    // eq. (21)
+}
+
+template <int EOS, bool R2>
+__global__ void __launch_bounds__(128) sweep_cell_kernel(const __grid_constant__ SweepParams P,
+                                                         const __grid_constant__ Consts<double> k, long long ncell,
+                                                         double diff, int emit)
+{
+    constexpr int W = R2 ? 6 : GH;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ncell) return;
+    const long long sa = P.stride_axis;
+    const int N = P.N;
+    const int j = (int)((i / sa) % N);
+    CellWin<W> w;
+    // 1.+2. ghost-extended window and its time-n primitives
+#pragma unroll
+    for (int m = -W; m <= W; ++m) {
+        const long long o = i + (long long)(ghost_index(j + m, N, P.periodic) - j) * sa;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) w.u[f][m + W] = ((const double*)P.in[f])[o];
+        const Prim pr = cons2prim_general<EOS>(k.d, w.u[0][m + W], w.u[1][m + W], w.u[2][m + W], w.u[3][m + W], w.u[4][m + W]);
+        w.v[m + W] = w.u[1][m + W] * pr.y;
+        w.p[m + W] = pr.p;
+    }
+    const double lam = k.lam, h = k.hlam;
+    // 3. predictor at m = -3..3 (G4: R1 = eq. (17) alone; R2 = eq. (17) then eqs. (18)-(22)), 4. half-step primitives
+    double vh[7], ph[7];
+    double ut[NF][7];
+    if (!R2) {
+#pragma unroll
+        for (int m = -3; m <= 3; ++m) {
+            const int c = m + W;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                double fm = 0.0, fp = 0.0;
+                if (f == 0) { fm = w.p[c - 1] * w.v[c - 1]; fp = w.p[c + 1] * w.v[c + 1]; }
+                if (f == 1) { fm = w.p[c - 1]; fp = w.p[c + 1]; }
+                ut[f][m + 3] = cell_transport(w.u[f][c - 1], w.u[f][c], w.u[f][c + 1], h * w.v[c - 1], h * w.v[c], h * w.v[c + 1],
+                                              h, fm, fp);
+            }
+        }
+    } else {
+        double up[NF][11];          // transported half step at m = -5..5
+#pragma unroll
+        for (int m = -5; m <= 5; ++m) {
+            const int c = m + W;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                double fm = 0.0, fp = 0.0;
+                if (f == 0) { fm = w.p[c - 1] * w.v[c - 1]; fp = w.p[c + 1] * w.v[c + 1]; }
+                if (f == 1) { fm = w.p[c - 1]; fp = w.p[c + 1]; }
+                up[f][m + 5] = cell_transport(w.u[f][c - 1], w.u[f][c], w.u[f][c + 1], h * w.v[c - 1], h * w.v[c], h * w.v[c + 1],
+                                              h, fm, fp);
+            }
+        }
+#pragma unroll
+        for (int m = -3; m <= 3; ++m) {
+            const int c = m + W, q = m + 5;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                const double a1 = cell_antiflux(up[f][q - 1], up[f][q], up[f][q + 1], up[f][q + 2], w.u[f][c - 1], w.u[f][c],
+                                                w.u[f][c + 1], w.u[f][c + 2], diff);
+                const double a0 = cell_antiflux(up[f][q - 2], up[f][q - 1], up[f][q], up[f][q + 1], w.u[f][c - 2], w.u[f][c - 1],
+                                                w.u[f][c], w.u[f][c + 1], diff);
+                ut[f][m + 3] = up[f][q] - a1 + a0;                          // eq. (22)
+            }
+        }
+    }
+#pragma unroll
+    for (int m = 0; m < 7; ++m) {
+        const Prim pr = cons2prim_general<EOS>(k.d, ut[0][m], ut[1][m], ut[2][m], ut[3][m], ut[4][m]);
+        vh[m] = ut[1][m] * pr.y;
+        ph[m] = pr.p;
+    }
+    // 5. corrector transport of U^n at m = -2..2, 6.+7. antidiffusion, limiter, update of the centre cell
+    double un[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        double uh[5];
+#pragma unroll
+        for (int m = -2; m <= 2; ++m) {
+            const int c = m + W, q = m + 3;
+            double fm = 0.0, fp = 0.0;
+            if (f == 0) { fm = ph[q - 1] * vh[q - 1]; fp = ph[q + 1] * vh[q + 1]; }
+            if (f == 1) { fm = ph[q - 1]; fp = ph[q + 1]; }
+            uh[m + 2] = cell_transport(w.u[f][c - 1], w.u[f][c], w.u[f][c + 1], lam * vh[q - 1], lam * vh[q], lam * vh[q + 1],
+                                       lam, fm, fp);
+        }
+        const double a1 = cell_antiflux(uh[1], uh[2], uh[3], uh[4], w.u[f][W - 1], w.u[f][W], w.u[f][W + 1], w.u[f][W + 2], diff);
+        const double a0 = cell_antiflux(uh[0], uh[1], uh[2], uh[3], w.u[f][W - 2], w.u[f][W - 1], w.u[f][W], w.u[f][W + 1], diff);
+        un[f] = uh[2] - a1 + a0;                                            // eq. (22)
+    }
+    // 8. Pi written back (G8), primitives in the last sweep of a step
+    Cnt cnt;
+    cnt.zero();
+    project(k.d, un, cnt);
+#pragma unroll
+    for (int f = 0; f < NF; ++f) ((double*)P.out[f])[i] = un[f];
+    if (emit) {
+        double pr[6];
+        primitives<EOS>(k.d, un, pr, cnt);
+#pragma unroll
+        for (int q = 0; q < 6; ++q) ((double*)P.prim[q])[i] = pr[q];
+    }
+    flush_counts(cnt, P.counts);
 }
 
 }  // namespace shk

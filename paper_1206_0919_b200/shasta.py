@@ -12,7 +12,8 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libshasta.so")
 
-BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA = 0, 1, 2, 3, 4, 5, 6
+BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
+R1, R2 = 0, 1
 OUTFLOW, PERIODIC = 0, 1
 BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 
@@ -97,7 +98,7 @@ class Shasta:
     """One solver handle = shasta_create ... shasta_destroy.  Method names follow the C ABI."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, precision=64,
-                 segment=0, no_tma=0):
+                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0):
         L = load()
         self._L = L
         self._h = _vp()
@@ -115,6 +116,12 @@ class Shasta:
             self.set_option(SEGMENT, segment)
         if no_tma:
             self.set_option(NO_TMA, 1)
+        if predictor:
+            self.set_option(PREDICTOR, predictor)
+        if diff != 1.0:
+            self.set_option(DIFF, diff)
+        if cell_path:
+            self.set_option(CELL_PATH, 1)
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:

@@ -193,6 +193,54 @@ def test_conserved_totals_periodic(oracle):
     assert np.max(np.abs(t[1:4])) <= 1e-12 * abs(s0[0])
 
 
+# ------------------------------------------------------------------ f2: scheme variants (oracle pins: test_oracle_variants.py)
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("diff", [0.0, 0.5])
+def test_variant_diff_fused_kernels(oracle, bc, diff):
+    # `diff` and its diff = 0 case "n/af" run in the fused kernels: ragged shape
+    c = inputs.random_state(37, 19, 23, seed=21 + bc, kind="rough", boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=2, diff=diff)
+    got, _ = parity.run_gpu(c, steps=2, diff=diff)
+    assert_kernel_parity(got, ref, f"diff {diff} bc {bc}")
+    c = inputs.random_state(64, 33, 6, seed=22 + bc, kind="rough", boundary=bc)      # TMA-fed shapes
+    ref, _ = parity.run_oracle(oracle, c, steps=2, diff=diff)
+    got, _ = parity.run_gpu(c, steps=2, diff=diff)
+    assert_kernel_parity(got, ref, f"diff {diff} bc {bc} (tma)")
+
+
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("predictor,diff", [(1, 1.0), (1, 0.5), (0, 1.0)])
+def test_variant_predictor_per_cell_kernels(oracle, bc, predictor, diff):
+    # R2 predictor and, as a cross-check of the per-cell path itself, the default scheme through it
+    c = inputs.random_state(37, 19, 23, seed=31 + bc, kind="rough", boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=2, predictor=predictor, diff=diff)
+    got, s = parity.run_gpu(c, steps=2, predictor=predictor, diff=diff, cell_path=1)
+    assert s.kernel_name(0) == "sweep_cell_kernel"
+    assert_kernel_parity(got, ref, f"predictor {predictor} diff {diff} bc {bc}")
+    for shape in ((5, 1, 9), (2, 3, 4), (64, 1, 1)):
+        c = inputs.random_state(*shape, seed=7, kind="rough", boundary=bc)
+        ref, _ = parity.run_oracle(oracle, c, steps=3, predictor=predictor, diff=diff)
+        got, _ = parity.run_gpu(c, steps=3, predictor=predictor, diff=diff, cell_path=1)
+        assert_kernel_parity(got, ref, f"predictor {predictor} shape {shape}")
+
+
+@pytest.mark.parametrize("predictor,diff,cell", [(0, 0.0, 0), (0, 0.5, 0), (1, 1.0, 1), (0, 1.0, 1)])
+def test_variants_config1(oracle, predictor, diff, cell):
+    c = inputs.shock_tube(400, 0.01)
+    ref, o = parity.run_oracle(oracle, c, predictor=predictor, diff=diff)
+    got, s = parity.run_gpu(c, predictor=predictor, diff=diff, cell_path=cell)
+    rep = parity.field_report(got, ref)
+    parity.record(f"config1 eR=0.01 variant predictor={predictor} diff={diff} cell_path={cell}", rep, steps=c["steps"])
+    parity.assert_parity(got, ref, TOL64, label=f"config1 predictor {predictor} diff {diff}")
+
+
+def test_variant_general_eos_per_cell(oracle):
+    c = inputs.random_state(24, 20, 28, seed=4, kind="rough", gamma=5.0 / 3.0, mass=1.0, boundary=inputs.PERIODIC)
+    ref, _ = parity.run_oracle(oracle, c, steps=3, predictor=1)
+    got, _ = parity.run_gpu(c, steps=3, predictor=1)
+    assert_kernel_parity(got, ref, "general EOS R2", tol_cons=1e-11, tol_prim=1e-11)
+
+
 # ------------------------------------------------------------------ T2: the configs
 # Bars (north_star): fp64 err_max <= 1e-10 per field, err_L1 reported (expected <= 1e-12).  Configs 3 and 4
 # amplify rounding noise: two equally valid fp64 evaluations of the ORACLE (strict vs FMA-contracted build) already
