@@ -343,6 +343,45 @@ __device__ __forceinline__ void c2p_sweep(const Consts<T>& k, const T (&u)[NF], 
     p = (T)pd;
 }
 
+// In-sweep cons2prim of the FOUR cells of a hand-over group.  Gamma-law: the common case (no vacuum, causality clamp not
+// active) is the bare closed form, 19 fp64 operations per cell and no select; whether ANY lane of the warp holds a
+// vacuum or clamped cell is decided by one vote per group, and only then is the cell redone by c2p_sweep_d (the
+// select form above, identical bits for ordinary cells).  The branch-free select form for every cell (round 2, first
+// version) paid the direction-preserving scale factor (8 fp64 operations) and 8 selects per cons2prim for the ~0.2 %
+// of the cells that need them; one warp-uniform branch per four cells keeps the four chains in one basic block.
+template <typename T, int EOS, typename RL>
+__device__ __forceinline__ void c2p_group(const Consts<T>& k, T (&c0)[NF], T (&c1)[NF], T (&c2)[NF], T (&c3)[NF],
+                                          T (&v)[4], T (&p)[4], const RL& reload)
+{
+    if constexpr (EOS == EOS_GAMMA) {
+        bool rare[4];
+#define SHK_C2P_FAST(J, C)                                                                      \
+        {                                                                                       \
+            const double E = (double)C[0], M1 = (double)C[1];                                   \
+            const double M2 = fma(M1, M1, fma((double)C[2], (double)C[2], (double)C[3] * (double)C[3])); \
+            const double t = E * E;                                                             \
+            rare[J] = gt_nonneg(M2, k.d.omd2 * t) | c2p_is_vacuum(E);                           \
+            const double y = c2p_fast_y(k.d, E, M2, t);                                         \
+            v[J] = (T)(M1 * y);                                                                 \
+            p[J] = (T)(k.d.gm1 * fma(-M2, y, E));                                               \
+        }
+        SHK_C2P_FAST(0, c0) SHK_C2P_FAST(1, c1) SHK_C2P_FAST(2, c2) SHK_C2P_FAST(3, c3)
+#undef SHK_C2P_FAST
+        if (__any_sync(0xffffffffu, rare[0] | rare[1] | rare[2] | rare[3])) {
+            reload();                       // the cells again (from shared memory: not held in registers for this)
+            if (__any_sync(0xffffffffu, rare[0])) c2p_sweep<T, EOS>(k, c0, v[0], p[0]);
+            if (__any_sync(0xffffffffu, rare[1])) c2p_sweep<T, EOS>(k, c1, v[1], p[1]);
+            if (__any_sync(0xffffffffu, rare[2])) c2p_sweep<T, EOS>(k, c2, v[2], p[2]);
+            if (__any_sync(0xffffffffu, rare[3])) c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
+        }
+    } else {
+        c2p_sweep<T, EOS>(k, c0, v[0], p[0]);
+        c2p_sweep<T, EOS>(k, c1, v[1], p[1]);
+        c2p_sweep<T, EOS>(k, c2, v[2], p[2]);
+        c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
+    }
+}
+
 // eq. (21) branch-free (reading G12): A = sigma max(0, min(sigma D^_{j+1}, |A^ph|, sigma D^_{j-1}))
 template <typename T>
 __device__ __forceinline__ T limiter(T aph, T dhp, T dhm)
@@ -507,6 +546,24 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // dependent chain is half as long.  P -> C traffic per pencil and step is four doubles through a
 // shared-memory queue: a_c = 1/2 - Q+, b_c = Q+^2/2 of the interface (i-2,i-1) at n+1/2, and the two
 // source increments -lambda Delta(p v)/2-form for E and M_par of cell i-2.
+// two adjacent elements with one shared-memory access (LDS.128 for fp64); p is 2-element aligned
+__device__ __forceinline__ void load2(const double* p, double& a, double& b)
+{
+    const double2 v = *reinterpret_cast<const double2*>(p);
+    a = v.x; b = v.y;
+}
+__device__ __forceinline__ void load2(const float* p, float& a, float& b)
+{
+    const float2 v = *reinterpret_cast<const float2*>(p);
+    a = v.x; b = v.y;
+}
+
+__device__ __forceinline__ void store2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
+__device__ __forceinline__ void store2(float* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
+
+// keeps shared-memory loads below this point (registers: a pair of cells is 20 registers)
+__device__ __forceinline__ void load_fence() { asm volatile("" ::: "memory"); }
+
 template <typename T, int EOS>
 struct Producer {
     // fields the producer needs: the Gamma-law pressure does not depend on R, so R's predictor is skipped there
@@ -565,6 +622,93 @@ struct Producer {
         eps1 = eps0; fE[S2] = fE0; fM[S2] = p0;
         epsh2 = epsh1; gE[G3] = gE1; gM[G3] = ph;
     }
+
+    // One hand-over group = four march steps with front cells c1..c4 (c0 = the cell before them), arranged in PHASES:
+    // S1 of the four cells, S2 of the four cells, S3 of the four cells, geometry -- the same arithmetic as four step<PH>()
+    // calls (identical bits), but each cons2prim phase is four INDEPENDENT chains behind one rare-path vote (c2p_group).
+    // State slots here: fE[0]/fM[0] = cell -2, [1] = cell -1 (time n); gE/gM likewise for half-step cells -3, -2.
+    // `ld` reads cells of the group from the shared-memory ring: ld.first(c0, c1, c2) the cell before the group and its
+    // first two cells, ld.second(c3, c4) the last two.  It is called again in every phase that needs U^n (behind a
+    // compiler fence), so that U^n is not held in registers across the cons2prim phases (96 registers per thread).
+    // `scr` is this lane's slice of the message buffer of the group (16 elements, stride as written by the caller): it
+    // holds U~ of the four cells while S3 runs, so that the rare path of S3 can read them back instead of keeping 16
+    // values alive in registers.
+    template <typename L>
+    __device__ __forceinline__ void group(const Consts<T>& k, const L& ld, T* scr, T (&msg)[4][4])
+    {
+        if constexpr (EOS != EOS_GAMMA) {
+            T c0[NF], c1[NF], c2[NF], c3[NF], c4[NF];
+            ld.first(c0, c1, c2);
+            ld.second(c3, c4);
+            step<0>(k, c0, c1, msg[0]);
+            step<1>(k, c1, c2, msg[1]);
+            step<2>(k, c2, c3, msg[2]);
+            step<3>(k, c3, c4, msg[3]);
+        } else {
+            T v[4], p[4];
+            {
+                T c0[NF], c1[NF], c2[NF], c3[NF], c4[NF];
+                ld.first(c0, c1, c2);
+                ld.second(c3, c4);
+                c2p_group<T, EOS>(k, c1, c2, c3, c4, v, p, [&]() { load_fence(); ld.first(c0, c1, c2); ld.second(c3, c4); });    // S1
+            }
+            T eps[5], pv[6], pp[6];
+            eps[0] = eps1; pv[0] = fE[0]; pv[1] = fE[1]; pp[0] = fM[0]; pp[1] = fM[1];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { eps[j + 1] = k.hlam * v[j]; pv[j + 2] = p[j] * v[j]; pp[j + 2] = p[j]; }
+            T ut[4][NF];
+#define SHK_PRED(J, UL, UR)                                                                     \
+            {                                                                                   \
+                const T q = (T(0.5) - eps[J]) * fast_rcp(T(1) + (eps[J + 1] - eps[J]));         \
+                const T a = T(0.5) - q, b = (T(0.5) * q) * q;                                   \
+                _Pragma("unroll") for (int f = 0; f < NP; ++f) {                                \
+                    const T d = UR[f] - UL[f];                                                  \
+                    const T fl = t_fma(a, UL[f], -(b * d));                                     \
+                    ut[J][f] = UL[f] - (fl - ft[f]);                                            \
+                    ft[f] = fl;                                                                 \
+                }                                                                               \
+                ut[J][NF - 1] = T(0);                                                           \
+                ut[J][0] = t_fma(-k.qlam, pv[J + 2] - pv[J], ut[J][0]);                         \
+                ut[J][1] = t_fma(-k.qlam, pp[J + 2] - pp[J], ut[J][1]);                         \
+                store2(scr + 128 * J, ut[J][0], ut[J][1]);                                      \
+                store2(scr + 128 * J + 64, ut[J][2], ut[J][3]);                                 \
+            }
+            {                                                                                   // S2
+                T c0[NF], c1[NF], c2[NF], c3[NF], c4[NF];
+                load_fence();
+                ld.first(c0, c1, c2);
+                SHK_PRED(0, c0, c1) SHK_PRED(1, c1, c2)
+                load_fence();
+                ld.second(c3, c4);
+                SHK_PRED(2, c2, c3) SHK_PRED(3, c3, c4)
+            }
+#undef SHK_PRED
+            eps1 = eps[4]; fE[0] = pv[4]; fE[1] = pv[5]; fM[0] = pp[4]; fM[1] = pp[5];
+            T vh[4], ph[4];
+            c2p_group<T, EOS>(k, ut[0], ut[1], ut[2], ut[3], vh, ph, [&]() {           // S3
+                load_fence();
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    load2(scr + 128 * j, ut[j][0], ut[j][1]);
+                    load2(scr + 128 * j + 64, ut[j][2], ut[j][3]);
+                    ut[j][NF - 1] = T(0);
+                }
+            });
+            T eh[5], gv[6], gp[6];
+            eh[0] = epsh2; gv[0] = gE[0]; gv[1] = gE[1]; gp[0] = gM[0]; gp[1] = gM[1];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { eh[j + 1] = k.lam * vh[j]; gv[j + 2] = ph[j] * vh[j]; gp[j + 2] = ph[j]; }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {                                       // geometry + sources of S4
+                const T q = (T(0.5) - eh[j]) * fast_rcp(T(1) + (eh[j + 1] - eh[j]));
+                msg[j][0] = T(0.5) - q;
+                msg[j][1] = (T(0.5) * q) * q;
+                msg[j][2] = -k.hlam * (gv[j + 2] - gv[j]);
+                msg[j][3] = -k.hlam * (gp[j + 2] - gp[j]);
+            }
+            epsh2 = eh[4]; gE[0] = gv[4]; gE[1] = gv[5]; gM[0] = gp[4]; gM[1] = gp[5];
+        }
+    }
 };
 
 template <typename T>
@@ -614,21 +758,6 @@ struct Consumer {
         }
     }
 };
-
-// two adjacent elements with one shared-memory access (LDS.128 for fp64); p is 2-element aligned
-__device__ __forceinline__ void load2(const double* p, double& a, double& b)
-{
-    const double2 v = *reinterpret_cast<const double2*>(p);
-    a = v.x; b = v.y;
-}
-__device__ __forceinline__ void load2(const float* p, float& a, float& b)
-{
-    const float2 v = *reinterpret_cast<const float2*>(p);
-    a = v.x; b = v.y;
-}
-
-__device__ __forceinline__ void store2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
-__device__ __forceinline__ void store2(float* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
 
 // Producer/consumer hand-over of one warp pair: named barriers of 64 threads each, 32 that arrive (do not wait) and 32
 // that sync (wait): the PTX producer/consumer pattern.
@@ -694,6 +823,11 @@ constexpr int YZ_CH = 4;          // cells per group = steps per hand-over chunk
 #endif
 constexpr int YZ_PREG = SHK_YZ_PREG;          // registers per producer thread (setmaxnreg); consumer gets 256 - YZ_PREG
 constexpr int YZ_CREG = 256 - YZ_PREG;
+#ifndef SHK_X_PREG
+#define SHK_X_PREG 96
+#endif
+constexpr int X_PREG = SHK_X_PREG;            // x sweep: its consumer (staging tile addresses) needs the full 160
+constexpr int X_CREG = 256 - X_PREG;
 
 template <typename T>
 struct alignas(128) YzPair {      // TMA destinations need 128 B alignment
@@ -717,8 +851,6 @@ struct YzMaps {
 };
 
 // one lane of a converged warp: ptxas then knows the region is single-threaded and issues UTMALDG without an ELECT loop
-// keeps shared-memory loads below this point (registers: a pair of cells is 20 registers)
-__device__ __forceinline__ void load_fence() { asm volatile("" ::: "memory"); }
 __device__ __forceinline__ bool elect_one()
 {
     unsigned pred;
@@ -822,25 +954,33 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
             }
             const T* tp = &S.ring[(g + YZ_G - 1) & (YZ_G - 1)][0][YZ_CH - 1][lane];     // last cell of the previous group
             const T* tc = &S.ring[g & (YZ_G - 1)][0][0][lane];
-            T um[NF], c0[NF], c1[NF], c2[NF], c3[NF], m0[4], m1[4], m2[4], m3[4];
-            um[NF - 1] = c0[NF - 1] = c1[NF - 1] = c2[NF - 1] = c3[NF - 1] = T(0);
+            T mm[4][4];
+            struct {
+                const T *tp, *tc;
+                __device__ __forceinline__ void first(T (&um)[NF], T (&c0)[NF], T (&c1)[NF]) const
+                {
+                    um[NF - 1] = c0[NF - 1] = c1[NF - 1] = T(0);
 #pragma unroll
-            for (int f = 0; f < NP; ++f) {
-                um[f] = tp[f * YZ_CH * 32];
-                c0[f] = tc[f * YZ_CH * 32];
-                c1[f] = tc[f * YZ_CH * 32 + 32];
-                c2[f] = tc[f * YZ_CH * 32 + 64];
-                c3[f] = tc[f * YZ_CH * 32 + 96];
-            }
+                    for (int f = 0; f < NP; ++f) {
+                        um[f] = tp[f * YZ_CH * 32];
+                        c0[f] = tc[f * YZ_CH * 32];
+                        c1[f] = tc[f * YZ_CH * 32 + 32];
+                    }
+                }
+                __device__ __forceinline__ void second(T (&c2)[NF], T (&c3)[NF]) const
+                {
+                    c2[NF - 1] = c3[NF - 1] = T(0);
+#pragma unroll
+                    for (int f = 0; f < NP; ++f) {
+                        c2[f] = tc[f * YZ_CH * 32 + 64];
+                        c3[f] = tc[f * YZ_CH * 32 + 96];
+                    }
+                }
+            } ld = {tp, tc};
             T* mq = &S.msg[g & 1][0][0][lane][0];
-            pr.template step<0>(k, um, c0, m0);
-            store2(mq, m0[0], m0[1]);           store2(mq + 64, m0[2], m0[3]);
-            pr.template step<1>(k, c0, c1, m1);
-            store2(mq + 128, m1[0], m1[1]);     store2(mq + 192, m1[2], m1[3]);
-            pr.template step<2>(k, c1, c2, m2);
-            store2(mq + 256, m2[0], m2[1]);     store2(mq + 320, m2[2], m2[3]);
-            pr.template step<3>(k, c2, c3, m3);
-            store2(mq + 384, m3[0], m3[1]);     store2(mq + 448, m3[2], m3[3]);
+            pr.group(k, ld, mq, mm);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { store2(mq + 128 * j, mm[j][0], mm[j][1]); store2(mq + 128 * j + 64, mm[j][2], mm[j][3]); }
             bar_arrive64(bar_id + (g & 1));
         }
         if (!TMA) cp_async_wait<0>();
@@ -954,7 +1094,7 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
     const int sw = (lane >> 2) & 1;                         // 32 B swizzle of this lane's row
 
     if (producer) {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(YZ_PREG));
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(X_PREG));
         if (idle) return;
         Producer<T, EOS> pr;
         pr.init();
@@ -1014,30 +1154,35 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
             const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;           // tile of group g-1
             const T* tp = &S.ring[qm][0][xv_off(lane, 3)];
             const T* tc = &S.ring[q0][0][lane * 4];
-            T um[NF], c0[NF], c1[NF], c2[NF], c3[NF], m0[4], m1[4], m2[4], m3[4];
-            um[NF - 1] = c0[NF - 1] = c1[NF - 1] = c2[NF - 1] = c3[NF - 1] = T(0);
+            T mm[4][4];
+            struct {
+                const T *tp, *tc;
+                int sw;
+                __device__ __forceinline__ void first(T (&um)[NF], T (&c0)[NF], T (&c1)[NF]) const
+                {
+                    um[NF - 1] = c0[NF - 1] = c1[NF - 1] = T(0);
 #pragma unroll
-            for (int f = 0; f < NP; ++f) {
-                um[f] = tp[f * XV_TILE];
-                load2(tc + f * XV_TILE + 2 * sw, c0[f], c1[f]);
-            }
+                    for (int f = 0; f < NP; ++f) {
+                        um[f] = tp[f * XV_TILE];
+                        load2(tc + f * XV_TILE + 2 * sw, c0[f], c1[f]);
+                    }
+                }
+                __device__ __forceinline__ void second(T (&c2)[NF], T (&c3)[NF]) const
+                {
+                    c2[NF - 1] = c3[NF - 1] = T(0);
+#pragma unroll
+                    for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (1 ^ sw), c2[f], c3[f]);
+                }
+            } ld = {tp, tc, sw};
             T* mq = &S.msg[g & 1][0][0][lane][0];
-            pr.template step<0>(k, um, c0, m0);
-            store2(mq, m0[0], m0[1]);           store2(mq + 64, m0[2], m0[3]);
-            load_fence();
+            pr.group(k, ld, mq, mm);
 #pragma unroll
-            for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (1 ^ sw), c2[f], c3[f]);
-            pr.template step<1>(k, c0, c1, m1);
-            store2(mq + 128, m1[0], m1[1]);     store2(mq + 192, m1[2], m1[3]);
-            pr.template step<2>(k, c1, c2, m2);
-            store2(mq + 256, m2[0], m2[1]);     store2(mq + 320, m2[2], m2[3]);
-            pr.template step<3>(k, c2, c3, m3);
-            store2(mq + 384, m3[0], m3[1]);     store2(mq + 448, m3[2], m3[3]);
+            for (int j = 0; j < 4; ++j) { store2(mq + 128 * j, mm[j][0], mm[j][1]); store2(mq + 128 * j + 64, mm[j][2], mm[j][3]); }
             bar_arrive64(bar_id + (g & 1));
         }
         cp_async_wait<0>();
     } else {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(YZ_CREG));
+        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(X_CREG));
         if (idle) return;
         Cnt cnt;
         cnt.zero();
