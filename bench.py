@@ -242,26 +242,41 @@ def ours(args):
 
     # ---- region B: the same K steps sweep by sweep, CUDA events around every kernel launch
     from paper_1206_0919_b200.shasta import BRANCH as table
+    # The sweeps are issued exactly as shasta_step issues them: a step whose last sweep runs along x leaves its primitives
+    # to the first sweep of the next step (emit_primitives = 2); only when no such sweep follows inside the region does
+    # the x sweep write them at once (x kernel + element-wise cons2prim_kernel, timed as one entry).
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(3 * K + 1)]
     kinds = []
     base = s.step_index
     barrier()
     w0 = time.perf_counter()
     evs[0].record(stream)
+    deferred = False
     for i in range(K):
         for k in range(3):
             a = table[(3 * (base + i) + k) % len(table)]
-            s.sweep(a, emit_primitives=(k == 2))
+            emit, label, nbytes = (1 if k == 2 else 0), "", B_SWEEP
+            if deferred:
+                deferred, emit, label, nbytes = False, 2, "<emit_in>", B_SWEEP + B_PRIM
+            elif k == 2 and a == 0:
+                nxt = table[(3 * (base + i + 1)) % len(table)]
+                if i + 1 < K and nxt != 0:
+                    deferred, emit = True, 0
+                else:
+                    label, nbytes = "+cons2prim_kernel", 2 * B_SWEEP + B_PRIM - 40.0     # 80 + (40 read + 48 written)
+            elif k == 2:
+                label, nbytes = "<emit>", B_SWEEP + B_PRIM
+            s.sweep(a, emit_primitives=emit)
             evs[3 * i + k + 1].record(stream)
-            kinds.append((s.kernel_name(a) + ("<emit>" if k == 2 else ""), k == 2))
+            kinds.append((s.kernel_name(a) + label, nbytes))
     barrier()
     sampler.windows.append((w0, time.perf_counter()))
     per = {}
-    for j, (name, emit) in enumerate(kinds):
+    for j, (name, nbytes) in enumerate(kinds):
         d = per.setdefault(name, {"ms": 0.0, "launches": 0, "bytes": 0.0})
         d["ms"] += evs[j].elapsed_time(evs[j + 1])
         d["launches"] += 1
-        d["bytes"] += ncell * (B_SWEEP + (B_PRIM if emit else 0.0)) * (args.precision / 64.0)
+        d["bytes"] += ncell * nbytes * (args.precision / 64.0)
     ms_sweeps = sum(d["ms"] for d in per.values())
     dom_name = max(per, key=lambda k: per[k]["ms"])
     dom = per[dom_name]

@@ -53,6 +53,13 @@ typedef struct shasta shasta_t;   /* opaque */
 #define SHASTA_CELL_PATH  9   /* 1 = per-cell kernels for the default scheme too (A/B datapoint "the paper's design on
                                  this GPU", tests); default 0 = fused sweep kernels                                    */
 
+#define SHASTA_NO_DEFER  10   /* test hook / A-B: 1 = a step whose last sweep runs along x writes its primitives at once with
+                                 the element-wise pass; default 0 = shasta_step lets the first sweep of the next step write
+                                 them (same values, one pass over the conserved fields less)            */
+
+#define SHASTA_PRIMS_RAW 11   /* test hook: 1 = shasta_get_primitives[_host] copies the primitive fields as they are stored,
+                                 without recomputing them when they are stale (reads back what emit_primitives = 2 wrote) */
+
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only
  * (eqs. (15)-(17)); dx enters shasta_conserved_totals.  0 < lambda <= 0.5
@@ -100,9 +107,11 @@ int shasta_get_conserved(shasta_t* h, double* E_dev, double* Mx_dev, double* My_
 int shasta_step(shasta_t* h, int nsteps, void* stream);
 
 /* One sweep ("round") along `axis` (0=x,1=y,2=z) by the full dt: the fused kernel of
- * shasta_step, launched once.  emit_primitives != 0 also writes the primitive fields of the new state (as
- * the last sweep of a step does).  Does not advance the step counter.  An axis of extent 1 is a no-op
- * (reading G15).  Used by tests (single-axis parity) and by bench.py to time each kernel with CUDA events. */
+ * shasta_step, launched once.  emit_primitives: 0 = conserved fields only; 1 = also write the primitive fields of
+ * the new state (as the last sweep of a step does); 2 = also write the primitive fields of the state BEFORE this
+ * sweep (y and z only, SHASTA_EINVAL otherwise): what shasta_step uses after a step that ended with an x sweep.
+ * Does not advance the step counter.  An axis of extent 1 is a no-op (reading G15).  Used by tests (single-axis
+ * parity) and by bench.py to time each kernel with CUDA events. */
 int shasta_sweep(shasta_t* h, int axis, int emit_primitives, void* stream);
 
 /* Primitive fields of the current state (phases 3-4): e = E - |M| v,

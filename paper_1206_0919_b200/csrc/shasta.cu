@@ -34,6 +34,8 @@ struct shasta {
     int precision;          // 64 | 32
     int seg_override;
     int no_tma;             // test hook: 1 = x sweep through cp.async even where TMA is possible
+    int prims_raw;          // test hook: get_primitives copies the primitive fields as stored, without refreshing them
+    int no_defer;           // test hook / A-B: 1 = x-last steps write their primitives at once (separate element-wise pass)
     long long step;
     int table[64];
     int ntable;
@@ -347,7 +349,7 @@ int auto_segment(const shasta_t* h, int axis, int N, long long base)
     return (int)(seg < N ? seg : N);
 }
 
-template <typename T, int EOS, bool EMIT>
+template <typename T, int EOS, int EMIT>
 int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
 {
     const int n[3] = {h->nx, h->ny, h->nz};
@@ -386,12 +388,12 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
             const size_t smem = sizeof(X2Smem<T>);
             dim3 grid((unsigned)((P.npencil + 127) / 128), (unsigned)P.nseg);
             if (tma) {
-                auto kern = sweep_x2_kernel<T, EOS, EMIT, true>;
+                auto kern = sweep_x2_kernel<T, EOS, EMIT == 1, true>;
                 int rc = opt_in_smem(h, (const void*)kern, smem);
                 if (rc) return rc;
                 kern<<<grid, 256, smem, st>>>(P, k, maps);
             } else {
-                auto kern = sweep_x2_kernel<T, EOS, EMIT, false>;
+                auto kern = sweep_x2_kernel<T, EOS, EMIT == 1, false>;
                 int rc = opt_in_smem(h, (const void*)kern, smem);
                 if (rc) return rc;
                 kern<<<grid, 256, smem, st>>>(P, k, maps);
@@ -466,23 +468,24 @@ int launch_cell_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
     return 0;
 }
 
-int launch_sweep_raw(shasta_t* h, int axis, bool emit, cudaStream_t st)
+// emit: 0 none, 1 primitives of the new state, 2 primitives of the state the sweep reads (y/z fused kernels only)
+template <typename T, int EOS>
+int launch_sweep_e(shasta_t* h, int axis, int emit, cudaStream_t st)
+{
+    if (emit == 2 && axis != 0) return launch_sweep_t<T, EOS, 2>(h, axis, st);
+    return emit ? launch_sweep_t<T, EOS, 1>(h, axis, st) : launch_sweep_t<T, EOS, 0>(h, axis, st);
+}
+
+int launch_sweep_raw(shasta_t* h, int axis, int emit, cudaStream_t st)
 {
     const bool general = use_general_eos(h);
     if (h->predictor || h->cell_path) {
         if (h->precision != 64) return fail(h, SHASTA_ESTATE, "the per-cell kernels (R2 predictor) run in fp64 only");
-        return general ? launch_cell_sweep<EOS_MASS>(h, axis, emit, st) : launch_cell_sweep<EOS_GAMMA>(h, axis, emit, st);
+        return general ? launch_cell_sweep<EOS_MASS>(h, axis, emit != 0, st) : launch_cell_sweep<EOS_GAMMA>(h, axis, emit != 0, st);
     }
-    if (h->precision == 64) {
-        if (general) return emit ? launch_sweep_t<double, EOS_MASS, true>(h, axis, st)
-                                 : launch_sweep_t<double, EOS_MASS, false>(h, axis, st);
-        return emit ? launch_sweep_t<double, EOS_GAMMA, true>(h, axis, st)
-                    : launch_sweep_t<double, EOS_GAMMA, false>(h, axis, st);
-    }
-    if (general) return emit ? launch_sweep_t<float, EOS_MASS, true>(h, axis, st)
-                             : launch_sweep_t<float, EOS_MASS, false>(h, axis, st);
-    return emit ? launch_sweep_t<float, EOS_GAMMA, true>(h, axis, st)
-                : launch_sweep_t<float, EOS_GAMMA, false>(h, axis, st);
+    if (h->precision == 64)
+        return general ? launch_sweep_e<double, EOS_MASS>(h, axis, emit, st) : launch_sweep_e<double, EOS_GAMMA>(h, axis, emit, st);
+    return general ? launch_sweep_e<float, EOS_MASS>(h, axis, emit, st) : launch_sweep_e<float, EOS_GAMMA>(h, axis, emit, st);
 }
 
 template <typename T>
@@ -505,14 +508,19 @@ int refresh_prims_t(shasta_t* h, cudaStream_t st)
     return 0;
 }
 
-// One sweep.  When the LAST sweep of a step runs along x, its primitives are written by the element-wise
-// cons2prim kernel instead of the sweep's write-back: in the warp-specialised x kernel the consumer warp is the
-// critical one, and computing six more fields there costs more (+0.5 ms at 256^3) than re-reading the five
-// conserved fields once (88 B/cell, ~0.3 ms).  y/z sweeps emit in place (+0.08 ms).
-int launch_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
+bool fused_path(const shasta_t* h) { return !h->predictor && !h->cell_path; }
+
+// One sweep.  emit: 0 none, 1 primitives of the new state, 2 primitives of the state BEFORE the sweep (fused y/z kernels).
+// When a sweep along x has to emit (the last sweep of a step), the primitives are written by the element-wise cons2prim
+// kernel after it: in the warp-specialised x kernel the consumer warp is the critical one, and six more fields through
+// its staging tile cost more than re-reading the five conserved fields once.  shasta_step avoids that pass where it can
+// (see there): the NEXT sweep reads those fields anyway and emits their primitives (emit = 2).
+int launch_sweep(shasta_t* h, int axis, int emit, cudaStream_t st)
 {
-    if (emit && axis == 0 && !h->predictor && !h->cell_path) {
-        int rc = launch_sweep_raw(h, axis, false, st);
+    if (emit == 2 && (axis == 0 || !fused_path(h)))
+        return fail(h, SHASTA_EINVAL, "emit = 2 (primitives of the input state) exists for the fused y and z sweeps only");
+    if (emit == 1 && axis == 0 && fused_path(h)) {
+        int rc = launch_sweep_raw(h, axis, 0, st);
         if (rc) return rc;
         return h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
     }
@@ -617,6 +625,12 @@ int shasta_set_option(shasta_t* h, int key, double value)
         return 0;
     case SHASTA_NO_TMA:
         h->no_tma = value != 0.0;
+        return 0;
+    case SHASTA_PRIMS_RAW:
+        h->prims_raw = value != 0.0;
+        return 0;
+    case SHASTA_NO_DEFER:
+        h->no_defer = value != 0.0;
         return 0;
     case SHASTA_DIFF:
         if (!(value >= 0.0) || value > 8.0) return fail(h, SHASTA_EINVAL, "SHASTA_DIFF must be in [0, 8]");
@@ -735,6 +749,11 @@ int shasta_step(shasta_t* h, int nsteps, void* stream)
     if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_step: call shasta_set_state first");
     cudaStream_t st = (cudaStream_t)stream;
     const int n[3] = {h->nx, h->ny, h->nz};
+    // A step whose last sweep runs along x does not write its primitives at once: the first sweep of the NEXT step reads
+    // the same five conserved fields anyway and writes the primitives of its input state beside its own work (emit = 2,
+    // +0.1 ms at 256^3 instead of +0.26 ms for the separate element-wise pass).  Every step's primitives are still
+    // written exactly once; the deferral never leaves this call (the last step of the call is completed below).
+    bool deferred = false;
     for (int s = 0; s < nsteps; ++s) {
         int axes[3], na = 0;
         for (int k = 0; k < 3; ++k) {
@@ -742,11 +761,26 @@ int shasta_step(shasta_t* h, int nsteps, void* stream)
             if (n[a] > 1) axes[na++] = a;                 // reading G15: axes of extent 1 are skipped
         }
         for (int k = 0; k < na; ++k) {
-            int rc = launch_sweep(h, axes[k], k == na - 1, st);
+            const bool last = k == na - 1;
+            int emit = last ? 1 : 0;
+            if (deferred) {                               // k == 0
+                deferred = false;
+                if (!last && axes[k] != 0) emit = 2;
+                else {
+                    int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
+                    if (rc) return rc;
+                }
+            }
+            if (last && axes[k] == 0 && fused_path(h) && !h->no_defer) { emit = 0; deferred = true; }
+            int rc = launch_sweep(h, axes[k], emit, st);
             if (rc) return rc;
         }
         if (na > 0) h->prims_valid = true;
         h->step++;
+    }
+    if (deferred) {
+        int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
+        if (rc) return rc;
     }
     return 0;
 }
@@ -758,9 +792,10 @@ int shasta_sweep(shasta_t* h, int axis, int emit_primitives, void* stream)
     if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_sweep: call shasta_set_state first");
     const int n[3] = {h->nx, h->ny, h->nz};
     if (n[axis] == 1) return 0;
-    int rc = launch_sweep(h, axis, emit_primitives != 0, (cudaStream_t)stream);
+    if (emit_primitives < 0 || emit_primitives > 2) return fail(h, SHASTA_EINVAL, "shasta_sweep: emit_primitives must be 0, 1 or 2");
+    int rc = launch_sweep(h, axis, emit_primitives, (cudaStream_t)stream);
     if (rc) return rc;
-    h->prims_valid = emit_primitives != 0;
+    h->prims_valid = emit_primitives == 1;
     return 0;
 }
 
@@ -770,7 +805,7 @@ int shasta_get_primitives(shasta_t* h, double* e, double* p, double* n, double* 
     if (!h) return SHASTA_EINVAL;
     if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_get_primitives: no state set");
     cudaStream_t st = (cudaStream_t)stream;
-    if (!h->prims_valid) {
+    if (!h->prims_valid && !h->prims_raw) {
         int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
         if (rc) return rc;
     }
@@ -789,7 +824,7 @@ int shasta_get_primitives_host(shasta_t* h, double* e, double* p, double* n, dou
     if (!h) return SHASTA_EINVAL;
     if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_get_primitives_host: no state set");
     cudaStream_t st = (cudaStream_t)stream;
-    if (!h->prims_valid) {
+    if (!h->prims_valid && !h->prims_raw) {
         int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
         if (rc) return rc;
     }

@@ -866,7 +866,10 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
 // P.axis: 1 = y sweep (pencil = (x, z), cell stride nx), 2 = z sweep (pencil = (x, y), cell stride nx ny).
 // grid.x = ceil(nxb * n_other / 4) with nxb = ceil(nx / 32) x-blocks per row: warp pair w of CTA b owns the 32 pencils
 // x0 .. x0+31 of row `oth`, (xb, oth) = divmod(4 b + w, nxb); grid.y = segments.
-template <typename T, int EOS, bool EMIT, bool TMA>
+// EMIT: 0 = conserved fields only; 1 = also the six primitives of the NEW state (last sweep of a step); 2 = also the six
+// primitives of the state this sweep READS (the deferred primitive output of a step whose last sweep ran along x: the
+// consumer has U^n of its output cell in the ring tile of the previous group).
+template <typename T, int EOS, int EMIT, bool TMA>
 __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant__ SweepParams P,
                                                           const __grid_constant__ Consts<T> k,
                                                           const __grid_constant__ YzMaps maps)
@@ -998,9 +1001,9 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
         {                                                                                           \
             if (g >= 2 && (S_) < left) {                                                            \
                 T pv[6];                                                                            \
-                finish_cell<T, EOS, EMIT>(k, UN, pv, cnt);                                          \
+                finish_cell<T, EOS, EMIT == 1>(k, UN, pv, cnt);                                     \
                 _Pragma("unroll") for (int f = 0; f < NF; ++f) ((T*)P.out[f])[o] = UN[f];           \
-                if (EMIT) { _Pragma("unroll") for (int qq = 0; qq < 6; ++qq) ((T*)P.prim[qq])[o] = pv[qq]; } \
+                if (EMIT == 1) { _Pragma("unroll") for (int qq = 0; qq < 6; ++qq) ((T*)P.prim[qq])[o] = pv[qq]; } \
             }                                                                                       \
             o += sa;                                                                                \
         }
@@ -1033,6 +1036,32 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
             load2(mq + 384, msg[0], msg[1]); load2(mq + 448, msg[2], msg[3]);
             co.template step<3>(c1, c2, msg, un);
             SHK_YZ_OUT(un, 3)
+            if (EMIT == 2 && g >= 2) {
+                // primitives of the INPUT state of this group's output cells = the four cells of the previous group's ring
+                // tile; done after the four steps, when only the carried window is alive in registers
+                load_fence();
+#pragma unroll 1
+                for (int c = 0; c < YZ_CH; ++c) {
+                    if (c < left) {
+                        // momenta in NATURAL order (x, y, z), so that |M|^2 rounds as in the element-wise pass this replaces
+                        // (same bits): slots of a y sweep hold (My, Mz, Mx), of a z sweep (Mz, Mx, My)
+                        T ui[NF], pv[6];
+                        const T m1 = tp[1 * YZ_CH * 32 + 32 * c], m2 = tp[2 * YZ_CH * 32 + 32 * c], m3 = tp[3 * YZ_CH * 32 + 32 * c];
+                        ui[0] = tp[32 * c];
+                        ui[1] = ysweep ? m3 : m2;
+                        ui[2] = ysweep ? m1 : m3;
+                        ui[3] = ysweep ? m2 : m1;
+                        ui[4] = tp[4 * YZ_CH * 32 + 32 * c];
+                        emit_primitives<T, EOS>(k, ui, pv, cnt);
+                        const long long oc = o + (long long)(c - YZ_CH) * sa;
+#pragma unroll
+                        for (int qq = 0; qq < 3; ++qq) ((T*)P.prim[qq])[oc] = pv[qq];
+                        ((T*)P.prim[ysweep ? 5 : 4])[oc] = pv[3];
+                        ((T*)P.prim[ysweep ? 3 : 5])[oc] = pv[4];
+                        ((T*)P.prim[ysweep ? 4 : 3])[oc] = pv[5];
+                    }
+                }
+            }
             if (g >= 2) left -= YZ_CH;
             if (g + 2 < ngroups) bar_arrive64(bar_id + 2 + (g & 1));
         }

@@ -12,7 +12,7 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libshasta.so")
 
-BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
+BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH, NO_DEFER, PRIMS_RAW = range(12)
 R1, R2 = 0, 1
 OUTFLOW, PERIODIC = 0, 1
 BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
@@ -98,7 +98,7 @@ class Shasta:
     """One solver handle = shasta_create ... shasta_destroy.  Method names follow the C ABI."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, precision=64,
-                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0):
+                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0):
         L = load()
         self._L = L
         self._h = _vp()
@@ -122,6 +122,8 @@ class Shasta:
             self.set_option(DIFF, diff)
         if cell_path:
             self.set_option(CELL_PATH, 1)
+        if no_defer:
+            self.set_option(NO_DEFER, 1)
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
@@ -157,7 +159,7 @@ class Shasta:
         self._chk(self._L.shasta_step(self._h, int(nsteps), _stream_ptr(stream)), "shasta_step")
 
     def sweep(self, axis, emit_primitives=False, stream=None):
-        self._chk(self._L.shasta_sweep(self._h, int(axis), int(bool(emit_primitives)), _stream_ptr(stream)),
+        self._chk(self._L.shasta_sweep(self._h, int(axis), int(emit_primitives), _stream_ptr(stream)),
                   "shasta_sweep")
 
     def get_conserved(self, stream=None):

@@ -173,6 +173,56 @@ def test_step_split_and_step_index(oracle):
     assert s.launch_count >= 21
 
 
+@pytest.mark.parametrize("shape", [(70, 45, 50), (64, 33, 6), (37, 19, 23)])
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+def test_deferred_primitives_of_x_last_steps(oracle, shape, bc):
+    # a step whose last sweep runs along x leaves its primitives to the first sweep of the next step (emit = 2, DESIGN.md
+    # 7.2); SHASTA_NO_DEFER writes them at once.  Same bits either way, wherever the call is cut (steps 3 and 4 of the
+    # paper's table end with x), and both equal the oracle.
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    c = inputs.random_state(*shape, seed=31 + bc, kind="rough", boundary=bc)
+    dev = [torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")]
+    for cuts in [(4,), (5,), (3, 1, 1, 2), (6, 6)]:
+        res = []
+        for nd in (0, 1):
+            s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"], no_defer=nd)
+            s.set_state(*dev)
+            for n in cuts:
+                s.step(n)
+            r = {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
+            r.update({k: v.cpu().numpy() for k, v in s.get_primitives().items()})
+            res.append((r, s.launch_count))
+        for k in parity.CONS + parity.PRIM:
+            assert np.array_equal(res[0][0][k], res[1][0][k]), (cuts, k)
+        assert res[0][1] <= res[1][1]
+        if cuts in [(5,), (6, 6)]:          # an x-last step followed by another step inside one call
+            assert res[0][1] < res[1][1], "the deferred path must launch fewer kernels"
+    ref, _ = parity.run_oracle(oracle, c, steps=5)
+    got, _ = parity.run_gpu(c, steps=5)
+    assert_kernel_parity(got, ref, f"deferred primitives shape {shape} bc {bc}")
+    # single sweeps through the ABI: emit_primitives = 2 writes the primitives of the state BEFORE the sweep; they are
+    # read back as stored (SHASTA_PRIMS_RAW: no refresh) and must equal, bit for bit, what the x sweep + element-wise
+    # pass writes for that state
+    from paper_1206_0919_b200 import shasta as sh
+    mk = lambda: Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"])
+    for axis in (1, 2):
+        s, want = mk(), mk()
+        s.set_state(*dev); want.set_state(*dev)
+        want.sweep(0, 1)
+        pw = {k: v.cpu().numpy() for k, v in want.get_primitives().items()}
+        want.sweep(axis, 0)
+        s.sweep(0, 0)
+        s.sweep(axis, 2)
+        s.set_option(sh.PRIMS_RAW, 1)
+        for k, v in s.get_primitives().items():
+            assert np.array_equal(v.cpu().numpy(), pw[k]), (axis, k)
+        for k, v in s.get_conserved().items():
+            assert np.array_equal(v.cpu().numpy(), want.get_conserved()[k].cpu().numpy()), (axis, k)
+    with pytest.raises(Exception):
+        mk().sweep(0, 2)
+
+
 def test_host_buffer_entry_points(oracle):
     c = inputs.random_state(21, 17, 13, seed=8, kind="smooth")
     ref, _ = parity.run_oracle(oracle, c, steps=2)
