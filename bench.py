@@ -54,6 +54,7 @@ def parse_args():
     ap.add_argument("--size", type=int, default=256, help="grid extent (256 = the metric's workload)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--segment", type=int, default=0, help="tuning: cells marched per work item (0 = auto)")
+    ap.add_argument("--batch", type=int, default=1, help="independent events per GPU advanced by one launch (SHASTA_BATCH)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -206,15 +207,18 @@ def ours(args):
 
     # one independent event per rank (weak scaling, replicas: DESIGN.md 9)
     n = args.size
-    c = inputs.hotspots(n, steps=args.steps, seed=replicas.event_seed(rank))
-    ncell = n ** 3
+    import numpy as np
+    B = max(1, args.batch)
+    cs = [inputs.hotspots(n, steps=args.steps, seed=replicas.event_seed(rank) + 1000 * b) for b in range(B)]
+    c = cs[0]
+    ncell = B * n ** 3              # cells advanced per step on this GPU (all events of the batch)
     names = ("e", "n", "vx", "vy", "vz")
-    host_in = [torch.from_numpy(c[k]).pin_memory() for k in names]
-    host_out = [torch.empty((n, n, n), dtype=torch.float64).pin_memory() for _ in range(6)]
+    host_in = [torch.from_numpy(c[k] if B == 1 else np.stack([cb[k] for cb in cs])).pin_memory() for k in names]
+    host_out = [torch.empty(host_in[0].shape, dtype=torch.float64).pin_memory() for _ in range(6)]
     dev_in = [t.cuda(non_blocking=True) for t in host_in]
     stream = torch.cuda.current_stream()
     s = Shasta(n, n, n, c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"], precision=args.precision,
-               segment=args.segment)
+               segment=args.segment, batch=B)
     s.set_state(*dev_in)
     K, W = args.steps, args.warmup
     s.step(W)
@@ -351,7 +355,7 @@ def ours(args):
             "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
             "config": {"workload": f"hotspots {n}^3 (BASELINE.json configs[3]): 50 Gaussian hotspots + "
                                    "vz=tanh(z/4), dx=0.1 fm, lambda=0.4, p=e/3, outflow; one event per GPU",
-                       "grid": [n, n, n], "cells_per_gpu": ncell, "parallelism": f"replicas x{world}",
+                       "grid": [n, n, n], "batch": B, "cells_per_gpu": ncell, "parallelism": f"replicas x{world}",
                        "l2": "state (2x5 fields ping-pong + 6 primitives, "
                              f"{16 * ncell * args.precision // 8 / 1e6:.0f} MB) is larger than the 126 MB L2; no flush",
                        "timing": "CUDA events on the launching stream, max over ranks"},

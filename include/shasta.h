@@ -60,6 +60,17 @@ typedef struct shasta shasta_t;   /* opaque */
 #define SHASTA_PRIMS_RAW 11   /* test hook: 1 = shasta_get_primitives[_host] copies the primitive fields as they are stored,
                                  without recomputing them when they are stale (reads back what emit_primitives = 2 wrote) */
 
+#define SHASTA_BATCH     12   /* B >= 1 independent events of the same grid advanced together by every launch (the paper's
+                                 use case is event-by-event statistics).  Every
+                                 field argument then holds B consecutive events, B*nx*ny*nz doubles, event b at offset
+                                 b*nx*ny*nz; shasta_conserved_totals writes 5*B values.  Events never interact: each has
+                                 its own boundary.  Before the first set_state; default 1                               */
+
+#define SHASTA_GRAPH     13   /* launch mode of shasta_step: 0 = every kernel launched on its own; 1 = whole cycles of the axis
+                                 table (6 steps = 18 sweeps for the paper's table) are captured once into a CUDA graph and
+                                 replayed; 2 (default) = 1 for grids below 2^22 cells, where a sweep lasts ~10 us and the
+                                 "orchestration overhead" of PAPER.md:155 shows, else 0.  Same kernels, same results.  */
+
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only
  * (eqs. (15)-(17)); dx enters shasta_conserved_totals.  0 < lambda <= 0.5
@@ -122,7 +133,8 @@ int shasta_get_primitives_host(shasta_t* h, double* e_host, double* p_host, doub
                                double* vx_host, double* vy_host, double* vz_host, void* stream);
 
 /* dx^3 * sum over cells of E, Mx, My, Mz, R (the conserved totals of eqs. (12)-(14)),
- * compensated fp64 summation.  `totals_host` is a host pointer to 5 doubles.  SYNCHRONISES `stream`. */
+ * compensated fp64 summation.  `totals_host` is a host pointer to 5 doubles (5*B for a batch of B events, event
+ * after event).  SYNCHRONISES `stream`. */
 int shasta_conserved_totals(shasta_t* h, double* totals_host, void* stream);
 
 /* Cumulative counters since create (host pointer to 4 values): [0] cells where the projection Pi
@@ -132,6 +144,8 @@ int shasta_diagnostics(shasta_t* h, unsigned long long* counts_host);
 
 /* Number of kernels this handle has launched since create (bench.py's gpu_launches). */
 long long shasta_launch_count(const shasta_t* h);
+/* Number of CUDA-graph launches shasta_step has made (each replays one cycle of the axis table; SHASTA_GRAPH). */
+long long shasta_graph_launch_count(const shasta_t* h);
 /* Step counter s (number of steps taken, or the value set by SHASTA_STEP_INDEX). */
 long long shasta_step_index(const shasta_t* h);
 /* Name of the sweep kernel variant used for `axis` with the current options (for profiles/). */

@@ -25,7 +25,9 @@ constexpr int RED_THREADS = 256;
 
 struct shasta {
     int nx, ny, nz;
-    long long ncell;
+    long long ncell;        // cells of ALL events of the batch: nbatch * ncell1
+    long long ncell1;       // cells of one event, nx * ny * nz
+    int nbatch;             // independent events stacked along z (SHASTA_BATCH); 1 by default
     double dx, lambda, gamma, mass;
     double diff;            // factor on the antidiffusive flux; 1 by default
     int cell_path;          // 1 = run the per-cell kernels also for the default scheme (A/B datapoint, tests)
@@ -34,6 +36,11 @@ struct shasta {
     int precision;          // 64 | 32
     int seg_override;
     int no_tma;             // test hook: 1 = x sweep through cp.async even where TMA is possible
+    int graph_mode;         // SHASTA_GRAPH: 0 never, 1 always, 2 auto (grids whose sweeps are launch/latency bound)
+    struct GraphEntry { int phase, cur, chunk; cudaGraphExec_t exec; long long launches; } graphs[8];
+    int ngraphs;
+    long long graph_launches;
+    cudaStream_t cap_stream;
     int prims_raw;          // test hook: get_primitives copies the primitive fields as stored, without refreshing them
     int no_defer;           // test hook / A-B: 1 = x-last steps write their primitives at once (separate element-wise pass)
     long long step;
@@ -115,7 +122,7 @@ int make_tensor_maps(shasta_t* h)
         cudaGetLastError();
         return 0;                                   // no TMA: the cp.async path still works
     }
-    const cuuint64_t dims[2] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny * (cuuint64_t)h->nz};
+    const cuuint64_t dims[2] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny * (cuuint64_t)h->nz * (cuuint64_t)h->nbatch};
     const cuuint64_t strides[1] = {(cuuint64_t)h->nx * sizeof(double)};
     const cuuint32_t box[2] = {(cuuint32_t)XV_CH, 32u};
     const cuuint32_t estr[2] = {1u, 1u};
@@ -148,7 +155,7 @@ int make_yz_maps(shasta_t* h)
         return 0;
     }
     const CUtensorMapDataType dt = es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-    const cuuint64_t dims[3] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz};
+    const cuuint64_t dims[3] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz * (cuuint64_t)h->nbatch};
     const cuuint64_t strides[2] = {(cuuint64_t)h->nx * es, (cuuint64_t)h->nx * (cuuint64_t)h->ny * es};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const cuuint32_t boxes[3][3] = {{32u, (cuuint32_t)YZ_CH, 1u}, {32u, 1u, (cuuint32_t)YZ_CH}, {32u, 1u, 1u}};
@@ -370,10 +377,11 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
     P.stride_axis = stride[axis];
     P.periodic = h->periodic;
     P.axis = axis;
+    P.odiv = 0x7fffffff;
     P.counts = h->d_counts;
     const Consts<T> k = make_consts<T>(h);
     if (axis == 0) {
-        P.npencil = (long long)h->ny * h->nz;
+        P.npencil = (long long)h->ny * h->nz * h->nbatch;
         P.stride_other = 0;
         P.seg = auto_segment(h, axis, P.N, (P.npencil + 127) / 128);
         P.nseg = (P.N + P.seg - 1) / P.seg;
@@ -406,7 +414,8 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
         {
             // producer/consumer warp pairs, 32 pencils (one x-block of a row) per pair, 4 pairs per CTA; TMA-fed when possible
             const long long nxb = (h->nx + 31) / 32;
-            P.npencil = nxb * n[other];                                         // pencil GROUPS
+            P.npencil = nxb * n[other] * h->nbatch;                             // pencil GROUPS (all events)
+            P.odiv = (axis == 2 && h->nbatch > 1) ? h->ny : 0x7fffffff;
             const long long ctas = (P.npencil + 3) / 4;
             P.seg = auto_segment(h, axis, P.N, ctas);
             P.nseg = (P.N + P.seg - 1) / P.seg;
@@ -540,6 +549,88 @@ int export_field(shasta_t* h, const void* src, double* dst_dev, cudaStream_t st)
     return 0;
 }
 
+// cached CUDA graphs of whole axis-table cycles (shasta_step): dropped whenever an option or the table changes
+void drop_graphs(shasta_t* h)
+{
+    for (int i = 0; i < h->ngraphs; ++i) cudaGraphExecDestroy(h->graphs[i].exec);
+    h->ngraphs = 0;
+}
+
+// `nsteps` time steps, launch by launch (step s runs the sweeps branch[3s .. 3s+2]).
+int run_steps(shasta_t* h, int nsteps, cudaStream_t st)
+{
+    const int n[3] = {h->nx, h->ny, h->nz};
+    // A step whose last sweep runs along x does not write its primitives at once: the first sweep of the NEXT step reads
+    // the same five conserved fields anyway and writes the primitives of its input state beside its own work (emit = 2,
+    // +0.14 ms at 256^3 instead of +0.26 ms for the separate element-wise pass).  Every step's primitives are still
+    // written exactly once; the deferral never leaves this call (the last step of the call is completed below).
+    bool deferred = false;
+    for (int s = 0; s < nsteps; ++s) {
+        int axes[3], na = 0;
+        for (int k = 0; k < 3; ++k) {
+            const int a = h->table[(3 * h->step + k) % h->ntable];
+            if (n[a] > 1) axes[na++] = a;                 // reading G15: axes of extent 1 are skipped
+        }
+        for (int k = 0; k < na; ++k) {
+            const bool last = k == na - 1;
+            int emit = last ? 1 : 0;
+            if (deferred) {                               // k == 0
+                deferred = false;
+                if (!last && axes[k] != 0) emit = 2;
+                else {
+                    int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
+                    if (rc) return rc;
+                }
+            }
+            if (last && axes[k] == 0 && fused_path(h) && !h->no_defer) { emit = 0; deferred = true; }
+            int rc = launch_sweep(h, axes[k], emit, st);
+            if (rc) return rc;
+        }
+        if (na > 0) h->prims_valid = true;
+        h->step++;
+    }
+    if (deferred) {
+        int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+// The graph of `chunk` steps starting at table phase `phase` with the state in buffer `cur` (captured on a private
+// stream on first use; the capture executes nothing).  PAPER.md:155 names the "orchestration overhead" of many small
+// kernels: for grids whose sweeps take ~10 us the launches of a whole cycle (18 sweeps) go to the GPU as one graph.
+int get_graph(shasta_t* h, int phase, int chunk, shasta::GraphEntry** out)
+{
+    *out = nullptr;
+    for (int i = 0; i < h->ngraphs; ++i)
+        if (h->graphs[i].phase == phase && h->graphs[i].cur == h->cur && h->graphs[i].chunk == chunk) { *out = &h->graphs[i]; return 0; }
+    if (h->ngraphs == 8) drop_graphs(h);
+    if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    const long long step0 = h->step, l0 = h->launches;
+    const int cur0 = h->cur;
+    const bool pv0 = h->prims_valid;
+    CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    const int rc = run_steps(h, chunk, h->cap_stream);
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
+    const long long nl = h->launches - l0;
+    const bool same_buffer = h->cur == cur0;
+    h->step = step0; h->launches = l0; h->cur = cur0; h->prims_valid = pv0;
+    if (rc || e != cudaSuccess || !g || !same_buffer) {
+        if (g) cudaGraphDestroy(g);
+        cudaGetLastError();
+        return rc ? rc : 1;                              // 1 = no graph: the caller launches directly
+    }
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t e2 = cudaGraphInstantiate(&exec, g, 0);
+    cudaGraphDestroy(g);
+    if (e2 != cudaSuccess) { cudaGetLastError(); return 1; }
+    shasta::GraphEntry& ge = h->graphs[h->ngraphs++];
+    ge.phase = phase; ge.cur = cur0; ge.chunk = chunk; ge.exec = exec; ge.launches = nl;
+    *out = &ge;
+    return 0;
+}
+
 }  // namespace
 
 // =========================================================================== C ABI
@@ -569,10 +660,12 @@ int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lamb
     if (!h) return fail(nullptr, SHASTA_ENOMEM, "shasta_create: host allocation failed");
     memset(h, 0, sizeof(*h));
     h->nx = nx; h->ny = ny; h->nz = nz;
-    h->ncell = (long long)nx * ny * nz;
+    h->ncell = h->ncell1 = (long long)nx * ny * nz;
+    h->nbatch = 1;
     h->dx = dx; h->lambda = lambda; h->gamma = eos_gamma; h->mass = 0.0;
     h->precision = 64;
     h->diff = 1.0;
+    h->graph_mode = 2;
     memcpy(h->table, kBranch, sizeof(kBranch));
     h->ntable = 18;
     h->sm_count = prop.multiProcessorCount;
@@ -583,6 +676,8 @@ int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lamb
 void shasta_destroy(shasta_t* h)
 {
     if (!h) return;
+    drop_graphs(h);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (int b = 0; b < 2; ++b)
         for (int f = 0; f < NF; ++f) cudaFree(h->U[b][f]);
     for (int q = 0; q < 6; ++q) cudaFree(h->prim[q]);
@@ -598,7 +693,12 @@ void shasta_destroy(shasta_t* h)
 int shasta_set_option(shasta_t* h, int key, double value)
 {
     if (!h) return SHASTA_EINVAL;
+    drop_graphs(h);                                       // cached graphs bake the options in
     switch (key) {
+    case SHASTA_GRAPH:
+        if (value != 0.0 && value != 1.0 && value != 2.0) return fail(h, SHASTA_EINVAL, "SHASTA_GRAPH must be 0, 1 or 2");
+        h->graph_mode = (int)value;
+        return 0;
     case SHASTA_BOUNDARY:
         if (value != 0.0 && value != 1.0) return fail(h, SHASTA_EINVAL, "SHASTA_BOUNDARY must be 0 or 1");
         h->periodic = (int)value;
@@ -625,6 +725,16 @@ int shasta_set_option(shasta_t* h, int key, double value)
         return 0;
     case SHASTA_NO_TMA:
         h->no_tma = value != 0.0;
+        return 0;
+    case SHASTA_BATCH:
+        if (!(value >= 1.0) || value > 65536.0 || value != (double)(int)value)
+            return fail(h, SHASTA_EINVAL, "SHASTA_BATCH must be an integer in [1, 65536]");
+        if (h->allocated && (int)value != h->nbatch)
+            return fail(h, SHASTA_ESTATE, "SHASTA_BATCH must be set before the first set_state");
+        if ((double)h->nz * value > 2147483647.0 / 2)
+            return fail(h, SHASTA_EINVAL, "SHASTA_BATCH: nz * batch too large");
+        h->nbatch = (int)value;
+        h->ncell = h->ncell1 * h->nbatch;
         return 0;
     case SHASTA_PRIMS_RAW:
         h->prims_raw = value != 0.0;
@@ -658,6 +768,7 @@ int shasta_set_sweep_table(shasta_t* h, const int* axes, int n)
     if (!axes || n < 3 || n > 63 || n % 3) return fail(h, SHASTA_EINVAL, "sweep table: need n % 3 == 0, 3 <= n <= 63");
     for (int i = 0; i < n; ++i)
         if (axes[i] < 0 || axes[i] > 2) return fail(h, SHASTA_EINVAL, "sweep table: axes must be 0, 1 or 2");
+    drop_graphs(h);
     memcpy(h->table, axes, sizeof(int) * (size_t)n);
     h->ntable = n;
     return 0;
@@ -748,41 +859,33 @@ int shasta_step(shasta_t* h, int nsteps, void* stream)
     if (nsteps < 0) return fail(h, SHASTA_EINVAL, "shasta_step: nsteps < 0");
     if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_step: call shasta_set_state first");
     cudaStream_t st = (cudaStream_t)stream;
-    const int n[3] = {h->nx, h->ny, h->nz};
-    // A step whose last sweep runs along x does not write its primitives at once: the first sweep of the NEXT step reads
-    // the same five conserved fields anyway and writes the primitives of its input state beside its own work (emit = 2,
-    // +0.1 ms at 256^3 instead of +0.26 ms for the separate element-wise pass).  Every step's primitives are still
-    // written exactly once; the deferral never leaves this call (the last step of the call is completed below).
-    bool deferred = false;
-    for (int s = 0; s < nsteps; ++s) {
-        int axes[3], na = 0;
-        for (int k = 0; k < 3; ++k) {
-            const int a = h->table[(3 * h->step + k) % h->ntable];
-            if (n[a] > 1) axes[na++] = a;                 // reading G15: axes of extent 1 are skipped
+    // whole cycles of the axis table as one CUDA graph each (auto: only where a sweep is short enough for launch gaps to
+    // show, < 2^22 cells); the remainder launch by launch
+    const bool want_graph = h->graph_mode == 1 || (h->graph_mode == 2 && h->ncell < (1LL << 22));
+    if (want_graph && h->ntable % 3 == 0) {
+        const int period = h->ntable / 3;
+        int na = 0;
+        if (h->nx > 1) ++na;
+        if (h->ny > 1) ++na;
+        if (h->nz > 1) ++na;
+        int sweeps = 0;                                   // sweeps of one period (every table entry of an active axis)
+        const int n[3] = {h->nx, h->ny, h->nz};
+        for (int i = 0; i < h->ntable; ++i) sweeps += n[h->table[i]] > 1;
+        const int chunk = (sweeps % 2 == 0) ? period : 2 * period;      // the state must return to the buffer it started in
+        while (na > 0 && nsteps >= chunk) {
+            shasta::GraphEntry* ge = nullptr;
+            const int rc = get_graph(h, (int)(h->step % period), chunk, &ge);
+            if (rc < 0) return rc;
+            if (!ge) break;
+            CK(cudaGraphLaunch(ge->exec, st));
+            h->launches += ge->launches;
+            h->graph_launches++;
+            h->step += chunk;
+            h->prims_valid = true;
+            nsteps -= chunk;
         }
-        for (int k = 0; k < na; ++k) {
-            const bool last = k == na - 1;
-            int emit = last ? 1 : 0;
-            if (deferred) {                               // k == 0
-                deferred = false;
-                if (!last && axes[k] != 0) emit = 2;
-                else {
-                    int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
-                    if (rc) return rc;
-                }
-            }
-            if (last && axes[k] == 0 && fused_path(h) && !h->no_defer) { emit = 0; deferred = true; }
-            int rc = launch_sweep(h, axes[k], emit, st);
-            if (rc) return rc;
-        }
-        if (na > 0) h->prims_valid = true;
-        h->step++;
     }
-    if (deferred) {
-        int rc = h->precision == 64 ? refresh_prims_t<double>(h, st) : refresh_prims_t<float>(h, st);
-        if (rc) return rc;
-    }
-    return 0;
+    return run_steps(h, nsteps, st);
 }
 
 int shasta_sweep(shasta_t* h, int axis, int emit_primitives, void* stream)
@@ -853,26 +956,29 @@ int shasta_conserved_totals(shasta_t* h, double* totals, void* stream)
     if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_conserved_totals: no state set");
     cudaStream_t st = (cudaStream_t)stream;
     void** U = h->U[h->cur];
-    if (h->precision == 64)
-        totals_kernel<double><<<RED_BLOCKS, RED_THREADS, 0, st>>>(h->ncell, (double*)U[0], (double*)U[1],
-            (double*)U[2], (double*)U[3], (double*)U[4], h->d_partial);
-    else
-        totals_kernel<float><<<RED_BLOCKS, RED_THREADS, 0, st>>>(h->ncell, (float*)U[0], (float*)U[1],
-            (float*)U[2], (float*)U[3], (float*)U[4], h->d_partial);
-    CK(cudaGetLastError());
-    h->launches++;
-    CK(cudaMemcpyAsync(h->h_partial, h->d_partial, sizeof(double) * RED_BLOCKS * NF * 2, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
     const double dv = h->dx * h->dx * h->dx;
-    for (int f = 0; f < NF; ++f) {
-        double s = 0.0, c = 0.0;
-        for (int b = 0; b < RED_BLOCKS; ++b) {
-            const double x = h->h_partial[(b * NF + f) * 2 + 0];
-            const double t = s + x;
-            c += h->h_partial[(b * NF + f) * 2 + 1] + ((fabs(s) >= fabs(x)) ? ((s - t) + x) : ((x - t) + s));
-            s = t;
+    for (int b = 0; b < h->nbatch; ++b) {           // one event at a time (totals are per event)
+        const size_t off = (size_t)b * (size_t)h->ncell1;
+        if (h->precision == 64)
+            totals_kernel<double><<<RED_BLOCKS, RED_THREADS, 0, st>>>(h->ncell1, (double*)U[0] + off, (double*)U[1] + off,
+                (double*)U[2] + off, (double*)U[3] + off, (double*)U[4] + off, h->d_partial);
+        else
+            totals_kernel<float><<<RED_BLOCKS, RED_THREADS, 0, st>>>(h->ncell1, (float*)U[0] + off, (float*)U[1] + off,
+                (float*)U[2] + off, (float*)U[3] + off, (float*)U[4] + off, h->d_partial);
+        CK(cudaGetLastError());
+        h->launches++;
+        CK(cudaMemcpyAsync(h->h_partial, h->d_partial, sizeof(double) * RED_BLOCKS * NF * 2, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        for (int f = 0; f < NF; ++f) {
+            double s = 0.0, c = 0.0;
+            for (int k = 0; k < RED_BLOCKS; ++k) {
+                const double x = h->h_partial[(k * NF + f) * 2 + 0];
+                const double t = s + x;
+                c += h->h_partial[(k * NF + f) * 2 + 1] + ((fabs(s) >= fabs(x)) ? ((s - t) + x) : ((x - t) + s));
+                s = t;
+            }
+            totals[b * NF + f] = dv * (s + c);
         }
-        totals[f] = dv * (s + c);
     }
     return 0;
 }
@@ -889,6 +995,7 @@ int shasta_diagnostics(shasta_t* h, unsigned long long* counts)
 
 long long shasta_launch_count(const shasta_t* h) { return h ? h->launches : -1; }
 long long shasta_step_index(const shasta_t* h) { return h ? h->step : -1; }
+long long shasta_graph_launch_count(const shasta_t* h) { return h ? h->graph_launches : -1; }
 
 const char* shasta_kernel_name(const shasta_t* h, int axis)
 {

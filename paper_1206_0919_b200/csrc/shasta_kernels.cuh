@@ -72,6 +72,7 @@ struct SweepParams {
     int nseg;               // segments per pencil
     int periodic;           // boundary rule (reading G11)
     int axis;               // 0 x, 1 y, 2 z
+    int odiv;               // y/z kernel, batch of events: `other` index = oy + odiv * event (z sweep: odiv = ny); else INT_MAX
     unsigned long long* counts;   // diagnostics [4]
 };
 
@@ -885,6 +886,10 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
     const bool idle = pg >= P.npencil;                      // npencil = nxb * n_other pencil GROUPS for this kernel
     const int oth = (int)(pg / nxb);
     const int x0 = 32 * (int)(pg - (long long)oth * nxb);
+    // batch of independent events stacked along z: a y sweep sees nz * B planes, a z sweep B * ny rows of
+    // pencils, event `ob` owning the cells [ob * N, (ob + 1) * N) of the stacked z axis
+    const int ob = oth / P.odiv, oy = oth - ob * P.odiv;
+    const int zoff = ob * P.N;
     const bool active = x0 + lane < P.nx;
     const int xl = active ? x0 + lane : P.nx - 1;           // idle lanes shadow a valid pencil (non-TMA fill), store nothing
     const int j0 = blockIdx.y * P.seg;
@@ -910,7 +915,7 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
             __syncwarp();
         }
         unsigned phase = 0;             // bit q: parity to wait for on bar[q]
-        const long long lbase = (long long)xl + (long long)oth * P.stride_other;
+        const long long lbase = (long long)xl + (long long)oy * P.stride_other + (long long)zoff * sa;
         constexpr int NP = Producer<T, EOS>::NP;
         // group g = cells ilo+4g .. ilo+4g+3 -> ring tile g % 4.  Group g+1 is requested at the start of group g into
         // the tile of group g-3, which the consumer finished reading in its group g-2 (the `empty` barrier below).
@@ -926,14 +931,14 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
                         if (jg >= 0 && jg + YZ_CH <= N) {
 #pragma unroll
                             for (int f = 0; f < NF; ++f)
-                                tma_load_3d(&S.ring[q][f][0][0], maps.in4 + maps.fidx[f], x0, ysweep ? jg : oth, ysweep ? oth : jg, &S.bar[q]);
+                                tma_load_3d(&S.ring[q][f][0][0], maps.in4 + maps.fidx[f], x0, ysweep ? jg : oy, ysweep ? oth : zoff + jg, &S.bar[q]);
                         } else {        // ghost group (reading G11): 1-cell boxes at the ghost-mapped coordinate; rare, kept small
 #pragma unroll 1
                             for (int c = 0; c < YZ_CH; ++c) {
                                 const int jj = ghost_index(jg + c, N, P.periodic);
 #pragma unroll 1
                                 for (int f = 0; f < NF; ++f)
-                                    tma_load_3d(&S.ring[q][f][c][0], maps.in1 + maps.fidx[f], x0, ysweep ? jj : oth, ysweep ? oth : jj, &S.bar[q]);
+                                    tma_load_3d(&S.ring[q][f][c][0], maps.in1 + maps.fidx[f], x0, ysweep ? jj : oy, ysweep ? oth : zoff + jj, &S.bar[q]);
                             }
                         }
                     }
@@ -995,7 +1000,7 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
         Consumer<T> co;
         co.init(k.aq);
         // element offset of the output cell of the NEXT step: cell ilo - 4 (the first two groups store nothing)
-        long long o = (long long)(x0 + lane) + (long long)oth * P.stride_other + (long long)(ilo - GH) * sa;
+        long long o = (long long)(x0 + lane) + (long long)oy * P.stride_other + (long long)(zoff + ilo - GH) * sa;
         int left = active ? (j1 - j0) : 0;      // output cells this lane still has to store
 #define SHK_YZ_OUT(UN, S_)                                                                          \
         {                                                                                           \

@@ -12,7 +12,7 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libshasta.so")
 
-BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH, NO_DEFER, PRIMS_RAW = range(12)
+BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH, NO_DEFER, PRIMS_RAW, BATCH, GRAPH = range(14)
 R1, R2 = 0, 1
 OUTFLOW, PERIODIC = 0, 1
 BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
@@ -22,7 +22,7 @@ SYMBOLS = (
     "shasta_create", "shasta_destroy", "shasta_set_option", "shasta_set_sweep_table", "shasta_set_state",
     "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_step", "shasta_sweep",
     "shasta_get_primitives", "shasta_get_primitives_host", "shasta_conserved_totals", "shasta_diagnostics",
-    "shasta_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
+    "shasta_launch_count", "shasta_graph_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
 )
 
 _lib = None
@@ -56,6 +56,8 @@ def load():
     L.shasta_diagnostics.argtypes = [_vp, C.POINTER(C.c_ulonglong)]
     L.shasta_launch_count.argtypes = [_vp]
     L.shasta_launch_count.restype = C.c_longlong
+    L.shasta_graph_launch_count.argtypes = [_vp]
+    L.shasta_graph_launch_count.restype = C.c_longlong
     L.shasta_step_index.argtypes = [_vp]
     L.shasta_step_index.restype = C.c_longlong
     L.shasta_kernel_name.argtypes = [_vp, C.c_int]
@@ -98,12 +100,13 @@ class Shasta:
     """One solver handle = shasta_create ... shasta_destroy.  Method names follow the C ABI."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, precision=64,
-                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0):
+                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0, batch=1, graph=None):
         L = load()
         self._L = L
         self._h = _vp()
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
-        self.shape = (self.nz, self.ny, self.nx)
+        self.batch = int(batch)
+        self.shape = (self.nz, self.ny, self.nx) if self.batch == 1 else (self.batch, self.nz, self.ny, self.nx)
         rc = L.shasta_create(C.byref(self._h), nx, ny, nz, dx, lam, eos_gamma)
         if rc != 0:
             msg = L.shasta_last_error(None).decode()
@@ -124,6 +127,10 @@ class Shasta:
             self.set_option(CELL_PATH, 1)
         if no_defer:
             self.set_option(NO_DEFER, 1)
+        if self.batch != 1:
+            self.set_option(BATCH, self.batch)
+        if graph is not None:
+            self.set_option(GRAPH, graph)
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
@@ -184,9 +191,10 @@ class Shasta:
         return out
 
     def conserved_totals(self, stream=None):
-        t = (C.c_double * 5)()
+        t = (C.c_double * (5 * self.batch))()
         self._chk(self._L.shasta_conserved_totals(self._h, t, _stream_ptr(stream)), "shasta_conserved_totals")
-        return [float(x) for x in t]
+        v = [float(x) for x in t]
+        return v if self.batch == 1 else [v[5 * b:5 * b + 5] for b in range(self.batch)]
 
     def diagnostics(self):
         c = (C.c_ulonglong * 4)()
@@ -196,6 +204,10 @@ class Shasta:
     @property
     def launch_count(self):
         return int(self._L.shasta_launch_count(self._h))
+
+    @property
+    def graph_launch_count(self):
+        return int(self._L.shasta_graph_launch_count(self._h))
 
     @property
     def step_index(self):

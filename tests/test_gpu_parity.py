@@ -223,6 +223,56 @@ def test_deferred_primitives_of_x_last_steps(oracle, shape, bc):
         mk().sweep(0, 2)
 
 
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("shape", [(37, 19, 23), (64, 12, 10), (8, 5, 3)])
+def test_batch_of_independent_events(oracle, shape, bc):
+    # SHASTA_BATCH (row f4): B different events advanced by the same launches must equal B separate
+    # oracle runs -- no cell of one event may see another event across the stacked z axis (both boundary rules)
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    B = 3
+    cs = [inputs.random_state(*shape, seed=50 + b, kind="rough" if b != 1 else "smooth", boundary=bc) for b in range(B)]
+    c = cs[0]
+    s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"], batch=B)
+    s.set_state(*[torch.from_numpy(np.stack([cb[k] for cb in cs])).cuda() for k in ("e", "n", "vx", "vy", "vz")])
+    s.step(6)
+    got = {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
+    got.update({k: v.cpu().numpy() for k, v in s.get_primitives().items()})
+    tot = s.conserved_totals()
+    for b in range(B):
+        ref, o = parity.run_oracle(oracle, cs[b], steps=6)
+        assert_kernel_parity({k: v[b] for k, v in got.items()}, ref, f"batch event {b} shape {shape} bc {bc}")
+        t_ref = o.conserved_totals()
+        assert np.max(np.abs(np.array(tot[b]) - t_ref)) <= 1e-12 * abs(t_ref[0])
+    # one event of the batch alone gives the same bits as inside the batch
+    one, _ = parity.run_gpu(cs[1], steps=6)
+    for k in parity.CONS + parity.PRIM:
+        assert np.array_equal(one[k], got[k][1]), k
+
+
+@pytest.mark.parametrize("shape", [(40, 24, 20), (64, 1, 32), (1, 1, 80)])
+def test_cuda_graph_cycles_same_bits(shape):
+    # SHASTA_GRAPH: whole cycles of the axis table replayed as one CUDA graph ("orchestration overhead");
+    # same kernels, so the same bits as launch-by-launch, from any starting phase and with a remainder
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    c = inputs.random_state(*shape, seed=61, kind="rough")
+    dev = [torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")]
+    res = []
+    for graph in (0, 1):
+        s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"], graph=graph)
+        s.set_state(*dev)
+        s.step(2); s.step(15); s.step(6); s.step(1)
+        r = {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
+        r.update({k: v.cpu().numpy() for k, v in s.get_primitives().items()})
+        res.append((r, s.launch_count, s.graph_launch_count, s.step_index, s.diagnostics()))
+    for k in parity.CONS + parity.PRIM:
+        assert np.array_equal(res[0][0][k], res[1][0][k]), k
+    assert res[0][2] == 0 and res[1][2] == 3, (res[0][2], res[1][2])        # 15 = 2 cycles + 3, 6 = 1 cycle
+    assert res[0][3] == res[1][3] == 24 and res[0][4] == res[1][4]
+    assert res[0][1] == res[1][1], "launch_count counts the kernels inside the replayed graphs"
+
+
 def test_host_buffer_entry_points(oracle):
     c = inputs.random_state(21, 17, 13, seed=8, kind="smooth")
     ref, _ = parity.run_oracle(oracle, c, steps=2)
