@@ -36,7 +36,13 @@ B_SWEEP = 80.0      # algorithmic bytes per cell of one fused sweep: 5 fields re
 B_PRIM = 48.0       # + six primitive fields written by the last sweep of a step
 B_STEP = 3 * B_SWEEP + B_PRIM   # 288 B per cell-update
 HBM_FALLBACK_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-FP64_PER_CELL_SWEEP = 157.0     # fp64 instructions per cell of one Gamma-law sweep: producer 90 + consumer 67
+# fp64 instructions (DADD/DMUL/DFMA/DSETP + 64-bit MUFU seeds) per UPDATED cell of one plain Gamma-law y/z sweep: 174.1 per
+# marched cell (producer 96.1 + consumer 78.0, profiles/r2_sass_mix.md: executed-instruction counts of the ncu capture)
+# x 1.0625 marched cells per updated cell (segments of 128 re-march 8 halo cells)
+FP64_PER_CELL_SWEEP = 185.0
+# fp64 issue rate: 16 lanes per SM sub-partition = 64 results/clk/SM nominal; the round-1 micro-benchmark on this pool
+# measured 58.9 (DFMA) / 60.9 (DADD) results/clk/SM, so 60 is used as the measured ALU peak
+FP64_RESULTS_PER_CLK_SM = 60.0
 
 
 def sampler_clock_mhz(sampler):
@@ -294,20 +300,22 @@ def ours(args):
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": "profiles/traffic.json (committed ncu --set full capture, not measured in this run)",
+                "peak_source": peak_src,
                 "bytes_per_launch": dom["bytes"] / dom["launches"],
                 "avg_launch_ms": dom["ms"] / dom["launches"], "share_of_step": dom["ms"] / ms_sweeps,
                 "kernels": {k: {"avg_launch_ms": v["ms"] / v["launches"], "launches": v["launches"],
                                 "GB/s": v["bytes"] / (v["ms"] * 1e-3) / 1e9} for k, v in per.items()}}
-    # the second roof of this path: fp64 instructions.  157 per cell and sweep (SASS count of the
-    # Gamma-law producer 90 + consumer 67), 64 results/clk/SM measured on B200, at the SM clock sampled in this run
+    # the second roof of this path: fp64 instructions per cell and sweep against the fp64 issue rate at the
+    # SM clock sampled in this run
     clk = sampler_clock_mhz(sampler)
-    fp64_peak = 64.0 * torch.cuda.get_device_properties(local).multi_processor_count * clk * 1e6 / 1e9
+    fp64_peak = FP64_RESULTS_PER_CLK_SM * torch.cuda.get_device_properties(local).multi_processor_count * clk * 1e6 / 1e9
     fp64_ach = ncell * FP64_PER_CELL_SWEEP / (dom["ms"] / dom["launches"] * 1e-3) / 1e9
     alu_roofline = {"bound": "alu", "kernel": dom_name, "achieved": fp64_ach, "peak": fp64_peak,
                     "unit": "G fp64 warp-lane results/s", "frac": fp64_ach / fp64_peak,
                     "per_cell_sweep": FP64_PER_CELL_SWEEP, "clock_mhz": clk,
-                    "note": "halo re-march (+6 %) and rare-path instructions not counted in achieved"}
+                    "results_per_clk_sm": FP64_RESULTS_PER_CLK_SM,
+                    "note": "per-cell count and peak: profiles/r2_sass_mix.md; measured 58.9-60.9 results/clk/SM (nominal 64)"}
     step_gbs = value / world * B_STEP * (args.precision / 64.0) / 1e9
     step_roofline = {"bytes_per_cell_update": B_STEP * (args.precision / 64.0), "achieved": step_gbs,
                      "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,

@@ -21,6 +21,9 @@
  *   half step       PAPER.md:161      "implemented based on a half-step method"
  *   fixed point     PAPER.md:109      velocity by fixed-point root finding
  *   axis table      PAPER.md:295-297  branch[] = {0,1,2,0,2,1,2,0,1,2,1,0,1,2,0,1,0,2}
+ *   tabled EOS      PAPER.md:36, 109, 175  "easy implementation of a tabled equation of state": P(e,n) by bilinear
+ *                   interpolation in a table; the paper gives no table and no interpolation rule,
+ *                   the rule used is stated at eos_table_P below and in DESIGN.md 3 (reading T1)
  *
  * Where the paper is silent the readings G1-G19 of SURVEY.md 8(c.2), restated in
  * DESIGN.md section 3, are used; each is marked "reading Gn" below.
@@ -49,6 +52,12 @@
 
 enum { BC_OUTFLOW = 0, BC_PERIODIC = 1 };
 
+typedef struct eos_table {
+    int ne, nn;
+    double de, dn;
+    const double *p;
+} eos_table_t;
+
 typedef struct oracle_shasta {
     int nx, ny, nz;
     double dx, lambda, gamma, mass;
@@ -61,6 +70,8 @@ typedef struct oracle_shasta {
     double *U[NF];                /* conserved state, x fastest: ix + nx*(iy + ny*iz) */
     int have_state;
     unsigned long long counts[4]; /* Pi fired, vacuum cells, e<0 floored, p<0 floored */
+    eos_table_t tab;              /* tabled EOS (reading T1); have_tab = 0: ideal gas */
+    int have_tab;
 } oracle_t;
 
 static int g_threads = 1;
@@ -68,18 +79,39 @@ void oracle_set_threads(int n) { g_threads = n < 1 ? 1 : n; }
 int oracle_get_threads(void) { return g_threads; }
 
 /* ---------------------------------------------------------------- EOS ---- */
-/* ideal gas, reading G10: P(e,n) = max((Gamma-1)(e - m n), 0) */
-static double eos_P(double e, double n, double gamma, double mass)
+/* Tabled EOS (reading T1): pressure at the nodes (e_i, n_j) = (i de, j dn), i < ne, j < nn, stored e fastest:
+   p[i + ne*j].  Between nodes bilinear, outside the table the bilinear form of the nearest cell continues
+   (linear extrapolation); the result is floored at 0 like the ideal gas. */
+
+double oracle_eos_table_P(const eos_table_t *t, double e, double n)
 {
+    double xe = e / t->de, xn = n / t->dn;
+    int i = (int)floor(xe), j = (int)floor(xn);
+    if (i < 0) i = 0;
+    if (i > t->ne - 2) i = t->ne - 2;
+    if (j < 0) j = 0;
+    if (j > t->nn - 2) j = t->nn - 2;
+    double te = xe - i, tn = xn - j;
+    const double *q = t->p + i + (size_t)t->ne * j;
+    double p0 = q[0] + te * (q[1] - q[0]);                      /* along e at n_j */
+    double p1 = q[t->ne] + te * (q[t->ne + 1] - q[t->ne]);      /* along e at n_{j+1} */
+    double P = p0 + tn * (p1 - p0);
+    return P > 0.0 ? P : 0.0;
+}
+
+/* ideal gas, reading G10: P(e,n) = max((Gamma-1)(e - m n), 0); with a table: the table */
+static double eos_P(double e, double n, double gamma, double mass, const eos_table_t *tab)
+{
+    if (tab) return oracle_eos_table_P(tab, e, n);
     double p = (gamma - 1.0) * (e - mass * n);
     return p > 0.0 ? p : 0.0;
 }
 
 /* --------------------------------------------- eqs. (9)-(11): prim -> cons */
-void oracle_prim2cons(double e, double n, double vx, double vy, double vz,
-                      double gamma, double mass, double out[NF])
+void oracle_prim2cons_eos(double e, double n, double vx, double vy, double vz,
+                          double gamma, double mass, const eos_table_t *tab, double out[NF])
 {
-    double p = eos_P(e, n, gamma, mass);
+    double p = eos_P(e, n, gamma, mass, tab);
     double v2 = (vx * vx + vy * vy) + vz * vz;
     double g2 = 1.0 / (1.0 - v2);             /* gamma_L^2 */
     double w = (e + p) * g2;                  /* (eps + p) gamma^2 */
@@ -88,6 +120,11 @@ void oracle_prim2cons(double e, double n, double vx, double vy, double vz,
     out[2] = w * vy;
     out[3] = w * vz;
     out[4] = n * sqrt(g2);                    /* eq. (9) */
+}
+void oracle_prim2cons(double e, double n, double vx, double vy, double vz,
+                      double gamma, double mass, double out[NF])
+{
+    oracle_prim2cons_eos(e, n, vx, vy, vz, gamma, mass, NULL, out);
 }
 
 /* ------------------- phases 3+4: relativistic correction + EOS (cons2prim) */
@@ -108,8 +145,8 @@ int oracle_project(double E, double M[3])
 
 /* out = {e, p, n, vx, vy, vz, |v|}; returns the number of fixed-point iterations.
    flags (may be NULL): flags[0] += e floored, flags[1] += p floored. */
-int oracle_cons2prim(double E, double Mx, double My, double Mz, double R,
-                     double gamma, double mass, double out[7], int flags[2])
+int oracle_cons2prim_eos(double E, double Mx, double My, double Mz, double R,
+                         double gamma, double mass, const eos_table_t *tab, double out[7], int flags[2])
 {
     double M = sqrt((Mx * Mx + My * My) + Mz * Mz);
     if (!(E > 0.0)) {                         /* vacuum, reading G7 */
@@ -121,7 +158,7 @@ int oracle_cons2prim(double E, double Mx, double My, double Mz, double R,
     double v = 0.0;
     int it = 0;
     for (it = 0; it < FP_MAXIT; ++it) {       /* PAPER.md:109 fixed point, reading G9 */
-        double P = eos_P(E - Mc * v, R * sqrt(1.0 - v * v), gamma, mass);
+        double P = eos_P(E - Mc * v, R * sqrt(1.0 - v * v), gamma, mass, tab);
         double vnew = Mc / (E + P);
         double d = fabs(vnew - v);
         v = vnew;
@@ -131,13 +168,18 @@ int oracle_cons2prim(double E, double Mx, double My, double Mz, double R,
     if (e < 0.0) { e = 0.0; if (flags) flags[0]++; }
     double n = R * sqrt(1.0 - v * v);
     double praw = (gamma - 1.0) * (e - mass * n);
-    if (praw < 0.0 && flags) flags[1]++;
-    double p = eos_P(e, n, gamma, mass);
+    if (!tab && praw < 0.0 && flags) flags[1]++;
+    double p = eos_P(e, n, gamma, mass, tab);
     out[0] = e; out[1] = p; out[2] = n;
     if (M > 0.0) { out[3] = v * Mx / M; out[4] = v * My / M; out[5] = v * Mz / M; }
     else         { out[3] = out[4] = out[5] = 0.0; }
     out[6] = v;
     return it;
+}
+int oracle_cons2prim(double E, double Mx, double My, double Mz, double R,
+                     double gamma, double mass, double out[7], int flags[2])
+{
+    return oracle_cons2prim_eos(E, Mx, My, Mz, R, gamma, mass, NULL, out, flags);
 }
 
 /* ------------------------------------------------------------ eq. (15) --- */
@@ -223,8 +265,9 @@ static int ghost_index(int j, int N, int bc)
      predictor  0 = R1 (reading G4, the default): half step = eq. (17) alone with lambda/2;
                 1 = R2: half step = the complete kernel with lambda/2, i.e. eq. (17) AND eqs. (18)-(22), which is what
                 Listing 2 suggests (the ordinary prop kernels run after half_cfl).  Radius 6. */
-void oracle_sweep_pencil_ex(int N, double *U[NF], int a, double lambda, double gamma,
-                            double mass, int bc, unsigned long long counts[2], double diff, int predictor)
+void oracle_sweep_pencil_eos(int N, double *U[NF], int a, double lambda, double gamma,
+                             double mass, int bc, unsigned long long counts[2], double diff, int predictor,
+                             const eos_table_t *tab)
 {
     const int g = predictor ? G2 : G;         /* ghost depth */
     const int NE = N + 2 * g;                 /* extended length, j = -g .. N+g-1 at offset +g */
@@ -251,7 +294,7 @@ void oracle_sweep_pencil_ex(int N, double *U[NF], int a, double lambda, double g
     /* 2. time-n primitives on the whole extended pencil */
     for (int i = 0; i < NE; ++i) {
         double o[7];
-        oracle_cons2prim(Ue[0][i], Ue[1][i], Ue[2][i], Ue[3][i], Ue[4][i], gamma, mass, o, NULL);
+        oracle_cons2prim_eos(Ue[0][i], Ue[1][i], Ue[2][i], Ue[3][i], Ue[4][i], gamma, mass, tab, o, NULL);
         v[i] = o[3 + a]; pr[i] = o[1]; pv[i] = o[1] * o[3 + a];
     }
     /* 3. predictor (readings G4, G5): eq. (17) with lambda/2, time-n v and p */
@@ -271,7 +314,7 @@ void oracle_sweep_pencil_ex(int N, double *U[NF], int a, double lambda, double g
     /* 4. half-step primitives, j = -3 .. N+2 */
     for (int i = h_lo; i < h_hi; ++i) {
         double o[7];
-        oracle_cons2prim(Ut[0][i], Ut[1][i], Ut[2][i], Ut[3][i], Ut[4][i], gamma, mass, o, NULL);
+        oracle_cons2prim_eos(Ut[0][i], Ut[1][i], Ut[2][i], Ut[3][i], Ut[4][i], gamma, mass, tab, o, NULL);
         vh[i] = o[3 + a]; ph[i] = o[1]; pvh[i] = o[1] * o[3 + a];
     }
     /* 5. corrector transport: eq. (17) with lambda, half-step v and p, transports U^n;
@@ -294,6 +337,12 @@ void oracle_sweep_pencil_ex(int N, double *U[NF], int a, double lambda, double g
         U[4][j] = Un[4][g + j];
     }
     free(buf);
+}
+
+void oracle_sweep_pencil_ex(int N, double *U[NF], int a, double lambda, double gamma,
+                            double mass, int bc, unsigned long long counts[2], double diff, int predictor)
+{
+    oracle_sweep_pencil_eos(N, U, a, lambda, gamma, mass, bc, counts, diff, predictor, NULL);
 }
 
 /* the default scheme: diff = 1, predictor R1 */
@@ -343,7 +392,21 @@ void oracle_destroy(oracle_t *o)
 {
     if (!o) return;
     for (int f = 0; f < NF; ++f) free(o->U[f]);
+    free((void *)o->tab.p);
     free(o);
+}
+/* Tabled EOS for this grid (copied): p[i + ne*j] at (i e_max/(ne-1), j n_max/(nn-1)); p == NULL: back to the ideal gas */
+int oracle_set_eos_table(oracle_t *o, const double *p, int ne, int nn, double e_max, double n_max)
+{
+    if (!o) return -1;
+    free((void *)o->tab.p); o->tab.p = NULL; o->have_tab = 0;
+    if (!p) return 0;
+    if (ne < 2 || nn < 2 || !(e_max > 0.0) || !(n_max > 0.0)) return -1;
+    double *c = (double *)malloc(sizeof(double) * (size_t)ne * nn);
+    memcpy(c, p, sizeof(double) * (size_t)ne * nn);
+    o->tab.ne = ne; o->tab.nn = nn; o->tab.de = e_max / (ne - 1); o->tab.dn = n_max / (nn - 1); o->tab.p = c;
+    o->have_tab = 1;
+    return 0;
 }
 /* keys: 0 boundary (0 outflow, 1 periodic), 1 EOS mass m, 3 step index, 4 predictor (0 = R1, 1 = R2), 5 diff >= 0 */
 int oracle_set_option(oracle_t *o, int key, double value)
@@ -373,7 +436,7 @@ int oracle_set_state(oracle_t *o, const double *e, const double *n, const double
 #pragma omp parallel for num_threads(g_threads) schedule(static)
     for (long long i = 0; i < nc; ++i) {
         double c[NF];
-        oracle_prim2cons(e[i], n[i], vx[i], vy[i], vz[i], o->gamma, o->mass, c);
+        oracle_prim2cons_eos(e[i], n[i], vx[i], vy[i], vz[i], o->gamma, o->mass, o->have_tab ? &o->tab : NULL, c);
         for (int f = 0; f < NF; ++f) o->U[f][i] = c[f];
     }
     o->have_state = 1;
@@ -419,7 +482,8 @@ static void sweep_grid(oracle_t *o, int a)
             for (int j = 0; j < N; ++j) P[f][j] = o->U[f][base + j * stride[a]];
         }
         unsigned long long cnt[2] = { 0, 0 };
-        oracle_sweep_pencil_ex(N, P, a, o->lambda, o->gamma, o->mass, o->bc, cnt, o->diff, o->predictor);
+        oracle_sweep_pencil_eos(N, P, a, o->lambda, o->gamma, o->mass, o->bc, cnt, o->diff, o->predictor,
+                                o->have_tab ? &o->tab : NULL);
         for (int f = 0; f < NF; ++f)
             for (int j = 0; j < N; ++j) o->U[f][base + j * stride[a]] = P[f][j];
         c0 += cnt[0]; c1 += cnt[1];
@@ -455,8 +519,8 @@ int oracle_get_primitives(oracle_t *o, double *e, double *p, double *n, double *
 #pragma omp parallel for num_threads(g_threads) schedule(static) reduction(+:f0,f1)
     for (long long i = 0; i < nc; ++i) {
         double out[7]; int fl[2] = { 0, 0 };
-        oracle_cons2prim(o->U[0][i], o->U[1][i], o->U[2][i], o->U[3][i], o->U[4][i],
-                         o->gamma, o->mass, out, fl);
+        oracle_cons2prim_eos(o->U[0][i], o->U[1][i], o->U[2][i], o->U[3][i], o->U[4][i],
+                             o->gamma, o->mass, o->have_tab ? &o->tab : NULL, out, fl);
         if (e) e[i] = out[0];
         if (p) p[i] = out[1];
         if (n) n[i] = out[2];

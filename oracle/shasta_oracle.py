@@ -44,6 +44,18 @@ _libs = {}
 _dp = C.POINTER(C.c_double)
 
 
+class EosTable(C.Structure):
+    """eos_table_t of shasta_oracle.c: p[i + ne*j] at (i de, j dn) (reading T1)."""
+    _fields_ = [("ne", C.c_int), ("nn", C.c_int), ("de", C.c_double), ("dn", C.c_double), ("p", _dp)]
+
+
+def make_table(p2d, e_max, n_max):
+    """p2d: array (nn, ne), p2d[j, i] = P(i e_max/(ne-1), j n_max/(nn-1)).  Returns (EosTable, keep-alive array)."""
+    a = np.ascontiguousarray(p2d, dtype=np.float64)
+    nn, ne = a.shape
+    return EosTable(ne, nn, e_max / (ne - 1), n_max / (nn - 1), a.ctypes.data_as(_dp)), a
+
+
 def lib(variant: str = "strict"):
     if variant not in _libs:
         L = C.CDLL(build(variant=variant))
@@ -78,6 +90,12 @@ def lib(variant: str = "strict"):
                                           C.c_double, C.c_int, C.POINTER(C.c_ulonglong)]
         L.oracle_sweep_pencil_ex.argtypes = [C.c_int, C.POINTER(_dp), C.c_int, C.c_double, C.c_double,
                                              C.c_double, C.c_int, C.POINTER(C.c_ulonglong), C.c_double, C.c_int]
+        L.oracle_set_eos_table.argtypes = [C.c_void_p, _dp, C.c_int, C.c_int, C.c_double, C.c_double]
+        L.oracle_eos_table_P.restype = C.c_double
+        L.oracle_eos_table_P.argtypes = [C.POINTER(EosTable), C.c_double, C.c_double]
+        L.oracle_prim2cons_eos.argtypes = [C.c_double] * 7 + [C.POINTER(EosTable), _dp]
+        L.oracle_cons2prim_eos.restype = C.c_int
+        L.oracle_cons2prim_eos.argtypes = [C.c_double] * 7 + [C.POINTER(EosTable), _dp, C.POINTER(C.c_int)]
         L.oracle_advect_pencil.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_int, C.c_int, _dp]
         L.oracle_set_threads(_threads[0])
         _libs[variant] = L
@@ -149,6 +167,23 @@ def cons2prim(E, Mx, My, Mz, R, gamma, mass=0.0):
     return out, it, (fl[0], fl[1])
 
 
+def eos_table_P(tab, e, n):
+    return lib().oracle_eos_table_P(C.byref(tab[0]), e, n)
+
+
+def prim2cons_table(e, n, vx, vy, vz, tab):
+    out = np.zeros(5)
+    lib().oracle_prim2cons_eos(e, n, vx, vy, vz, 4.0 / 3.0, 0.0, C.byref(tab[0]), _p(out))
+    return out
+
+
+def cons2prim_table(E, Mx, My, Mz, R, tab):
+    out = np.zeros(7)
+    fl = (C.c_int * 2)(0, 0)
+    it = lib().oracle_cons2prim_eos(E, Mx, My, Mz, R, 4.0 / 3.0, 0.0, C.byref(tab[0]), _p(out), fl)
+    return out, it, (fl[0], fl[1])
+
+
 def project(E, M):
     m = np.array(M, dtype=np.float64)
     r = lib().oracle_project(E, _p(m))
@@ -182,7 +217,7 @@ class Oracle:
     """Same call sequence as the product's C ABI (include/shasta.h) with host arrays."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, variant="strict",
-                 predictor=R1, diff=1.0):
+                 predictor=R1, diff=1.0, eos_table=None):
         self._L = lib(variant)
         self.shape = (nz, ny, nx)
         self._h = self._L.oracle_create(nx, ny, nz, dx, lam, eos_gamma)
@@ -194,6 +229,10 @@ class Oracle:
             self.set_option(PREDICTOR, predictor)
         if diff != 1.0:
             self.set_option(DIFF, diff)
+        if eos_table is not None:           # (p2d (nn, ne), e_max, n_max)
+            a = np.ascontiguousarray(eos_table[0], dtype=np.float64)
+            self._chk(self._L.oracle_set_eos_table(self._h, _p(a), a.shape[1], a.shape[0], float(eos_table[1]),
+                                                   float(eos_table[2])), "oracle_set_eos_table")
 
     def __del__(self):
         if getattr(self, "_h", None):

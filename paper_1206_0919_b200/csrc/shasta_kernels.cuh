@@ -1045,7 +1045,7 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
                 // primitives of the INPUT state of this group's output cells = the four cells of the previous group's ring
                 // tile; done after the four steps, when only the carried window is alive in registers
                 load_fence();
-#pragma unroll 1
+#pragma unroll
                 for (int c = 0; c < YZ_CH; ++c) {
                     if (c < left) {
                         // momenta in NATURAL order (x, y, z), so that |M|^2 rounds as in the element-wise pass this replaces
