@@ -84,6 +84,15 @@ void shasta_destroy(shasta_t* h);
 /* Options; BOUNDARY, EOS_MASS and PRECISION must be set before shasta_set_state. */
 int shasta_set_option(shasta_t* h, int key, double value);
 
+/* Tabled equation of state (the velocity is found by root finding "to allow
+ * for an easy implementation of a tabled equation of state").  p_host: HOST pointer to ne*nn pressures, e fastest:
+ * p[i + ne*j] = P(e_i, n_j) at the nodes e_i = i e_max/(ne-1), n_j = j n_max/(nn-1).  Between nodes P is bilinear, outside
+ * the table the nearest cell's bilinear form continues (linear extrapolation), and P is floored at 0 (DESIGN.md 3,
+ * reading T1 -- the paper prints no table and no interpolation rule).  The table is copied to the device; it replaces
+ * eos_gamma / SHASTA_EOS_MASS in every cons2prim of the path and in shasta_set_state.  p_host == NULL: back to the analytic
+ * EOS.  Call before shasta_set_state.  The EOS must be causal (0 <= dP/de <= 1) for the velocity root to be unique. */
+int shasta_set_eos_table(shasta_t* h, const double* p_host, int ne, int nn, double e_max, double n_max);
+
 /* Axis order: step s runs sweeps along axes[(3s+k) % n], k = 0,1,2 (0=x,1=y,2=z).  Default: the
  * paper's 18-entry table branch[], i.e. the six permutations.  n % 3 == 0, n <= 63.
  * `axes` is a host pointer. */

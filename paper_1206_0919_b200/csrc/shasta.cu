@@ -29,6 +29,9 @@ struct shasta {
     long long ncell1;       // cells of one event, nx * ny * nz
     int nbatch;             // independent events stacked along z (SHASTA_BATCH); 1 by default
     double dx, lambda, gamma, mass;
+    double* d_tab;          // tabled EOS (row f1): device copy of P at the nodes, e fastest; NULL = analytic EOS
+    int tab_ne, tab_nn;
+    double tab_de, tab_dn;
     double diff;            // factor on the antidiffusive flux; 1 by default
     int cell_path;          // 1 = run the per-cell kernels also for the default scheme (A/B datapoint, tests)
     int predictor;          // 0 = R1 (eq. (17) alone), 1 = R2 (complete kernel at lambda/2): per-cell kernels
@@ -201,7 +204,8 @@ int ensure_stage(shasta_t* h)
 
 // The EOS_GAMMA kernels (closed-form fast cons2prim, shasta_kernels.cuh c2p_fast_y) need m = 0 and Gamma <= 5/3
 // (two frozen-slope Newton steps suffice while (Gamma-1)/(2-Gamma) <= 2); everything else runs the EOS_MASS kernels.
-bool use_general_eos(const shasta_t* h) { return h->mass != 0.0 || h->gamma > 5.0 / 3.0 + 1e-12; }
+bool use_general_eos(const shasta_t* h) { return h->d_tab || h->mass != 0.0 || h->gamma > 5.0 / 3.0 + 1e-12; }
+int eos_mode(const shasta_t* h) { return h->d_tab ? EOS_TABLE : (use_general_eos(h) ? EOS_MASS : EOS_GAMMA); }
 
 template <typename T>
 Consts<T> make_consts(const shasta_t* h)
@@ -219,6 +223,10 @@ Consts<T> make_consts(const shasta_t* h)
     k.d.omd = 1.0 - 1e-12;
     k.d.omd2 = (1.0 - 1e-12) * (1.0 - 1e-12);
     k.d.mass = h->mass;
+    k.d.tab = h->d_tab;
+    k.d.ne = h->tab_ne; k.d.nn = h->tab_nn;
+    k.d.ide = h->d_tab ? 1.0 / h->tab_de : 0.0;
+    k.d.idn = h->d_tab ? 1.0 / h->tab_dn : 0.0;
     return k;
 }
 
@@ -227,14 +235,20 @@ Consts<T> make_consts(const shasta_t* h)
 template <typename T>
 __global__ void prim2cons_kernel(long long n, const double* __restrict__ e, const double* __restrict__ nd,
                                  const double* __restrict__ vx, const double* __restrict__ vy,
-                                 const double* __restrict__ vz, double gm1, double mass,
+                                 const double* __restrict__ vz, EosD kd,
                                  T* E, T* Mx, T* My, T* Mz, T* R, T* pe, T* pp, T* pn, T* pvx, T* pvy, T* pvz)
 {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
         const double ee = e[i], nn = nd[i], ax = vx[i], ay = vy[i], az = vz[i];
-        double p = gm1 * (ee - mass * nn);
-        p = p > 0.0 ? p : 0.0;
+        double p;
+        if (kd.tab) {                                   // tabled EOS (reading T1)
+            double a_, b_;
+            eos_table_eval(kd, ee, nn, p, a_, b_);
+        } else {
+            p = kd.gm1 * (ee - kd.mass * nn);
+            p = p > 0.0 ? p : 0.0;
+        }
         const double v2 = fma(ax, ax, fma(ay, ay, az * az));
         const double g2 = 1.0 / (1.0 - v2);
         const double w = (ee + p) * g2;
@@ -487,14 +501,18 @@ int launch_sweep_e(shasta_t* h, int axis, int emit, cudaStream_t st)
 
 int launch_sweep_raw(shasta_t* h, int axis, int emit, cudaStream_t st)
 {
-    const bool general = use_general_eos(h);
+    const int eos = eos_mode(h);
     if (h->predictor || h->cell_path) {
         if (h->precision != 64) return fail(h, SHASTA_ESTATE, "the per-cell kernels (R2 predictor) run in fp64 only");
-        return general ? launch_cell_sweep<EOS_MASS>(h, axis, emit != 0, st) : launch_cell_sweep<EOS_GAMMA>(h, axis, emit != 0, st);
+        if (eos == EOS_TABLE) return launch_cell_sweep<EOS_TABLE>(h, axis, emit != 0, st);
+        return eos == EOS_MASS ? launch_cell_sweep<EOS_MASS>(h, axis, emit != 0, st) : launch_cell_sweep<EOS_GAMMA>(h, axis, emit != 0, st);
     }
-    if (h->precision == 64)
-        return general ? launch_sweep_e<double, EOS_MASS>(h, axis, emit, st) : launch_sweep_e<double, EOS_GAMMA>(h, axis, emit, st);
-    return general ? launch_sweep_e<float, EOS_MASS>(h, axis, emit, st) : launch_sweep_e<float, EOS_GAMMA>(h, axis, emit, st);
+    if (h->precision == 64) {
+        if (eos == EOS_TABLE) return launch_sweep_e<double, EOS_TABLE>(h, axis, emit, st);
+        return eos == EOS_MASS ? launch_sweep_e<double, EOS_MASS>(h, axis, emit, st) : launch_sweep_e<double, EOS_GAMMA>(h, axis, emit, st);
+    }
+    if (eos == EOS_TABLE) return launch_sweep_e<float, EOS_TABLE>(h, axis, emit, st);
+    return eos == EOS_MASS ? launch_sweep_e<float, EOS_MASS>(h, axis, emit, st) : launch_sweep_e<float, EOS_GAMMA>(h, axis, emit, st);
 }
 
 template <typename T>
@@ -503,7 +521,11 @@ int refresh_prims_t(shasta_t* h, cudaStream_t st)
     void** U = h->U[h->cur];
     const int g = ew_grid(h, 256);
     const Consts<T> k = make_consts<T>(h);
-    if (use_general_eos(h))
+    if (eos_mode(h) == EOS_TABLE)
+        cons2prim_kernel<T, EOS_TABLE><<<g, 256, 0, st>>>(h->ncell, k, (T*)U[0], (T*)U[1], (T*)U[2], (T*)U[3],
+            (T*)U[4], (T*)h->prim[0], (T*)h->prim[1], (T*)h->prim[2], (T*)h->prim[3], (T*)h->prim[4],
+            (T*)h->prim[5], h->d_counts);
+    else if (use_general_eos(h))
         cons2prim_kernel<T, EOS_MASS><<<g, 256, 0, st>>>(h->ncell, k, (T*)U[0], (T*)U[1], (T*)U[2], (T*)U[3],
             (T*)U[4], (T*)h->prim[0], (T*)h->prim[1], (T*)h->prim[2], (T*)h->prim[3], (T*)h->prim[4],
             (T*)h->prim[5], h->d_counts);
@@ -682,6 +704,7 @@ void shasta_destroy(shasta_t* h)
         for (int f = 0; f < NF; ++f) cudaFree(h->U[b][f]);
     for (int q = 0; q < 6; ++q) cudaFree(h->prim[q]);
     cudaFree(h->stage);
+    cudaFree(h->d_tab);
     cudaFree(h->d_yzmaps);
     cudaFree(h->d_xmaps);
     cudaFree(h->d_counts);
@@ -762,6 +785,26 @@ int shasta_set_option(shasta_t* h, int key, double value)
     }
 }
 
+int shasta_set_eos_table(shasta_t* h, const double* p_host, int ne, int nn, double e_max, double n_max)
+{
+    if (!h) return SHASTA_EINVAL;
+    drop_graphs(h);
+    if (!p_host) {                                       // back to the analytic EOS
+        if (h->d_tab) { CK(cudaDeviceSynchronize()); cudaFree(h->d_tab); h->d_tab = nullptr; }
+        h->prims_valid = false;
+        return 0;
+    }
+    if (ne < 2 || nn < 2 || (long long)ne * nn > (1LL << 26)) return fail(h, SHASTA_EINVAL, "shasta_set_eos_table: need 2 <= ne, nn and ne*nn <= 2^26");
+    if (!(e_max > 0.0) || !(n_max > 0.0)) return fail(h, SHASTA_EINVAL, "shasta_set_eos_table: e_max and n_max must be > 0");
+    if (h->d_tab) { CK(cudaDeviceSynchronize()); cudaFree(h->d_tab); h->d_tab = nullptr; }
+    CK(cudaMalloc(&h->d_tab, sizeof(double) * (size_t)ne * nn));
+    CK(cudaMemcpy(h->d_tab, p_host, sizeof(double) * (size_t)ne * nn, cudaMemcpyHostToDevice));
+    h->tab_ne = ne; h->tab_nn = nn;
+    h->tab_de = e_max / (ne - 1); h->tab_dn = n_max / (nn - 1);
+    h->prims_valid = false;
+    return 0;
+}
+
 int shasta_set_sweep_table(shasta_t* h, const int* axes, int n)
 {
     if (!h) return SHASTA_EINVAL;
@@ -786,11 +829,11 @@ int shasta_set_state(shasta_t* h, const double* e, const double* n, const double
     void** U = h->U[0];
     const int g = ew_grid(h, 256);
     if (h->precision == 64)
-        prim2cons_kernel<double><<<g, 256, 0, st>>>(h->ncell, e, n, vx, vy, vz, h->gamma - 1.0, h->mass,
+        prim2cons_kernel<double><<<g, 256, 0, st>>>(h->ncell, e, n, vx, vy, vz, make_consts<double>(h).d,
             (double*)U[0], (double*)U[1], (double*)U[2], (double*)U[3], (double*)U[4], (double*)h->prim[0],
             (double*)h->prim[1], (double*)h->prim[2], (double*)h->prim[3], (double*)h->prim[4], (double*)h->prim[5]);
     else
-        prim2cons_kernel<float><<<g, 256, 0, st>>>(h->ncell, e, n, vx, vy, vz, h->gamma - 1.0, h->mass,
+        prim2cons_kernel<float><<<g, 256, 0, st>>>(h->ncell, e, n, vx, vy, vz, make_consts<double>(h).d,
             (float*)U[0], (float*)U[1], (float*)U[2], (float*)U[3], (float*)U[4], (float*)h->prim[0],
             (float*)h->prim[1], (float*)h->prim[2], (float*)h->prim[3], (float*)h->prim[4], (float*)h->prim[5]);
     CK(cudaGetLastError());

@@ -35,6 +35,7 @@ constexpr int NF = 5;       // E, M_par, M_perp1, M_perp2, R
 constexpr int GH = 4;       // ghost depth = dependency radius of one sweep
 constexpr int EOS_GAMMA = 0;    // p = (Gamma-1) e            (m = 0): closed-form velocity
 constexpr int EOS_MASS = 1;     // p = (Gamma-1)(e - m n)     (m > 0): safeguarded Newton
+constexpr int EOS_TABLE = 2;    // p = bilinear table P(e, n) (reading T1): the same safeguarded Newton
 
 // EOS / cons2prim constants.  cons2prim, the causality projection and the primitive output ALWAYS run in
 // fp64, also on the fp32 storage path (the paper's own plan: "double precision for ... the calculation of
@@ -48,7 +49,31 @@ struct EosD {
     double omd;     // 1 - delta, delta = 1e-12 (reading G7)
     double omd2;    // (1 - delta)^2
     double mass;    // m
+    // tabled EOS (EOS_TABLE, reading T1): P at nodes (i de, j dn), i < ne, j < nn, e fastest; device pointer
+    const double* tab;
+    int ne, nn;
+    double ide, idn;    // 1/de, 1/dn
 };
+
+// P(e, n) of the table and its two slopes in the cell that holds (e, n): bilinear between nodes, the nearest cell's bilinear
+// form outside the table (linear continuation), floored at 0 (then the slopes are 0 too).  Four read-only loads (L1/L2:
+// neighbouring cells of the grid hit the same table lines).
+__device__ __forceinline__ void eos_table_eval(const EosD& k, double e, double n, double& P, double& Pe, double& Pn)
+{
+    const double xe = e * k.ide, xn = n * k.idn;
+    const int i = min(max(__double2int_rd(xe), 0), k.ne - 2);
+    const int j = min(max(__double2int_rd(xn), 0), k.nn - 2);
+    const double te = xe - (double)i, tn = xn - (double)j;
+    const double* q = k.tab + i + (long long)k.ne * j;
+    const double p00 = __ldg(q), p10 = __ldg(q + 1), p01 = __ldg(q + k.ne), p11 = __ldg(q + k.ne + 1);
+    const double d0 = p10 - p00, d1 = p11 - p01;
+    const double p0 = fma(te, d0, p00), p1 = fma(te, d1, p01);
+    const double praw = fma(tn, p1 - p0, p0);
+    const bool pos = praw > 0.0;
+    P = pos ? praw : 0.0;
+    Pe = pos ? fma(tn, d1 - d0, d0) * k.ide : 0.0;
+    Pn = pos ? (p1 - p0) * k.idn : 0.0;
+}
 
 template <typename T>
 struct Consts {
@@ -229,7 +254,13 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
         double v;
         {
             const double w2h = fma(-hi, hi, double(1));
-            const double Ph = fmax(k.gm1 * ((E - Mabs * hi) - mR * (w2h * fast_rsqrt(w2h))), double(0));
+            double Ph;
+            if (EOS == EOS_TABLE) {
+                double a_, b_;
+                eos_table_eval(k, E - Mabs * hi, R * (w2h * fast_rsqrt(w2h)), Ph, a_, b_);
+            } else {
+                Ph = fmax(k.gm1 * ((E - Mabs * hi) - mR * (w2h * fast_rsqrt(w2h))), double(0));
+            }
             v = fmin(fmax(Mabs * fast_rcp(E + Ph), lo), hi);
         }
         for (int it = 0; it < 48; ++it) {
@@ -239,12 +270,22 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
             const double w2 = fma(-v, v, double(1));
             const double rw = fast_rsqrt(w2);
             const double w = w2 * rw;
-            const double praw = k.gm1 * ((E - Mabs * v) - mR * w);
-            const bool pos = praw > double(0);
-            const double P = pos ? praw : double(0);
-            const double dP = pos ? k.gm1 * (mR * v * rw - Mabs) : double(0);
+            double P, dP;
+            if (EOS == EOS_TABLE) {
+                // P(e(v), n(v)), e = E - |M| v, n = R sqrt(1 - v^2); dP/dv from the slopes of the table cell (piecewise
+                // constant: a kink at a cell border costs the Newton step at most the bisection safeguard below)
+                double Pe, Pn;
+                eos_table_eval(k, E - Mabs * v, R * w, P, Pe, Pn);
+                dP = -(Mabs * Pe) - (R * v * rw) * Pn;
+            } else {
+                const double praw = k.gm1 * ((E - Mabs * v) - mR * w);
+                const bool pos = praw > double(0);
+                P = pos ? praw : double(0);
+                dP = pos ? k.gm1 * (mR * v * rw - Mabs) : double(0);
+            }
             const double g = fma(v, E + P, -Mabs);
-            const double dg = fma(v, dP, E + P);
+            double dg = fma(v, dP, E + P);
+            if (EOS == EOS_TABLE) dg = dg > double(0.25) * E ? dg : E;      // a table may be steep: keep the Newton slope sane
             if (g > double(0)) hi = v; else lo = v;
             double vn = v - g * fast_rcp(dg);
             if (!(vn >= lo && vn <= hi)) vn = double(0.5) * (lo + hi);
@@ -258,9 +299,14 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
         if (eraw < double(0)) o.fl |= 1;
         o.e = fmax(eraw, double(0));
         const double n = (o.w > double(1e-300)) ? R * fast_sqrt(o.w) : double(0);
-        const double praw = k.gm1 * (o.e - k.mass * n);
-        if (praw < double(0)) o.fl |= 2;
-        o.p = fmax(praw, double(0));
+        if (EOS == EOS_TABLE) {
+            double a_, b_;
+            eos_table_eval(k, o.e, n, o.p, a_, b_);
+        } else {
+            const double praw = k.gm1 * (o.e - k.mass * n);
+            if (praw < double(0)) o.fl |= 2;
+            o.p = fmax(praw, double(0));
+        }
         o.y = (M2 > double(1e-300)) ? v * fast_rsqrt(M2) : double(0);
     }
     if (vac) { o.y = double(0); o.e = double(0); o.p = double(0); o.w = double(0); o.fl = 0; }   // n = R sqrt(w) = 0 (reading G7)

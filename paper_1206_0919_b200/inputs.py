@@ -147,3 +147,21 @@ CONFIGS = {
     "shock_tube": shock_tube, "fireball": fireball, "spherical_riemann": spherical_riemann,
     "hotspots": hotspots, "hotspots_crop": hotspots_crop, "slabs": slabs,
 }
+
+
+# ------------------------------------------------------------------ synthetic tabled equations of state (row f1)
+def eos_table(kind="soft", ne=193, nn=49, e_max=12.0, n_max=4.0, gamma=5.0 / 3.0, mass=1.0):
+    """A pressure table P(e_i, n_j), e_i = i e_max/(ne-1), n_j = j n_max/(nn-1), as (p2d (nn, ne), e_max, n_max): the
+    argument of shasta_set_eos_table and of the oracle's eos_table option.  No physical table is in the container
+    (PAPER.md:36 only names "non analytic equations of state"); two synthetic ones stand in:
+      "ideal"  the ideal gas (gamma-1)(e - m n) sampled on the grid (bilinear interpolation returns it exactly),
+      "soft"   a smooth causal crossover, p = e/3 (1 - 0.25 exp(-(e-2)^2/2)) + 0.05 n^2/(1+n)  (0 < dp/de < 0.45)."""
+    e = np.linspace(0.0, e_max, ne)[None, :]
+    n = np.linspace(0.0, n_max, nn)[:, None]
+    if kind == "ideal":
+        p = (gamma - 1.0) * (e - mass * n)
+    elif kind == "soft":
+        p = e / 3.0 * (1.0 - 0.25 * np.exp(-0.5 * (e - 2.0) ** 2)) + 0.05 * n * n / (1.0 + n) + 0.0 * e
+    else:
+        raise ValueError(kind)
+    return np.ascontiguousarray(p, dtype=np.float64), float(e_max), float(n_max)

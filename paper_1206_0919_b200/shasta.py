@@ -19,7 +19,7 @@ BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 
 # every symbol include/shasta.h declares
 SYMBOLS = (
-    "shasta_create", "shasta_destroy", "shasta_set_option", "shasta_set_sweep_table", "shasta_set_state",
+    "shasta_create", "shasta_destroy", "shasta_set_option", "shasta_set_eos_table", "shasta_set_sweep_table", "shasta_set_state",
     "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_step", "shasta_sweep",
     "shasta_get_primitives", "shasta_get_primitives_host", "shasta_conserved_totals", "shasta_diagnostics",
     "shasta_launch_count", "shasta_graph_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
@@ -43,6 +43,7 @@ def load():
     L.shasta_destroy.argtypes = [_vp]
     L.shasta_destroy.restype = None
     L.shasta_set_option.argtypes = [_vp, C.c_int, C.c_double]
+    L.shasta_set_eos_table.argtypes = [_vp, _dp, C.c_int, C.c_int, C.c_double, C.c_double]
     L.shasta_set_sweep_table.argtypes = [_vp, C.POINTER(C.c_int), C.c_int]
     L.shasta_set_state.argtypes = [_vp] + [_dp] * 5 + [_vp]
     L.shasta_set_state_host.argtypes = [_vp] + [_dp] * 5 + [_vp]
@@ -100,7 +101,7 @@ class Shasta:
     """One solver handle = shasta_create ... shasta_destroy.  Method names follow the C ABI."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, precision=64,
-                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0, batch=1, graph=None):
+                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0, batch=1, graph=None, eos_table=None):
         L = load()
         self._L = L
         self._h = _vp()
@@ -131,6 +132,8 @@ class Shasta:
             self.set_option(BATCH, self.batch)
         if graph is not None:
             self.set_option(GRAPH, graph)
+        if eos_table is not None:
+            self.set_eos_table(*eos_table)
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
@@ -145,6 +148,17 @@ class Shasta:
 
     def set_option(self, key, value):
         self._chk(self._L.shasta_set_option(self._h, key, float(value)), "shasta_set_option")
+
+    def set_eos_table(self, p2d, e_max, n_max):
+        """p2d: CPU float64 tensor or array of shape (nn, ne), p2d[j, i] = P(i e_max/(ne-1), j n_max/(nn-1)); None = analytic."""
+        import torch
+        if p2d is None:
+            self._chk(self._L.shasta_set_eos_table(self._h, None, 0, 0, 0.0, 0.0), "shasta_set_eos_table")
+            return
+        t = torch.as_tensor(p2d, dtype=torch.float64).contiguous().cpu()
+        nn, ne = t.shape
+        self._chk(self._L.shasta_set_eos_table(self._h, C.c_void_p(t.data_ptr()), ne, nn, float(e_max), float(n_max)),
+                  "shasta_set_eos_table")
 
     def set_sweep_table(self, axes):
         a = (C.c_int * len(axes))(*axes)

@@ -273,6 +273,36 @@ def test_cuda_graph_cycles_same_bits(shape):
     assert res[0][1] == res[1][1], "launch_count counts the kernels inside the replayed graphs"
 
 
+# ------------------------------------------------------------------ f1: tabled EOS (oracle pins: test_oracle_eos_table.py)
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("kind", ["soft", "ideal"])
+@pytest.mark.parametrize("shape", [(37, 19, 23), (64, 12, 10)])
+def test_tabled_eos_kernel_level(oracle, bc, kind, shape):
+    # shasta_set_eos_table (reading T1): every cons2prim of the path and set_state read P from
+    # the bilinear table.  "soft": a nonlinear synthetic EOS; "ideal": the m = 1 ideal gas as a table, which must ALSO
+    # equal the analytic m = 1 run (bilinear interpolation is exact on it)
+    tab = inputs.eos_table(kind)
+    c = inputs.random_state(*shape, seed=70 + bc, kind="rough", gamma=5.0 / 3.0, mass=0.0, boundary=bc)
+    ref, _ = parity.run_oracle(oracle, c, steps=6, eos_table=tab)
+    got, _ = parity.run_gpu(c, steps=6, eos_table=tab)
+    assert_kernel_parity(got, ref, f"tabled EOS {kind} shape {shape} bc {bc}", tol_cons=1e-11, tol_prim=1e-11)
+    if kind == "ideal":
+        ca = dict(c, mass=1.0)
+        ana, _ = parity.run_gpu(ca, steps=6)
+        parity.assert_parity(got, ana, 1e-10, label="table of the ideal gas vs the analytic kernels")
+
+
+def test_tabled_eos_cell_path_and_fp32(oracle):
+    tab = inputs.eos_table("soft")
+    c = inputs.random_state(24, 20, 28, seed=9, kind="smooth", gamma=5.0 / 3.0)
+    ref, _ = parity.run_oracle(oracle, c, steps=2, eos_table=tab)
+    got, _ = parity.run_gpu(c, steps=2, eos_table=tab, cell_path=1)
+    assert_kernel_parity(got, ref, "tabled EOS, per-cell kernels", tol_cons=1e-11, tol_prim=1e-11)
+    got32, _ = parity.run_gpu(c, steps=2, eos_table=tab, precision=32)
+    for k, (emax, el1) in parity.field_errors(got32, ref).items():
+        assert emax <= 2e-5 and el1 <= 2e-6, (k, emax, el1)
+
+
 def test_host_buffer_entry_points(oracle):
     c = inputs.random_state(21, 17, 13, seed=8, kind="smooth")
     ref, _ = parity.run_oracle(oracle, c, steps=2)
