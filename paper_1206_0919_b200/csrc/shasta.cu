@@ -347,7 +347,7 @@ int ew_grid(const shasta_t* h, int threads)
 int auto_segment(const shasta_t* h, int axis, int N, long long base)
 {
     if (h->seg_override > 0) return h->seg_override < N ? h->seg_override : N;
-    const long long slots = 2LL * h->sm_count;                     // CTAs resident at once
+    const long long slots = (long long)(eos_mode(h) == EOS_GAMMA ? 2 : GEN_CTAS) * h->sm_count;     // CTAs resident at once
     // base = CTAs per layer of segments
     const long long max_nseg = N / 16 > 1 ? N / 16 : 1;            // segments not shorter than 16 cells
     long long nseg = 1;

@@ -313,6 +313,87 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
     return o;
 }
 
+// The same solve as the non-Gamma branch of cons2prim_general, cut into init / iter / finish so that the in-sweep cons2prim
+// of TWO cells can run as one loop with two independent dependency chains (c2p_group below).  The Newton iteration of one
+// cell is a serial chain of ~25 dependent fp64 operations per step; with one cell at a time the producer warp issued an
+// instruction every ~7 cycles (round 1: config 3 at a third of the Gamma-law speed).  Same formulas, same bracket, same
+// tolerance; a cell that has converged keeps iterating at its fixed point until its partner (and the warp) is done.
+template <int EOS>
+struct Newt {
+    double E, Mabs, R, mR, v, lo, hi, M1, M2;
+    bool vac;
+    __device__ __forceinline__ void init(const EosD& k, const double (&u)[NF])
+    {
+        init_em(k, u[0], u[1], fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3])), u[4]);
+    }
+    // from E, M_par, |M|^2 and R: all the solve needs (what the producer hands to the consumer for S3)
+    __device__ __forceinline__ void init_em(const EosD& k, double E_, double M1_, double M2_, double R_)
+    {
+        E = E_; M1 = M1_; M2 = M2_; R = R_;
+        vac = !(E > 0.0);
+        if (vac) { E = 1.0; M1 = 0.0; M2 = 0.0; }
+        const double lim = k.omd * E;
+        const double lim2 = lim * lim;
+        const double Mq = M2 > lim2 ? lim2 : M2;
+        const bool moving = Mq > 1e-300;
+        Mabs = moving ? Mq * fast_rsqrt(Mq) : 0.0;
+        lo = 0.0;
+        hi = fmin(Mabs * fast_rcp(E), k.omd);
+        mR = k.mass * R;
+        const double w2h = fma(-hi, hi, 1.0);
+        double Ph;
+        if (EOS == EOS_TABLE) {
+            double a_, b_;
+            eos_table_eval(k, E - Mabs * hi, R * (w2h * fast_rsqrt(w2h)), Ph, a_, b_);
+        } else {
+            Ph = fmax(k.gm1 * ((E - Mabs * hi) - mR * (w2h * fast_rsqrt(w2h))), 0.0);
+        }
+        v = fmin(fmax(Mabs * fast_rcp(E + Ph), lo), hi);
+    }
+    __device__ __forceinline__ double iter(const EosD& k)
+    {
+        const double w2 = fma(-v, v, 1.0);
+        const double rw = fast_rsqrt3(w2);              // 2^-58: w enters P, which fixes the root
+        const double w = w2 * rw;
+        double P, dP;
+        if (EOS == EOS_TABLE) {
+            double Pe, Pn;
+            eos_table_eval(k, E - Mabs * v, R * w, P, Pe, Pn);
+            dP = -(Mabs * Pe) - (R * v * rw) * Pn;
+        } else {
+            const double praw = k.gm1 * ((E - Mabs * v) - mR * w);
+            const bool pos = praw > 0.0;
+            P = pos ? praw : 0.0;
+            dP = pos ? k.gm1 * (mR * v * rw - Mabs) : 0.0;
+        }
+        const double g = fma(v, E + P, -Mabs);
+        double dg = fma(v, dP, E + P);
+        if (EOS == EOS_TABLE) dg = dg > 0.25 * E ? dg : E;
+        if (g > 0.0) hi = v; else lo = v;
+        double vn = v - g * rcp64h(dg);                 // slope to 2^-20 is enough: the step it scales goes to 0
+        if (!(vn >= lo && vn <= hi)) vn = 0.5 * (lo + hi);
+        const double dv = fabs(vn - v);
+        v = vn;
+        return dv;
+    }
+    // v_par = M_par v / |M| and p of the converged state (vacuum: 0, 0)
+    __device__ __forceinline__ void finish(const EosD& k, double& vpar, double& p) const
+    {
+        const double w = fmax(fma(-v, v, 1.0), 0.0);
+        const double e = fmax(fma(-Mabs, v, E), 0.0);
+        const double n = (w > 1e-300) ? R * fast_sqrt(w) : 0.0;
+        if (EOS == EOS_TABLE) {
+            double a_, b_;
+            eos_table_eval(k, e, n, p, a_, b_);
+        } else {
+            p = fmax(k.gm1 * (e - k.mass * n), 0.0);
+        }
+        const double y = (M2 > 1e-300) ? v * fast_rsqrt(M2) : 0.0;
+        vpar = M1 * y;
+        if (vac) { vpar = 0.0; p = 0.0; }
+    }
+};
+
 // The EOS_GAMMA kernels have NO out-of-line path: vacuum / non-positive E (high word <= 0) is a two-line inline
 // branch (all primitives 0, M = 0), and the host instantiates them only for Gamma <= 5/3, where the frozen-slope
 // Newton of c2p_fast_y converges in two steps (larger Gamma runs the EOS_MASS kernels with m = 0).  The causality clamp Mc = min(|M|, (1-delta) E) stays inline: Mc^2 is a
@@ -422,10 +503,24 @@ __device__ __forceinline__ void c2p_group(const Consts<T>& k, T (&c0)[NF], T (&c
             if (__any_sync(0xffffffffu, rare[3])) c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
         }
     } else {
-        c2p_sweep<T, EOS>(k, c0, v[0], p[0]);
-        c2p_sweep<T, EOS>(k, c1, v[1], p[1]);
-        c2p_sweep<T, EOS>(k, c2, v[2], p[2]);
-        c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
+        // general EOS: two cells per Newton loop (see Newt), the warp leaves a loop together
+#define SHK_C2P_PAIR(J, CA, CB)                                                                 \
+        {                                                                                       \
+            double ua[NF], ub[NF], va, pa, vb, pb;                                              \
+            _Pragma("unroll") for (int f = 0; f < NF; ++f) { ua[f] = (double)CA[f]; ub[f] = (double)CB[f]; } \
+            Newt<EOS> na, nb;                                                                   \
+            na.init(k.d, ua); nb.init(k.d, ub);                                                 \
+            for (int it = 0; it < 48; ++it) {                                                   \
+                const double da = na.iter(k.d), db = nb.iter(k.d);                              \
+                if (__all_sync(0xffffffffu, fmax(da, db) <= 1e-15)) break;                      \
+            }                                                                                   \
+            na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);                                     \
+            v[J] = (T)va; p[J] = (T)pa; v[J + 1] = (T)vb; p[J + 1] = (T)pb;                     \
+        }
+        SHK_C2P_PAIR(0, c0, c1)
+        reload();                           // brings c2, c3 only now (ring / scratch): two cells alive at a time
+        SHK_C2P_PAIR(2, c2, c3)
+#undef SHK_C2P_PAIR
     }
 }
 
@@ -628,48 +723,6 @@ struct Producer {
         eps1 = epsh2 = fE[0] = fE[1] = fM[0] = fM[1] = gE[0] = gE[1] = gM[0] = gM[1] = T(0);
     }
 
-    // consumes U^n at the front cell i (u0) and at cell i-1 (u1: re-read from the ring by the caller, or the
-    // previous front cell still in registers -- never carried, so no hand-down moves);
-    // msg = {a_c, b_c, sE, sM} for the consumer's step i
-    template <int PH>
-    __device__ __forceinline__ void step(const Consts<T>& k, const T (&u1)[NF], const T (&u0)[NF], T (&msg)[4])
-    {
-        constexpr int S2 = PH & 1;              // time-n scalars _2 (new _0 takes its slot)
-        constexpr int G3 = (PH + 1) & 1;        // half-step scalars _3 (new _1 takes its slot)
-        T v0, p0;
-        c2p_sweep<T, EOS>(k, u0, v0, p0);                                   // S1
-        const T eps0 = k.hlam * v0;
-        const T fE0 = p0 * v0;
-        T ut[NF];
-        ut[NF - 1] = T(0);
-        {                                                                   // S2
-            const T q = (T(0.5) - eps1) * fast_rcp(T(1) + (eps0 - eps1));   // Q+_1, eq. (15)
-            const T a = T(0.5) - q, b = (T(0.5) * q) * q;
-#pragma unroll
-            for (int f = 0; f < NP; ++f) {
-                const T d = u0[f] - u1[f];                                  // eq. (16)
-                const T fl = t_fma(a, u1[f], -(b * d));
-                ut[f] = u1[f] - (fl - ft[f]);
-                ft[f] = fl;
-            }
-            ut[0] = t_fma(-k.qlam, fE0 - fE[S2], ut[0]);
-            ut[1] = t_fma(-k.qlam, p0 - fM[S2], ut[1]);
-        }
-        T vh1, ph;
-        c2p_sweep<T, EOS>(k, ut, vh1, ph);                                  // S3
-        const T epsh1 = k.lam * vh1;
-        const T gE1 = ph * vh1;
-        {                                                                   // geometry + sources of S4
-            const T q = (T(0.5) - epsh2) * fast_rcp(T(1) + (epsh1 - epsh2));
-            msg[0] = T(0.5) - q;
-            msg[1] = (T(0.5) * q) * q;
-            msg[2] = -k.hlam * (gE1 - gE[G3]);
-            msg[3] = -k.hlam * (ph - gM[G3]);
-        }
-        eps1 = eps0; fE[S2] = fE0; fM[S2] = p0;
-        epsh2 = epsh1; gE[G3] = gE1; gM[G3] = ph;
-    }
-
     // One hand-over group = four march steps with front cells c1..c4 (c0 = the cell before them), arranged in PHASES:
     // S1 of the four cells, S2 of the four cells, S3 of the four cells, geometry -- the same arithmetic as four step<PH>()
     // calls (identical bits), but each cons2prim phase is four INDEPENDENT chains behind one rare-path vote (c2p_group).
@@ -683,21 +736,17 @@ struct Producer {
     template <typename L>
     __device__ __forceinline__ void group(const Consts<T>& k, const L& ld, T* scr, T (&msg)[4][4])
     {
-        if constexpr (EOS != EOS_GAMMA) {
-            T c0[NF], c1[NF], c2[NF], c3[NF], c4[NF];
-            ld.first(c0, c1, c2);
-            ld.second(c3, c4);
-            step<0>(k, c0, c1, msg[0]);
-            step<1>(k, c1, c2, msg[1]);
-            step<2>(k, c2, c3, msg[2]);
-            step<3>(k, c3, c4, msg[3]);
-        } else {
+        {
             T v[4], p[4];
             {
                 T c0[NF], c1[NF], c2[NF], c3[NF], c4[NF];
                 ld.first(c0, c1, c2);
-                ld.second(c3, c4);
-                c2p_group<T, EOS>(k, c1, c2, c3, c4, v, p, [&]() { load_fence(); ld.first(c0, c1, c2); ld.second(c3, c4); });    // S1
+                if (EOS == EOS_GAMMA) {
+                    ld.second(c3, c4);
+                    c2p_group<T, EOS>(k, c1, c2, c3, c4, v, p, [&]() { load_fence(); ld.first(c0, c1, c2); ld.second(c3, c4); });    // S1
+                } else {
+                    c2p_group<T, EOS>(k, c1, c2, c3, c4, v, p, [&]() { load_fence(); ld.second(c3, c4); });
+                }
             }
             T eps[5], pv[6], pp[6];
             eps[0] = eps1; pv[0] = fE[0]; pv[1] = fE[1]; pp[0] = fM[0]; pp[1] = fM[1];
@@ -714,11 +763,13 @@ struct Producer {
                     ut[J][f] = UL[f] - (fl - ft[f]);                                            \
                     ft[f] = fl;                                                                 \
                 }                                                                               \
-                ut[J][NF - 1] = T(0);                                                           \
+                if (NP < NF) ut[J][NF - 1] = T(0);                                              \
                 ut[J][0] = t_fma(-k.qlam, pv[J + 2] - pv[J], ut[J][0]);                         \
                 ut[J][1] = t_fma(-k.qlam, pp[J + 2] - pp[J], ut[J][1]);                         \
-                store2(scr + 128 * J, ut[J][0], ut[J][1]);                                      \
-                store2(scr + 128 * J + 64, ut[J][2], ut[J][3]);                                 \
+                if (EOS == EOS_GAMMA) {             /* parked for the rare path of S3 */             \
+                    store2(scr + 128 * J, ut[J][0], ut[J][1]);                                  \
+                    store2(scr + 128 * J + 64, ut[J][2], ut[J][3]);                             \
+                }                                                                               \
             }
             {                                                                                   // S2
                 T c0[NF], c1[NF], c2[NF], c3[NF], c4[NF];
@@ -731,6 +782,18 @@ struct Producer {
             }
 #undef SHK_PRED
             eps1 = eps[4]; fE[0] = pv[4]; fE[1] = pv[5]; fM[0] = pp[4]; fM[1] = pp[5];
+            if constexpr (EOS != EOS_GAMMA) {
+                // general EOS: S3 and the geometry run in the CONSUMER (HalfStep below): the two Newton solves of a cell
+                // are split between the two warps of the pair.  The message is what S3 needs: E~, M~_par, |M~|^2, R~.
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    msg[j][0] = ut[j][0];
+                    msg[j][1] = ut[j][1];
+                    msg[j][2] = (T)fma((double)ut[j][1], (double)ut[j][1], fma((double)ut[j][2], (double)ut[j][2], (double)ut[j][3] * (double)ut[j][3]));
+                    msg[j][3] = ut[j][NF - 1];
+                }
+                return;
+            }
             T vh[4], ph[4];
             c2p_group<T, EOS>(k, ut[0], ut[1], ut[2], ut[3], vh, ph, [&]() {           // S3
                 load_fence();
@@ -755,6 +818,48 @@ struct Producer {
             }
             epsh2 = eh[4]; gE[0] = gv[4]; gE[1] = gv[5]; gM[0] = gp[4]; gM[1] = gp[5];
         }
+    }
+};
+
+// General EOS only: S3 (cons2prim of the half-step state) and the corrector's geometry, run by the CONSUMER at the top of a
+// group, before its four steps, when only its carried window is alive in registers.  Reads the producer's message
+// {E~, M~_par, |M~|^2, R~} of the four cells from this lane's slots of the message buffer and overwrites them with what
+// Consumer::step expects: {a_c, b_c, sE, sM}.  State: half-step cells -2 (epsh2, gE[1], gM[1]) and -3 (gE[0], gM[0]).
+template <typename T, int EOS>
+struct HalfStep {
+    T epsh2, gE[2], gM[2];
+    __device__ __forceinline__ void init() { epsh2 = gE[0] = gE[1] = gM[0] = gM[1] = T(0); }
+    __device__ __forceinline__ void group(const Consts<T>& k, T* mq)
+    {
+        T vh[4], ph[4];
+#pragma unroll
+        for (int jp = 0; jp < 4; jp += 2) {
+            T a0, a1, a2, a3, b0, b1, b2, b3;
+            load2(mq + 128 * jp, a0, a1); load2(mq + 128 * jp + 64, a2, a3);
+            load2(mq + 128 * (jp + 1), b0, b1); load2(mq + 128 * (jp + 1) + 64, b2, b3);
+            Newt<EOS> na, nb;
+            na.init_em(k.d, (double)a0, (double)a1, (double)a2, (double)a3);
+            nb.init_em(k.d, (double)b0, (double)b1, (double)b2, (double)b3);
+            for (int it = 0; it < 48; ++it) {
+                const double da = na.iter(k.d), db = nb.iter(k.d);
+                if (__all_sync(__activemask(), fmax(da, db) <= 1e-15)) break;
+            }
+            double va, pa, vb, pb;
+            na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);
+            vh[jp] = (T)va; ph[jp] = (T)pa; vh[jp + 1] = (T)vb; ph[jp + 1] = (T)pb;
+        }
+        T eh[5], gv[6], gp[6];
+        eh[0] = epsh2; gv[0] = gE[0]; gv[1] = gE[1]; gp[0] = gM[0]; gp[1] = gM[1];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { eh[j + 1] = k.lam * vh[j]; gv[j + 2] = ph[j] * vh[j]; gp[j + 2] = ph[j]; }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const T q = (T(0.5) - eh[j]) * fast_rcp(T(1) + (eh[j + 1] - eh[j]));
+            store2(mq + 128 * j, T(0.5) - q, (T(0.5) * q) * q);
+            store2(mq + 128 * j + 64, -k.hlam * (gv[j + 2] - gv[j]), -k.hlam * (gp[j + 2] - gp[j]));
+        }
+        epsh2 = eh[4]; gE[0] = gv[4]; gE[1] = gv[5]; gM[0] = gp[4]; gM[1] = gp[5];
+        load_fence();
     }
 };
 
@@ -875,6 +980,17 @@ constexpr int YZ_CREG = 256 - YZ_PREG;
 #endif
 constexpr int X_PREG = SHK_X_PREG;            // x sweep: its consumer (staging tile addresses) needs the full 160
 constexpr int X_CREG = 256 - X_PREG;
+// General-EOS kernels (EOS_MASS, EOS_TABLE): SHK_GEN_CTAS = 1 builds them as ONE CTA per SM with a wide register split and
+// no spill; measured on B200 (config 3, 128^3) that is slower (3.64 G cell-updates/s) than two CTAs per SM with the
+// ~100 B of spills the x kernels and the emitting y/z kernels keep (4.42 G): the Newton chains want the warps more.
+#ifndef SHK_GEN_CTAS
+#define SHK_GEN_CTAS 2
+#endif
+constexpr int GEN_CTAS = SHK_GEN_CTAS;
+#ifndef SHK_GEN_PREG
+#define SHK_GEN_PREG 80
+#endif
+constexpr int GEN_PREG = GEN_CTAS == 1 ? 168 : SHK_GEN_PREG, GEN_CREG = GEN_CTAS == 1 ? 232 : 256 - SHK_GEN_PREG;
 
 template <typename T>
 struct alignas(128) YzPair {      // TMA destinations need 128 B alignment
@@ -917,7 +1033,7 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
 // primitives of the state this sweep READS (the deferred primitive output of a step whose last sweep ran along x: the
 // consumer has U^n of its output cell in the ring tile of the previous group).
 template <typename T, int EOS, int EMIT, bool TMA>
-__global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant__ SweepParams P,
+__global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_yz_kernel(const __grid_constant__ SweepParams P,
                                                           const __grid_constant__ Consts<T> k,
                                                           const __grid_constant__ YzMaps maps)
 {
@@ -948,7 +1064,10 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
     const bool ysweep = P.axis == 1;
 
     if (producer) {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(YZ_PREG));
+        if (sizeof(T) == 8) {
+            if constexpr (EOS == EOS_GAMMA) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(YZ_PREG));
+            else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(GEN_PREG));
+        }
         if (idle) return;
         Producer<T, EOS> pr;
         pr.init();
@@ -1039,12 +1158,17 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
         }
         if (!TMA) cp_async_wait<0>();
     } else {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(YZ_CREG));
+        if (sizeof(T) == 8) {
+            if constexpr (EOS == EOS_GAMMA) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(YZ_CREG));
+            else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(GEN_CREG));
+        }
         if (idle) return;
         Cnt cnt;
         cnt.zero();
         Consumer<T> co;
         co.init(k.aq);
+        HalfStep<T, EOS> hs;
+        hs.init();
         // element offset of the output cell of the NEXT step: cell ilo - 4 (the first two groups store nothing)
         long long o = (long long)(x0 + lane) + (long long)oy * P.stride_other + (long long)(zoff + ilo - GH) * sa;
         int left = active ? (j1 - j0) : 0;      // output cells this lane still has to store
@@ -1063,7 +1187,8 @@ __global__ void __launch_bounds__(256, 2) sweep_yz_kernel(const __grid_constant_
             bar_sync64(bar_id + (g & 1));
             const T* tp = &S.ring[(g + YZ_G - 1) & (YZ_G - 1)][0][0][lane];
             const T* tc = &S.ring[g & (YZ_G - 1)][0][0][lane];
-            const T* mq = &S.msg[g & 1][0][0][lane][0];
+            T* mq = &S.msg[g & 1][0][0][lane][0];
+            if constexpr (EOS != EOS_GAMMA) hs.group(k, mq);       // S3 + geometry (general EOS)
             T uq[NF], ua[NF], c0[NF], c1[NF], c2[NF], msg[4], un[NF];
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
@@ -1151,7 +1276,7 @@ struct X2Maps {
 };
 
 template <typename T, int EOS, bool EMIT, bool TMA>
-__global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant__ SweepParams P,
+__global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_x2_kernel(const __grid_constant__ SweepParams P,
                                                           const __grid_constant__ Consts<T> k,
                                                           const __grid_constant__ X2Maps maps)
 {
@@ -1174,7 +1299,10 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
     const int sw = (lane >> 2) & 1;                         // 32 B swizzle of this lane's row
 
     if (producer) {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(X_PREG));
+        if (sizeof(T) == 8) {
+            if constexpr (EOS == EOS_GAMMA) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(X_PREG));
+            else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(GEN_PREG));
+        }
         if (idle) return;
         Producer<T, EOS> pr;
         pr.init();
@@ -1262,12 +1390,17 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
         }
         cp_async_wait<0>();
     } else {
-        if (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(X_CREG));
+        if (sizeof(T) == 8) {
+            if constexpr (EOS == EOS_GAMMA) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(X_CREG));
+            else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(GEN_CREG));
+        }
         if (idle) return;
         Cnt cnt;
         cnt.zero();
         Consumer<T> co;
         co.init(k.aq);
+        HalfStep<T, EOS> hs;
+        hs.init();
         int q0 = 0;                     // ring tile of group g
         bool store_pending = false;
 #pragma unroll 1
@@ -1276,7 +1409,7 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
             const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;
             const T* tp = &S.ring[qm][0][lane * 4 + 2 * (1 ^ sw)];          // cells 2, 3 of group g-1
             const T* tc = &S.ring[q0][0][lane * 4];
-            const T* mq = &S.msg[g & 1][0][0][lane][0];
+            T* mq = &S.msg[g & 1][0][0][lane][0];
             q0 = (q0 + 1 == X2_G) ? 0 : q0 + 1;
             T uq[NF], ua[NF], c0[NF], c1[NF], c2[NF], msg[4], un[NF], uo[NF];
 #pragma unroll
@@ -1299,6 +1432,7 @@ __global__ void __launch_bounds__(256, 2) sweep_x2_kernel(const __grid_constant_
                 store_pending = false;
             }
             T* ob = &S.outb[0][lane * 4];
+            if constexpr (EOS != EOS_GAMMA) hs.group(k, mq);       // S3 + geometry (general EOS)
             load2(mq, msg[0], msg[1]); load2(mq + 64, msg[2], msg[3]);
             co.template step<0>(uq, ua, msg, uo);
             if (any_out && jf < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, uo, pv, cnt); }
