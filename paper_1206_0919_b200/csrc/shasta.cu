@@ -107,9 +107,9 @@ int ensure_alloc(shasta_t* h)
     return make_yz_maps(h);
 }
 
-// TMA tensor maps of the conserved fields for the x sweep: 2-D {nx, ny*nz}, box {4 cells, 32 rows}, 32 B swizzle
-// (the shared-memory tile layout of sweep_x_ws_kernel).  Needs 16 B row strides: fp64 and even nx; otherwise the
-// kernel's cp.async path is used.  The driver entry point is resolved at run time (libshasta.so does not link libcuda).
+// TMA tensor maps of the conserved fields for the x sweep: 2-D {nx, ny*nz*batch}, box {4 cells, 32 rows}; fp64 with the
+// 32 B swizzle, fp32 dense (the shared-memory tile layouts of sweep_x2_kernel).  Needs 16 B row strides (fp64: even nx,
+// fp32: nx % 4 == 0); otherwise the kernel's cp.async path is used.  The driver entry point is resolved at run time (libshasta.so does not link libcuda).
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -117,7 +117,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 int make_tensor_maps(shasta_t* h)
 {
     h->have_tmap = false;
-    if (h->precision != 64 || (h->nx % 2) != 0 || h->nx < 4) return 0;
+    const size_t es = esize(h);
+    if (((size_t)h->nx * es) % 16 != 0 || h->nx < 4) return 0;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
@@ -126,13 +127,16 @@ int make_tensor_maps(shasta_t* h)
         return 0;                                   // no TMA: the cp.async path still works
     }
     const cuuint64_t dims[2] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny * (cuuint64_t)h->nz * (cuuint64_t)h->nbatch};
-    const cuuint64_t strides[1] = {(cuuint64_t)h->nx * sizeof(double)};
+    const cuuint64_t strides[1] = {(cuuint64_t)h->nx * es};
     const cuuint32_t box[2] = {(cuuint32_t)XV_CH, 32u};
     const cuuint32_t estr[2] = {1u, 1u};
+    // fp64: rows of 32 B, 32 B swizzle; fp32: rows of 16 B (one swizzle atom), dense tiles
+    const CUtensorMapDataType dt = es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const CUtensorMapSwizzle swz = es == 8 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE;
     for (int b = 0; b < 2; ++b)
         for (int f = 0; f < NF; ++f) {
-            CUresult r = ((EncodeTiledFn)fn)(&h->tmap[b][f], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, h->U[b][f], dims, strides,
-                                             box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B,
+            CUresult r = ((EncodeTiledFn)fn)(&h->tmap[b][f], dt, 2, h->U[b][f], dims, strides,
+                                             box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
                                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) return 0;
         }
@@ -366,7 +370,7 @@ int auto_segment(const shasta_t* h, int axis, int N, long long base)
         }
     }
     long long seg = (N + nseg - 1) / nseg;
-    if (axis == 0) seg = ((seg + 7) / 8) * 8;             // even, group-aligned segments for the x sweep (TMA boxes)
+    if (axis == 0) seg = ((seg + 7) / 8) * 8;             // group-aligned segments for the x sweep (TMA boxes start at 16 B)
     return (int)(seg < N ? seg : N);
 }
 
@@ -401,7 +405,7 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
         P.nseg = (P.N + P.seg - 1) / P.seg;
         {
             // producer/consumer warp pairs, 32 rows per pair, 4 pairs per CTA; TMA tiles when possible (fp64, even nx)
-            const bool tma = h->have_tmap && sizeof(T) == 8 && !h->no_tma;
+            const bool tma = h->have_tmap && !h->no_tma;
             X2Maps maps;
             memset(&maps, 0, sizeof(maps));
             maps.fidx[0] = 0; maps.fidx[4] = 4;

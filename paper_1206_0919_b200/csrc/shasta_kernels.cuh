@@ -956,7 +956,12 @@ __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk
 __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 // element offset of (row, cell c in 0..3) inside an x-sweep tile [32 rows][4 cells] with the 32 B swizzle
-__device__ __forceinline__ int xv_off(int row, int c) { return row * 4 + 2 * ((c >> 1) ^ ((row >> 2) & 1)) + (c & 1); }
+// (fp64: rows of 32 B).  fp32 tiles have 16 B rows, one swizzle atom, so they are dense (TMA: CU_TENSOR_MAP_SWIZZLE_NONE).
+template <typename T>
+__device__ __forceinline__ int xv_off(int row, int c)
+{
+    return sizeof(T) == 8 ? row * 4 + 2 * ((c >> 1) ^ ((row >> 2) & 1)) + (c & 1) : row * 4 + c;
+}
 
 // ================================================================================================
 // Round 2: TMA-fed y/z march, one 4-cell group per hand-over.
@@ -1296,7 +1301,8 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
     const int nsteps = (j1 - j0) + 2 * GH;
     const int ngroups = (nsteps + XV_CH - 1) / XV_CH;
     const int col = lane & 3, rsub = lane >> 2;             // element map of the LSU group copies: col, rows rsub + 8 kk
-    const int sw = (lane >> 2) & 1;                         // 32 B swizzle of this lane's row
+    const int sw = sizeof(T) == 8 ? (lane >> 2) & 1 : 0;    // 32 B swizzle of this lane's row (fp64 tiles only)
+    constexpr int XALIGN = 16 / (int)sizeof(T);             // cells per 16 B: TMA boxes start at 16 B aligned cells
 
     if (producer) {
         if (sizeof(T) == 8) {
@@ -1318,7 +1324,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
         constexpr int NP = Producer<T, EOS>::NP;
         // a group that lies inside [0, N) and starts at an even cell is one TMA box per field; a group that touches a
         // boundary needs the ghost map (reading G11) and is copied element by element (cp.async)
-        auto group_is_tma = [&](int g) { const int xg = ilo + XV_CH * g; return TMA && xg >= 0 && xg + XV_CH <= N && (xg & 1) == 0; };
+        auto group_is_tma = [&](int g) { const int xg = ilo + XV_CH * g; return TMA && xg >= 0 && xg + XV_CH <= N && (xg % XALIGN) == 0; };
         int q1 = 0;                     // ring tile of group g+1
 #pragma unroll 1
         for (int g = -1; g < ngroups; ++g) {
@@ -1340,7 +1346,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                         const int row = rsub + 8 * kk;
                         if (row < nrows) {
                             const long long o = (row0 + row) * (long long)N + gi;
-                            const int so = xv_off(row, col);
+                            const int so = xv_off<T>(row, col);
 #pragma unroll
                             for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * XV_TILE + so, (const T*)P.in[f] + o);
                         }
@@ -1360,7 +1366,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                 __syncwarp();
             }
             const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;           // tile of group g-1
-            const T* tp = &S.ring[qm][0][xv_off(lane, 3)];
+            const T* tp = &S.ring[qm][0][xv_off<T>(lane, 3)];
             const T* tc = &S.ring[q0][0][lane * 4];
             T mm[4][4];
             struct {
@@ -1458,7 +1464,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
             if (!any_out) continue;
             // the finished group leaves as one TMA box per field when all of its cells are output cells of this segment (or
             // are clipped by the grid edge); otherwise (ragged segment end, odd start, EMIT) through the LSU
-            if (TMA && !EMIT && (jf & 1) == 0 && (jf + XV_CH <= j1 || j1 == N)) {
+            if (TMA && !EMIT && (jf % XALIGN) == 0 && (jf + XV_CH <= j1 || j1 == N)) {
                 fence_proxy_async();                        // generic-proxy writes of outb -> visible to the TMA engine
                 __syncwarp();
                 if (lane == 0) {
@@ -1476,7 +1482,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                         const int row = rsub + 8 * kk;
                         if (row < nrows) {
                             const long long o = (row0 + row) * (long long)N + jo;
-                            const int so = xv_off(row, col);
+                            const int so = xv_off<T>(row, col);
                             T u[NF];
 #pragma unroll
                             for (int f = 0; f < NF; ++f) {

@@ -138,6 +138,22 @@ def test_fp32_storage_kernel_level(oracle, bc, shape):
         assert emax <= 2e-5 and el1 <= 2e-6, (k, emax, el1)
 
 
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("shape", [(64, 9, 7), (132, 33, 2), (40, 40, 3), (38, 19, 5)])
+@pytest.mark.parametrize("segment", [0, 8, 24])
+def test_fp32_tma_and_cp_async_paths_same_bits(oracle, bc, shape, segment):
+    # fp32 storage: nx % 4 == 0 gives 16 B row strides, so all three sweeps are TMA-fed (x: dense {4, 32} tiles);
+    # SHASTA_NO_TMA forces the cp.async fill and the LSU drain.  Same bits either way, and close to the fp64 oracle.
+    c = inputs.random_state(*shape, seed=shape[0] + 7 * bc, kind="smooth", boundary=bc)
+    got, _ = parity.run_gpu(c, steps=2, precision=32, segment=segment)
+    alt, _ = parity.run_gpu(c, steps=2, precision=32, segment=segment, no_tma=1)
+    for k in parity.CONS + parity.PRIM:
+        assert np.array_equal(got[k], alt[k]), k
+    ref, _ = parity.run_oracle(oracle, c, steps=2)
+    for k, (emax, el1) in parity.field_errors(got, ref).items():
+        assert emax <= 2e-5 and el1 <= 2e-6, (k, emax, el1)
+
+
 def test_vacuum_and_superluminal_cells(oracle):
     # E <= 0 cells and |M| > E cells fed through set_conserved: projection + vacuum rule (P13)
     import torch
