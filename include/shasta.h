@@ -81,7 +81,9 @@ typedef struct shasta shasta_t;   /* opaque */
 int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lambda, double eos_gamma);
 void shasta_destroy(shasta_t* h);
 
-/* Options; BOUNDARY, EOS_MASS and PRECISION must be set before shasta_set_state. */
+/* Options.  PRECISION, BATCH and EOS_MASS must be set before the first shasta_set_state (SHASTA_ESTATE afterwards);
+ * every other option may be changed between calls (it takes effect with the next launch).  A handle belongs to the
+ * device that was current at shasta_create: calls made with another device current return SHASTA_ESTATE. */
 int shasta_set_option(shasta_t* h, int key, double value);
 
 /* Tabled equation of state (the velocity is found by root finding "to allow

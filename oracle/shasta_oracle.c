@@ -47,6 +47,11 @@
 #define G  4          /* ghost depth of one sweep: dependency radius of the default scheme (R1) */
 #define G2 6          /* same for the R2 predictor (half step WITH antidiffusion, reading G4 alternative) */
 #define PI_DELTA 1e-12            /* reading G7 */
+#define VAC_E    0x1p-498         /* reading G7 (amended in round 2): a cell is vacuum when !(E >= 2^-498 ~ 1.2e-150), i.e. E <= 0,
+                                     NaN, or so small that E^2 and |M|^2 are not representable in fp64 -- there |M| =
+                                     sqrt(Mx^2+My^2+Mz^2) below is formed from underflowed squares and v = M/(E+P) is rounding
+                                     noise in ANY fp64 evaluation.  Such cells arise at a front running into an exact E = 0
+                                     exterior (the FCT front is so steep that they touch cells of visible size). */
 #define FP_TOL   1e-15            /* reading G9 */
 #define FP_MAXIT 200              /* reading G9 */
 
@@ -128,11 +133,11 @@ void oracle_prim2cons(double e, double n, double vx, double vy, double vz,
 }
 
 /* ------------------- phases 3+4: relativistic correction + EOS (cons2prim) */
-/* Pi, readings G6-G8: enforce |M| <= (1-delta) E; vacuum if !(E > 0).
+/* Pi, readings G6-G8: enforce |M| <= (1-delta) E; vacuum if !(E >= VAC_E).
    Returns 1 if the projection fired, 2 if vacuum, 0 otherwise.  E, R untouched. */
 int oracle_project(double E, double M[3])
 {
-    if (!(E > 0.0)) { M[0] = M[1] = M[2] = 0.0; return 2; }
+    if (!(E >= VAC_E)) { M[0] = M[1] = M[2] = 0.0; return 2; }
     double Mabs = sqrt((M[0] * M[0] + M[1] * M[1]) + M[2] * M[2]);
     double lim = (1.0 - PI_DELTA) * E;
     if (Mabs > lim) {
@@ -149,7 +154,7 @@ int oracle_cons2prim_eos(double E, double Mx, double My, double Mz, double R,
                          double gamma, double mass, const eos_table_t *tab, double out[7], int flags[2])
 {
     double M = sqrt((Mx * Mx + My * My) + Mz * Mz);
-    if (!(E > 0.0)) {                         /* vacuum, reading G7 */
+    if (!(E >= VAC_E)) {                      /* vacuum, reading G7 */
         for (int i = 0; i < 7; ++i) out[i] = 0.0;
         return 0;
     }

@@ -64,6 +64,7 @@ struct shasta {
     double* h_partial;      // pinned
     long long launches;
     int sm_count;
+    int device;             // device that was current at create
     char err[256];
 };
 
@@ -91,9 +92,18 @@ size_t esize(const shasta_t* h) { return h->precision == 64 ? 8 : 4; }
 int make_tensor_maps(shasta_t* h);
 int make_yz_maps(shasta_t* h);
 
-int ensure_alloc(shasta_t* h)
+void free_fields(shasta_t* h)
 {
-    if (h->allocated) return 0;
+    for (int b = 0; b < 2; ++b)
+        for (int f = 0; f < NF; ++f) { cudaFree(h->U[b][f]); h->U[b][f] = nullptr; }
+    for (int q = 0; q < 6; ++q) { cudaFree(h->prim[q]); h->prim[q] = nullptr; }
+    cudaFree(h->d_counts); h->d_counts = nullptr;
+    cudaFree(h->d_partial); h->d_partial = nullptr;
+    if (h->h_partial) { cudaFreeHost(h->h_partial); h->h_partial = nullptr; }
+}
+
+int alloc_fields(shasta_t* h)
+{
     const size_t nb = (size_t)h->ncell * esize(h);
     for (int b = 0; b < 2; ++b)
         for (int f = 0; f < NF; ++f) CK(cudaMalloc(&h->U[b][f], nb));
@@ -102,6 +112,26 @@ int ensure_alloc(shasta_t* h)
     CK(cudaMemset(h->d_counts, 0, 4 * sizeof(unsigned long long)));
     CK(cudaMalloc(&h->d_partial, sizeof(double) * RED_BLOCKS * NF * 2));
     CK(cudaMallocHost(&h->h_partial, sizeof(double) * RED_BLOCKS * NF * 2));
+    return 0;
+}
+
+// the handle belongs to the device that was current at shasta_create
+int check_device(shasta_t* h)
+{
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev != h->device)
+        return fail(h, SHASTA_ESTATE, "the handle was created on device %d but device %d is current", h->device, dev);
+    return 0;
+}
+
+int ensure_alloc(shasta_t* h)
+{
+    int rc = check_device(h);
+    if (rc) return rc;
+    if (h->allocated) return 0;
+    rc = alloc_fields(h);
+    if (rc) { free_fields(h); cudaGetLastError(); return rc; }      // nothing half-allocated is kept
     h->allocated = true;
     make_tensor_maps(h);
     return make_yz_maps(h);
@@ -695,6 +725,7 @@ int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lamb
     memcpy(h->table, kBranch, sizeof(kBranch));
     h->ntable = 18;
     h->sm_count = prop.multiProcessorCount;
+    h->device = dev;
     *out = h;
     return 0;
 }
@@ -704,16 +735,11 @@ void shasta_destroy(shasta_t* h)
     if (!h) return;
     drop_graphs(h);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
-    for (int b = 0; b < 2; ++b)
-        for (int f = 0; f < NF; ++f) cudaFree(h->U[b][f]);
-    for (int q = 0; q < 6; ++q) cudaFree(h->prim[q]);
+    free_fields(h);
     cudaFree(h->stage);
     cudaFree(h->d_tab);
     cudaFree(h->d_yzmaps);
     cudaFree(h->d_xmaps);
-    cudaFree(h->d_counts);
-    cudaFree(h->d_partial);
-    if (h->h_partial) cudaFreeHost(h->h_partial);
     delete h;
 }
 
@@ -732,6 +758,8 @@ int shasta_set_option(shasta_t* h, int key, double value)
         return 0;
     case SHASTA_EOS_MASS:
         if (!(value >= 0.0)) return fail(h, SHASTA_EINVAL, "SHASTA_EOS_MASS must be >= 0");
+        if (h->have_state && value != h->mass)
+            return fail(h, SHASTA_ESTATE, "SHASTA_EOS_MASS must be set before shasta_set_state (the conserved state was built with the old EOS)");
         h->mass = value;
         h->prims_valid = false;
         return 0;
@@ -905,6 +933,7 @@ int shasta_step(shasta_t* h, int nsteps, void* stream)
     if (!h) return SHASTA_EINVAL;
     if (nsteps < 0) return fail(h, SHASTA_EINVAL, "shasta_step: nsteps < 0");
     if (!h->have_state) return fail(h, SHASTA_ESTATE, "shasta_step: call shasta_set_state first");
+    if (int rc = check_device(h)) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     // whole cycles of the axis table as one CUDA graph each (auto: only where a sweep is short enough for launch gaps to
     // show, < 2^22 cells); the remainder launch by launch

@@ -33,6 +33,7 @@ namespace shk {
 
 constexpr int NF = 5;       // E, M_par, M_perp1, M_perp2, R
 constexpr int GH = 4;       // ghost depth = dependency radius of one sweep
+constexpr double VAC_E = 0x1p-498;      // reading G7: a cell with !(E >= 2^-498) is vacuum (E^2, |M|^2 not representable below)
 constexpr int EOS_GAMMA = 0;    // p = (Gamma-1) e            (m = 0): closed-form velocity
 constexpr int EOS_MASS = 1;     // p = (Gamma-1)(e - m n)     (m > 0): safeguarded Newton
 constexpr int EOS_TABLE = 2;    // p = bilinear table P(e, n) (reading T1): the same safeguarded Newton
@@ -217,7 +218,7 @@ template <int EOS>
 __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, double Ma, double Mb, double Mc, double R)
 {
     Prim o;
-    const bool vac = !(E > double(0));                   // vacuum (reading G7); also catches NaN
+    const bool vac = !(E >= VAC_E);                      // vacuum (reading G7); also catches NaN
     if (vac) { E = double(1); Ma = Mb = Mc = double(0); }     // keep the arithmetic below finite; result discarded
     o.fl = 0;
     const double M2 = fma(Ma, Ma, fma(Mb, Mb, Mc * Mc));
@@ -330,7 +331,7 @@ struct Newt {
     __device__ __forceinline__ void init_em(const EosD& k, double E_, double M1_, double M2_, double R_)
     {
         E = E_; M1 = M1_; M2 = M2_; R = R_;
-        vac = !(E > 0.0);
+        vac = !(E >= VAC_E);
         if (vac) { E = 1.0; M1 = 0.0; M2 = 0.0; }
         const double lim = k.omd * E;
         const double lim2 = lim * lim;
@@ -399,9 +400,12 @@ struct Newt {
 // Newton of c2p_fast_y converges in two steps (larger Gamma runs the EOS_MASS kernels with m = 0).  The causality clamp Mc = min(|M|, (1-delta) E) stays inline: Mc^2 is a
 // select on the bit patterns (non-negative doubles order like integers), and only a clamped cell (~0.2 % of
 // the cells of config 4) pays the extra rsqrt for the direction-preserving scale factor.
+// Vacuum test of the Gamma-law kernels on the high word: reading G7, !(E >= 2^-498): E <= 0, -0, and every E whose square
+// is not representable (exponent field < 0x20D = 1023 - 498); the closed form below would divide by zero there.  NaN with
+// a clear sign bit has a large exponent field and propagates instead of being called vacuum (a NaN input is an error).
 __device__ __forceinline__ bool c2p_is_vacuum(double E)
 {
-    return __double2hiint(E) <= 0;
+    return __double2hiint(E) < 0x20D00000;
 }
 __device__ __forceinline__ bool gt_nonneg(double a, double b)      // a > b for a, b >= 0, on the integer pipe
 {
@@ -550,7 +554,7 @@ __device__ __forceinline__ void project(const EosD& k, double (&un)[NF], Cnt& co
     const double E = un[0];
     const double M2 = fma(un[1], un[1], fma(un[2], un[2], un[3] * un[3]));
     const double lim = k.omd * E;
-    if (!(E > 0.0)) {
+    if (!(E >= VAC_E)) {
         un[1] = un[2] = un[3] = 0.0;
         counts.add(1);
     } else if (M2 > lim * lim) {

@@ -37,6 +37,7 @@ def test_single_axis_sweeps_ragged(oracle, axis, bc, kind):
     got, s = parity.run_gpu(c, steps=1, table=[axis] * 3)
     assert_kernel_parity(got, ref, f"axis {axis} bc {bc} {kind}")
     # Pi fires in the same cells up to those sitting within rounding of the limit |M| = (1-1e-12) E
+    # (cells within an ulp of the limit may fall on either side: at most 2, or 0.5 % of the firings)
     assert abs(s.diagnostics()[0] - o.diagnostics()[0]) <= max(2, o.diagnostics()[0] // 200)
 
 
@@ -173,6 +174,41 @@ def test_vacuum_and_superluminal_cells(oracle):
     got.update({k: v.cpu().numpy() for k, v in s.get_primitives().items()})
     assert_kernel_parity(got, ref, "vacuum", tol_cons=1e-11, tol_prim=1e-11)
     assert all(np.all(np.isfinite(v)) for v in got.values())
+
+
+@pytest.mark.parametrize("shape", [(600, 1, 1), (1, 600, 1), (40, 36, 44)])
+def test_matter_marching_into_exact_vacuum_stays_finite(oracle, shape):
+    # E = 0 exterior (accepted by shasta_set_conserved): the numerical diffusion front carries E down through 1e-150,
+    # where E^2 underflows, and through the subnormals.  The Gamma-law kernels call E < 2^-498 vacuum (c2p_is_vacuum);
+    # nothing may become NaN or inf, and everything of visible size must still agree with the oracle.
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    nx, ny, nz = shape
+    z, y, x = np.meshgrid(np.arange(nz) - nz / 2, np.arange(ny) - ny / 2, np.arange(nx) - nx / 2, indexing="ij")
+    inside = (x * x + y * y + z * z) < 36.0
+    E = np.where(inside, 1.0, 0.0)
+    M = [np.where(inside, 0.2 * s, 0.0) for s in (1.0, -0.5, 0.25)]
+    R = np.where(inside, 0.7, 0.0)
+    steps = 100 if max(shape) == 600 else 12
+    o = oracle.Oracle(nx, ny, nz, 0.1, 0.4, 4.0 / 3.0)
+    o.set_conserved(E, *M, R); o.step(steps)
+    s = Shasta(nx, ny, nz, 0.1, 0.4, 4.0 / 3.0)
+    s.set_conserved(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (E, *M, R)]); s.step(steps)
+    ref = dict(o.get_conserved()); ref.update(o.get_primitives())
+    got = {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
+    got.update({k: v.cpu().numpy() for k, v in s.get_primitives().items()})
+    assert all(np.all(np.isfinite(v)) for v in got.values())
+    assert (got["E"] > 0).sum() > inside.sum()
+    # Agreement with the oracle is loose BY NATURE here: next to an exact-zero exterior the new E of a front cell is a
+    # rounding residue of either sign (flux form here, eq. (17) as printed in the oracle), i.e. vacuum on one side and a
+    # light-like cell on the other, and its velocity enters Q+- of a neighbour of visible size.  Measured 2e-8 after 12
+    # steps; the oracle's own strict/FMA builds happen to agree (2.5e-14) because both use the same form.
+    scale = np.max(np.abs(ref["E"]))
+    for k in ("E", "Mx", "My", "Mz", "R", "e", "p"):
+        assert np.max(np.abs(got[k] - ref[k])) <= 1e-6 * scale, k
+    # E and R are never modified by Pi or the vacuum rule: their totals are conserved until the front reaches the boundary
+    if max(shape) == 600:
+        assert abs(got["E"].sum() - E.sum()) <= 1e-12 * E.sum() and abs(got["R"].sum() - R.sum()) <= 1e-12 * R.sum()
 
 
 def test_step_split_and_step_index(oracle):
