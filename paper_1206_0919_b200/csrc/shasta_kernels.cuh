@@ -31,6 +31,9 @@
 
 namespace shk {
 
+#ifndef SHK_GEOM_C
+#define SHK_GEOM_C 0
+#endif
 constexpr int NF = 5;       // E, M_par, M_perp1, M_perp2, R
 constexpr int GH = 4;       // ghost depth = dependency radius of one sweep
 constexpr double VAC_E = 0x1p-498;      // reading G7: a cell with !(E >= 2^-498) is vacuum (E^2, |M|^2 not representable below)
@@ -808,6 +811,11 @@ struct Producer {
                     ut[j][NF - 1] = T(0);
                 }
             });
+            if (SHK_GEOM_C) {       // A/B: the corrector's geometry in the consumer (HalfStep), the message is {v, p} at n+1/2
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { msg[j][0] = vh[j]; msg[j][1] = ph[j]; msg[j][2] = T(0); msg[j][3] = T(0); }
+                return;
+            }
             T eh[5], gv[6], gp[6];
             eh[0] = epsh2; gv[0] = gE[0]; gv[1] = gE[1]; gp[0] = gM[0]; gp[1] = gM[1];
 #pragma unroll
@@ -836,6 +844,10 @@ struct HalfStep {
     __device__ __forceinline__ void group(const Consts<T>& k, T* mq)
     {
         T vh[4], ph[4];
+        if constexpr (EOS == EOS_GAMMA) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) load2(mq + 128 * j, vh[j], ph[j]);
+        } else
 #pragma unroll
         for (int jp = 0; jp < 4; jp += 2) {
             T a0, a1, a2, a3, b0, b1, b2, b3;
@@ -1197,7 +1209,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
             const T* tp = &S.ring[(g + YZ_G - 1) & (YZ_G - 1)][0][0][lane];
             const T* tc = &S.ring[g & (YZ_G - 1)][0][0][lane];
             T* mq = &S.msg[g & 1][0][0][lane][0];
-            if constexpr (EOS != EOS_GAMMA) hs.group(k, mq);       // S3 + geometry (general EOS)
+            if constexpr (EOS != EOS_GAMMA || SHK_GEOM_C) hs.group(k, mq);       // S3 + geometry (general EOS)
             T uq[NF], ua[NF], c0[NF], c1[NF], c2[NF], msg[4], un[NF];
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
@@ -1442,7 +1454,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                 store_pending = false;
             }
             T* ob = &S.outb[0][lane * 4];
-            if constexpr (EOS != EOS_GAMMA) hs.group(k, mq);       // S3 + geometry (general EOS)
+            if constexpr (EOS != EOS_GAMMA || SHK_GEOM_C) hs.group(k, mq);       // S3 + geometry (general EOS)
             load2(mq, msg[0], msg[1]); load2(mq + 64, msg[2], msg[3]);
             co.template step<0>(uq, ua, msg, uo);
             if (any_out && jf < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, uo, pv, cnt); }
