@@ -60,6 +60,9 @@ def parse_args():
     ap.add_argument("--size", type=int, default=256, help="grid extent (256 = the metric's workload)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--segment", type=int, default=0, help="tuning: cells marched per work item (0 = auto)")
+    ap.add_argument("--workload", default="hotspots", choices=["hotspots", "spherical_riemann", "fireball"],
+                    help="hotspots = BASELINE.json configs[3], the metric's workload (default); the others are the parity "
+                         "configs 3 (general EOS) and 2, offered for profiling: their lines are not the headline metric")
     ap.add_argument("--batch", type=int, default=1, help="independent events per GPU advanced by one launch (SHASTA_BATCH)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -215,7 +218,10 @@ def ours(args):
     n = args.size
     import numpy as np
     B = max(1, args.batch)
-    cs = [inputs.hotspots(n, steps=args.steps, seed=replicas.event_seed(rank) + 1000 * b) for b in range(B)]
+    if args.workload == "hotspots":
+        cs = [inputs.hotspots(n, steps=args.steps, seed=replicas.event_seed(rank) + 1000 * b) for b in range(B)]
+    else:
+        cs = [getattr(inputs, args.workload)(n, steps=args.steps) for b in range(B)]
     c = cs[0]
     ncell = B * n ** 3              # cells advanced per step on this GPU (all events of the batch)
     names = ("e", "n", "vx", "vy", "vz")
@@ -361,8 +367,9 @@ def ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
-            "config": {"workload": f"hotspots {n}^3 (BASELINE.json configs[3]): 50 Gaussian hotspots + "
-                                   "vz=tanh(z/4), dx=0.1 fm, lambda=0.4, p=e/3, outflow; one event per GPU",
+            "config": {"workload": (f"hotspots {n}^3 (BASELINE.json configs[3]): 50 Gaussian hotspots + "
+                                    "vz=tanh(z/4), dx=0.1 fm, lambda=0.4, p=e/3, outflow; one event per GPU")
+                                   if args.workload == "hotspots" else f"{args.workload} {n}^3 (a parity config, NOT the metric's workload)",
                        "grid": [n, n, n], "batch": B, "cells_per_gpu": ncell, "parallelism": f"replicas x{world}",
                        "l2": "state (2x5 fields ping-pong + 6 primitives, "
                              f"{16 * ncell * args.precision // 8 / 1e6:.0f} MB) is larger than the 126 MB L2; no flush",

@@ -159,7 +159,8 @@ long long shasta_launch_count(const shasta_t* h);
 long long shasta_graph_launch_count(const shasta_t* h);
 /* Step counter s (number of steps taken, or the value set by SHASTA_STEP_INDEX). */
 long long shasta_step_index(const shasta_t* h);
-/* Name of the sweep kernel variant used for `axis` with the current options (for profiles/). */
+/* Name of the sweep kernel variant used for `axis` with the current options (for profiles/); the suffix "(cp.async)"
+ * says that the sweep fills its shared-memory tiles without TMA (no 16 B row strides, SHASTA_NO_TMA, ...). */
 const char* shasta_kernel_name(const shasta_t* h, int axis);
 
 const char* shasta_last_error(const shasta_t* h);   /* h may be NULL: error of the last failed create */

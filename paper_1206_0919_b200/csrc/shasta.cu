@@ -1077,7 +1077,13 @@ const char* shasta_kernel_name(const shasta_t* h, int axis)
 {
     if (!h || axis < 0 || axis > 2) return "";
     if (h->predictor || h->cell_path) return "sweep_cell_kernel";
-    return axis == 0 ? "sweep_x2_kernel" : "sweep_yz_kernel";
+    // "(cp.async)" marks a sweep that cannot (or may not) use its TMA tiles: no 16 B row strides, extent < 4 cells, no
+    // driver entry point, SHASTA_NO_TMA.  Before the first set_state the maps do not exist yet: reported as TMA-capable.
+    const int n[3] = {h->nx, h->ny, h->nz};
+    const bool have = axis == 0 ? h->have_tmap : (h->have_yzmap && n[axis] >= YZ_CH);
+    const bool tma = !h->no_tma && (have || !h->allocated);
+    if (axis == 0) return tma ? "sweep_x2_kernel" : "sweep_x2_kernel(cp.async)";
+    return tma ? "sweep_yz_kernel" : "sweep_yz_kernel(cp.async)";
 }
 
 const char* shasta_last_error(const shasta_t* h) { return h ? h->err : g_create_err; }
