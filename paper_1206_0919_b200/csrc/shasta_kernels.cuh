@@ -203,6 +203,24 @@ __device__ __forceinline__ double fast_rsqrt3(double x)
     return fma(r, p * e, r);
 }
 
+// two adjacent elements with one shared-memory access (LDS.128 for fp64); p is 2-element aligned
+__device__ __forceinline__ void load2(const double* p, double& a, double& b)
+{
+    const double2 v = *reinterpret_cast<const double2*>(p);
+    a = v.x; b = v.y;
+}
+__device__ __forceinline__ void load2(const float* p, float& a, float& b)
+{
+    const float2 v = *reinterpret_cast<const float2*>(p);
+    a = v.x; b = v.y;
+}
+
+__device__ __forceinline__ void store2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
+__device__ __forceinline__ void store2(float* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
+
+// keeps shared-memory loads below this point (registers: a pair of cells is 20 registers)
+__device__ __forceinline__ void load_fence() { asm volatile("" ::: "memory"); }
+
 // ------------------------------------------------------------------------------------------------
 // cons2prim: relativistic correction + EOS (phases 3-4; readings G6-G10).
 // Solves v (E + P(E - Mc v, R sqrt(1-v^2))) = Mc, Mc = min(|M|, (1-delta) E), on [0,1).
@@ -510,25 +528,43 @@ __device__ __forceinline__ void c2p_group(const Consts<T>& k, T (&c0)[NF], T (&c
             if (__any_sync(0xffffffffu, rare[3])) c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
         }
     } else {
-        // general EOS: two cells per Newton loop (see Newt), the warp leaves a loop together
-#define SHK_C2P_PAIR(J, CA, CB)                                                                 \
-        {                                                                                       \
-            double ua[NF], ub[NF], va, pa, vb, pb;                                              \
-            _Pragma("unroll") for (int f = 0; f < NF; ++f) { ua[f] = (double)CA[f]; ub[f] = (double)CB[f]; } \
-            Newt<EOS> na, nb;                                                                   \
-            na.init(k.d, ua); nb.init(k.d, ub);                                                 \
-            for (int it = 0; it < 48; ++it) {                                                   \
-                const double da = na.iter(k.d), db = nb.iter(k.d);                              \
-                if (__all_sync(0xffffffffu, fmax(da, db) <= 1e-15)) break;                      \
-            }                                                                                   \
-            na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);                                     \
-            v[J] = (T)va; p[J] = (T)pa; v[J + 1] = (T)vb; p[J + 1] = (T)pb;                     \
-        }
-        SHK_C2P_PAIR(0, c0, c1)
-        reload();                           // brings c2, c3 only now (ring / scratch): two cells alive at a time
-        SHK_C2P_PAIR(2, c2, c3)
-#undef SHK_C2P_PAIR
+        // general EOS: the sweeps use c2p_pairs_general below (one shared loop body); this form serves no kernel
+        (void)reload;
+        c2p_sweep<T, EOS>(k, c0, v[0], p[0]);
+        c2p_sweep<T, EOS>(k, c1, v[1], p[1]);
+        c2p_sweep<T, EOS>(k, c2, v[2], p[2]);
+        c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
     }
+}
+
+// General EOS, S1 of a group: two Newton loops of two cells each (see Newt), written as ONE loop body executed twice
+// (#pragma unroll 1): the results go through this lane's scratch slots `scr` (cell j at scr + 128 j) because a rolled
+// loop cannot index registers.  Unrolled, the two copies of the solver (with the consumer's two more) made the kernel
+// miss the instruction cache: ncu showed `no_inst` as 32 % of the consumer's and 12 % of the producer's stall samples.
+// `pairload(pi, a, b)` reads cells 2 pi, 2 pi + 1 of the group from the ring.
+template <typename T, int EOS, typename PL>
+__device__ __forceinline__ void c2p_pairs_general(const Consts<T>& k, const PL& pairload, T* scr, T (&v)[4], T (&p)[4])
+{
+#pragma unroll 1
+    for (int pi = 0; pi < 2; ++pi) {
+        T ca[NF], cb[NF];
+        pairload(pi, ca, cb);
+        double ua[NF], ub[NF], va, pa, vb, pb;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) { ua[f] = (double)ca[f]; ub[f] = (double)cb[f]; }
+        Newt<EOS> na, nb;
+        na.init(k.d, ua); nb.init(k.d, ub);
+        for (int it = 0; it < 48; ++it) {
+            const double da = na.iter(k.d), db = nb.iter(k.d);
+            if (__all_sync(0xffffffffu, fmax(da, db) <= 1e-15)) break;
+        }
+        na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);
+        store2(scr + 256 * pi, (T)va, (T)pa);
+        store2(scr + 256 * pi + 128, (T)vb, (T)pb);
+    }
+    load_fence();
+#pragma unroll
+    for (int j = 0; j < 4; ++j) load2(scr + 128 * j, v[j], p[j]);
 }
 
 // eq. (21) branch-free (reading G12): A = sigma max(0, min(sigma D^_{j+1}, |A^ph|, sigma D^_{j-1}))
@@ -695,24 +731,6 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // dependent chain is half as long.  P -> C traffic per pencil and step is four doubles through a
 // shared-memory queue: a_c = 1/2 - Q+, b_c = Q+^2/2 of the interface (i-2,i-1) at n+1/2, and the two
 // source increments -lambda Delta(p v)/2-form for E and M_par of cell i-2.
-// two adjacent elements with one shared-memory access (LDS.128 for fp64); p is 2-element aligned
-__device__ __forceinline__ void load2(const double* p, double& a, double& b)
-{
-    const double2 v = *reinterpret_cast<const double2*>(p);
-    a = v.x; b = v.y;
-}
-__device__ __forceinline__ void load2(const float* p, float& a, float& b)
-{
-    const float2 v = *reinterpret_cast<const float2*>(p);
-    a = v.x; b = v.y;
-}
-
-__device__ __forceinline__ void store2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
-__device__ __forceinline__ void store2(float* p, float a, float b) { *reinterpret_cast<float2*>(p) = make_float2(a, b); }
-
-// keeps shared-memory loads below this point (registers: a pair of cells is 20 registers)
-__device__ __forceinline__ void load_fence() { asm volatile("" ::: "memory"); }
-
 template <typename T, int EOS>
 struct Producer {
     // fields the producer needs: the Gamma-law pressure does not depend on R, so R's predictor is skipped there
@@ -752,7 +770,7 @@ struct Producer {
                     ld.second(c3, c4);
                     c2p_group<T, EOS>(k, c1, c2, c3, c4, v, p, [&]() { load_fence(); ld.first(c0, c1, c2); ld.second(c3, c4); });    // S1
                 } else {
-                    c2p_group<T, EOS>(k, c1, c2, c3, c4, v, p, [&]() { load_fence(); ld.second(c3, c4); });
+                    c2p_pairs_general<T, EOS>(k, [&](int pi, T (&a)[NF], T (&b)[NF]) { ld.pair(pi, a, b); }, scr, v, p);
                 }
             }
             T eps[5], pv[6], pp[6];
@@ -847,22 +865,29 @@ struct HalfStep {
         if constexpr (EOS == EOS_GAMMA) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) load2(mq + 128 * j, vh[j], ph[j]);
-        } else
-#pragma unroll
-        for (int jp = 0; jp < 4; jp += 2) {
-            T a0, a1, a2, a3, b0, b1, b2, b3;
-            load2(mq + 128 * jp, a0, a1); load2(mq + 128 * jp + 64, a2, a3);
-            load2(mq + 128 * (jp + 1), b0, b1); load2(mq + 128 * (jp + 1) + 64, b2, b3);
-            Newt<EOS> na, nb;
-            na.init_em(k.d, (double)a0, (double)a1, (double)a2, (double)a3);
-            nb.init_em(k.d, (double)b0, (double)b1, (double)b2, (double)b3);
-            for (int it = 0; it < 48; ++it) {
-                const double da = na.iter(k.d), db = nb.iter(k.d);
-                if (__all_sync(__activemask(), fmax(da, db) <= 1e-15)) break;
+        } else {
+            // one loop body for both pairs (instruction cache, see c2p_pairs_general): results back through the slots
+#pragma unroll 1
+            for (int jp = 0; jp < 4; jp += 2) {
+                T* ma = mq + 128 * jp;
+                T a0, a1, a2, a3, b0, b1, b2, b3;
+                load2(ma, a0, a1); load2(ma + 64, a2, a3);
+                load2(ma + 128, b0, b1); load2(ma + 192, b2, b3);
+                Newt<EOS> na, nb;
+                na.init_em(k.d, (double)a0, (double)a1, (double)a2, (double)a3);
+                nb.init_em(k.d, (double)b0, (double)b1, (double)b2, (double)b3);
+                for (int it = 0; it < 48; ++it) {
+                    const double da = na.iter(k.d), db = nb.iter(k.d);
+                    if (__all_sync(__activemask(), fmax(da, db) <= 1e-15)) break;
+                }
+                double va, pa, vb, pb;
+                na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);
+                store2(ma, (T)va, (T)pa);
+                store2(ma + 128, (T)vb, (T)pb);
             }
-            double va, pa, vb, pb;
-            na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);
-            vh[jp] = (T)va; ph[jp] = (T)pa; vh[jp + 1] = (T)vb; ph[jp + 1] = (T)pb;
+            load_fence();
+#pragma unroll
+            for (int j = 0; j < 4; ++j) load2(mq + 128 * j, vh[j], ph[j]);
         }
         T eh[5], gv[6], gp[6];
         eh[0] = epsh2; gv[0] = gE[0]; gv[1] = gE[1]; gp[0] = gM[0]; gp[1] = gM[1];
@@ -1170,6 +1195,15 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                         c3[f] = tc[f * YZ_CH * 32 + 96];
                     }
                 }
+                __device__ __forceinline__ void pair(int pi, T (&a)[NF], T (&b)[NF]) const      // cells 2 pi, 2 pi + 1
+                {
+                    a[NF - 1] = b[NF - 1] = T(0);
+#pragma unroll
+                    for (int f = 0; f < NP; ++f) {
+                        a[f] = tc[f * YZ_CH * 32 + 64 * pi];
+                        b[f] = tc[f * YZ_CH * 32 + 64 * pi + 32];
+                    }
+                }
             } ld = {tp, tc};
             T* mq = &S.msg[g & 1][0][0][lane][0];
             pr.group(k, ld, mq, mm);
@@ -1402,6 +1436,12 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                     c2[NF - 1] = c3[NF - 1] = T(0);
 #pragma unroll
                     for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (1 ^ sw), c2[f], c3[f]);
+                }
+                __device__ __forceinline__ void pair(int pi, T (&a)[NF], T (&b)[NF]) const      // cells 2 pi, 2 pi + 1
+                {
+                    a[NF - 1] = b[NF - 1] = T(0);
+#pragma unroll
+                    for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (pi ^ sw), a[f], b[f]);
                 }
             } ld = {tp, tc, sw};
             T* mq = &S.msg[g & 1][0][0][lane][0];
