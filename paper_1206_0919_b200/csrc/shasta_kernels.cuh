@@ -502,38 +502,43 @@ __device__ __forceinline__ void c2p_sweep(const Consts<T>& k, const T (&u)[NF], 
 // select form above, identical bits for ordinary cells).  The branch-free select form for every cell (round 2, first
 // version) paid the direction-preserving scale factor (8 fp64 operations) and 8 selects per cons2prim for the ~0.2 %
 // of the cells that need them; one warp-uniform branch per four cells keeps the four chains in one basic block.
-template <typename T, int EOS, typename RL>
-__device__ __forceinline__ void c2p_group(const Consts<T>& k, T (&c0)[NF], T (&c1)[NF], T (&c2)[NF], T (&c3)[NF],
-                                          T (&v)[4], T (&p)[4], const RL& reload)
+template <typename T, typename CL>
+__device__ __forceinline__ void c2p_group(const Consts<T>& k, const T (&c0)[NF], const T (&c1)[NF], const T (&c2)[NF],
+                                          const T (&c3)[NF], T (&v)[4], T (&p)[4], const CL& cell, T* out)
 {
-    if constexpr (EOS == EOS_GAMMA) {
-        bool rare[4];
+    // Gamma-law only (the general EOS runs c2p_pairs_general / HalfStep).  `cell(j, u)` re-reads cell j of the group from
+    // shared memory, `out + 128 j` is a free 16 B slot of this lane for the redone {v, p} of cell j: the rare path is ONE
+    // rolled loop body (its four inlined copies per phase were 5.5 KB of the producer's 17 KB of code; with the emitting
+    // consumer the pair no longer fitted the instruction cache: `no_inst` 7-10 % of the stall samples of both roles).
+    unsigned rmask = 0u;
 #define SHK_C2P_FAST(J, C)                                                                      \
-        {                                                                                       \
-            const double E = (double)C[0], M1 = (double)C[1];                                   \
-            const double M2 = fma(M1, M1, fma((double)C[2], (double)C[2], (double)C[3] * (double)C[3])); \
-            const double t = E * E;                                                             \
-            rare[J] = gt_nonneg(M2, k.d.omd2 * t) | c2p_is_vacuum(E);                           \
-            const double y = c2p_fast_y(k.d, E, M2, t);                                         \
-            v[J] = (T)(M1 * y);                                                                 \
-            p[J] = (T)(k.d.gm1 * fma(-M2, y, E));                                               \
-        }
-        SHK_C2P_FAST(0, c0) SHK_C2P_FAST(1, c1) SHK_C2P_FAST(2, c2) SHK_C2P_FAST(3, c3)
+    {                                                                                           \
+        const double E = (double)C[0], M1 = (double)C[1];                                       \
+        const double M2 = fma(M1, M1, fma((double)C[2], (double)C[2], (double)C[3] * (double)C[3])); \
+        const double t = E * E;                                                                 \
+        if (gt_nonneg(M2, k.d.omd2 * t) | c2p_is_vacuum(E)) rmask |= 1u << J;                   \
+        const double y = c2p_fast_y(k.d, E, M2, t);                                             \
+        v[J] = (T)(M1 * y);                                                                     \
+        p[J] = (T)(k.d.gm1 * fma(-M2, y, E));                                                   \
+    }
+    SHK_C2P_FAST(0, c0) SHK_C2P_FAST(1, c1) SHK_C2P_FAST(2, c2) SHK_C2P_FAST(3, c3)
 #undef SHK_C2P_FAST
-        if (__any_sync(0xffffffffu, rare[0] | rare[1] | rare[2] | rare[3])) {
-            reload();                       // the cells again (from shared memory: not held in registers for this)
-            if (__any_sync(0xffffffffu, rare[0])) c2p_sweep<T, EOS>(k, c0, v[0], p[0]);
-            if (__any_sync(0xffffffffu, rare[1])) c2p_sweep<T, EOS>(k, c1, v[1], p[1]);
-            if (__any_sync(0xffffffffu, rare[2])) c2p_sweep<T, EOS>(k, c2, v[2], p[2]);
-            if (__any_sync(0xffffffffu, rare[3])) c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
+    if (__any_sync(0xffffffffu, rmask != 0u)) {
+        unsigned redone = 0u;               // warp-uniform: cells whose {v, p} were redone for the whole warp
+#pragma unroll 1
+        for (int jj = 0; jj < 4; ++jj) {
+            if (__any_sync(0xffffffffu, (rmask >> jj) & 1u)) {
+                T u[NF], vv, pp;
+                cell(jj, u);
+                c2p_sweep<T, EOS_GAMMA>(k, u, vv, pp);          // select form: same bits for ordinary cells
+                store2(out + 128 * jj, vv, pp);
+                redone |= 1u << jj;
+            }
         }
-    } else {
-        // general EOS: the sweeps use c2p_pairs_general below (one shared loop body); this form serves no kernel
-        (void)reload;
-        c2p_sweep<T, EOS>(k, c0, v[0], p[0]);
-        c2p_sweep<T, EOS>(k, c1, v[1], p[1]);
-        c2p_sweep<T, EOS>(k, c2, v[2], p[2]);
-        c2p_sweep<T, EOS>(k, c3, v[3], p[3]);
+        load_fence();
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj)
+            if (redone & (1u << jj)) load2(out + 128 * jj, v[jj], p[jj]);
     }
 }
 
@@ -766,9 +771,9 @@ struct Producer {
             {
                 T c0[NF], c1[NF], c2[NF], c3[NF], c4[NF];
                 ld.first(c0, c1, c2);
-                if (EOS == EOS_GAMMA) {
+                if constexpr (EOS == EOS_GAMMA) {
                     ld.second(c3, c4);
-                    c2p_group<T, EOS>(k, c1, c2, c3, c4, v, p, [&]() { load_fence(); ld.first(c0, c1, c2); ld.second(c3, c4); });    // S1
+                    c2p_group<T>(k, c1, c2, c3, c4, v, p, [&](int jj, T (&u)[NF]) { ld.cell(jj, u); }, scr);       // S1
                 } else {
                     c2p_pairs_general<T, EOS>(k, [&](int pi, T (&a)[NF], T (&b)[NF]) { ld.pair(pi, a, b); }, scr, v, p);
                 }
@@ -820,15 +825,11 @@ struct Producer {
                 return;
             }
             T vh[4], ph[4];
-            c2p_group<T, EOS>(k, ut[0], ut[1], ut[2], ut[3], vh, ph, [&]() {           // S3
-                load_fence();
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    load2(scr + 128 * j, ut[j][0], ut[j][1]);
-                    load2(scr + 128 * j + 64, ut[j][2], ut[j][3]);
-                    ut[j][NF - 1] = T(0);
-                }
-            });
+            c2p_group<T>(k, ut[0], ut[1], ut[2], ut[3], vh, ph, [&](int jj, T (&u)[NF]) {      // S3: U~ was parked in scr
+                load2(scr + 128 * jj, u[0], u[1]);
+                load2(scr + 128 * jj + 64, u[2], u[3]);
+                u[NF - 1] = T(0);
+            }, scr);
             if (SHK_GEOM_C) {       // A/B: the corrector's geometry in the consumer (HalfStep), the message is {v, p} at n+1/2
 #pragma unroll
                 for (int j = 0; j < 4; ++j) { msg[j][0] = vh[j]; msg[j][1] = ph[j]; msg[j][2] = T(0); msg[j][3] = T(0); }
@@ -1204,6 +1205,12 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                         b[f] = tc[f * YZ_CH * 32 + 64 * pi + 32];
                     }
                 }
+                __device__ __forceinline__ void cell(int j, T (&u)[NF]) const                   // cell j of the group
+                {
+                    u[NF - 1] = T(0);
+#pragma unroll
+                    for (int f = 0; f < NP; ++f) u[f] = tc[f * YZ_CH * 32 + 32 * j];
+                }
             } ld = {tp, tc};
             T* mq = &S.msg[g & 1][0][0][lane][0];
             pr.group(k, ld, mq, mm);
@@ -1272,7 +1279,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                 // tile; done after the four steps, when only the carried window is alive in registers
                 load_fence();
 #pragma unroll
-                for (int c = 0; c < YZ_CH; ++c) {
+                for (int c = 0; c < YZ_CH; ++c) {           // unrolled: rolled measured 0.449 vs 0.421 ms (four independent chains)
                     if (c < left) {
                         // momenta in NATURAL order (x, y, z), so that |M|^2 rounds as in the element-wise pass this replaces
                         // (same bits): slots of a y sweep hold (My, Mz, Mx), of a z sweep (Mz, Mx, My)
@@ -1442,6 +1449,12 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                     a[NF - 1] = b[NF - 1] = T(0);
 #pragma unroll
                     for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (pi ^ sw), a[f], b[f]);
+                }
+                __device__ __forceinline__ void cell(int j, T (&u)[NF]) const                   // cell j of the group
+                {
+                    u[NF - 1] = T(0);
+#pragma unroll
+                    for (int f = 0; f < NP; ++f) u[f] = tc[f * XV_TILE + 2 * ((j >> 1) ^ sw) + (j & 1)];
                 }
             } ld = {tp, tc, sw};
             T* mq = &S.msg[g & 1][0][0][lane][0];
