@@ -95,3 +95,23 @@ def test_P13_vacuum_and_projection(oracle):
     # cons2prim applies the same min internally: superluminal input gives v just below 1, e >= 0
     out, _, _ = oracle.cons2prim(1.0, 0.0, 0.0, 5.0, 1.0, 4.0 / 3.0, 0.0)
     assert 0.999999 < out[5] < 1.0 and out[0] >= 0.0
+
+
+def test_P13b_vacuum_threshold_of_reading_G7(oracle):
+    # reading G7 as amended in round 2: a cell is vacuum when !(E >= 2^-498): E^2 is not representable below.
+    # Exactly at the threshold the cell is matter; one ulp below, zero, negative and NaN are vacuum (all primitives 0, M := 0).
+    thr = 2.0 ** -498
+    below = np.nextafter(thr, 0.0)
+    for E, vac in [(thr, False), (2.0 * thr, False), (below, True), (1e-200, True), (0.0, True), (-1.0, True), (np.nan, True)]:
+        M = [0.3 * thr, -0.2 * thr, 0.1 * thr] if E == E else [0.1, 0.0, 0.0]
+        out, _, _ = oracle.cons2prim(E, *M, 1.0, 4.0 / 3.0, 0.0)
+        m, r = oracle.project(E, M)
+        if vac:
+            assert np.all(out == 0.0) and r == 2 and np.all(m == 0.0), E
+        else:
+            assert out[0] > 0.0 and r == 0 and np.all(m == np.array(M)), E
+            # matter at the threshold is ordinary matter: the closed form still holds there
+            Mabs = np.linalg.norm(M)
+            G = 4.0 / 3.0
+            v = 2 * Mabs / (G * E + np.sqrt(G * G * E * E - 4 * (G - 1) * Mabs * Mabs))
+            assert abs(out[6] - v) <= 1e-12 * v

@@ -33,6 +33,7 @@ def _table(fn):
 def test_T1_linear_table_is_the_ideal_gas(oracle):
     G, m = 5.0 / 3.0, 1.0
     tab = oracle.make_table(_table(lambda e, n: (G - 1.0) * (e - m * n)), EMAX, NMAX)
+    assert oracle.eos_table_P(tab, 0.5, 2.0) == 0.0 and oracle.eos_table_P(tab, 0.0, 0.1) == 0.0      # floored at 0 (e < m n)
     rng = np.random.default_rng(1)
     for _ in range(2000):
         e = 10.0 ** rng.uniform(-3, 1.2); n = e * rng.uniform(0.0, 0.95); v = rng.uniform(-0.99, 0.99, 3) / np.sqrt(3)
