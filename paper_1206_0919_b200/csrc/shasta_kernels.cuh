@@ -602,7 +602,7 @@ __device__ __forceinline__ void project(const EosD& k, double (&un)[NF], Cnt& co
         un[1] = un[2] = un[3] = 0.0;
         counts.add(1);
     } else if (M2 > lim * lim) {
-        const double s = lim * rsqrt(M2);
+        const double s = lim * fast_rsqrt(M2);
         un[1] *= s; un[2] *= s; un[3] *= s;
         counts.add(0);
     }
@@ -1238,9 +1238,9 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
         {                                                                                           \
             if (g >= 2 && (S_) < left) {                                                            \
                 T pv[6];                                                                            \
-                finish_cell<T, EOS, EMIT == 1>(k, UN, pv, cnt);                                     \
+                finish_cell<T, EOS, EMIT == 1 && EOS == EOS_GAMMA>(k, UN, pv, cnt);                 \
                 _Pragma("unroll") for (int f = 0; f < NF; ++f) ((T*)P.out[f])[o] = UN[f];           \
-                if (EMIT == 1) { _Pragma("unroll") for (int qq = 0; qq < 6; ++qq) ((T*)P.prim[qq])[o] = pv[qq]; } \
+                if (EMIT == 1 && EOS == EOS_GAMMA) { _Pragma("unroll") for (int qq = 0; qq < 6; ++qq) ((T*)P.prim[qq])[o] = pv[qq]; } \
             }                                                                                       \
             o += sa;                                                                                \
         }
@@ -1274,12 +1274,28 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
             load2(mq + 384, msg[0], msg[1]); load2(mq + 448, msg[2], msg[3]);
             co.template step<3>(c1, c2, msg, un);
             SHK_YZ_OUT(un, 3)
+            if (EMIT == 1 && EOS != EOS_GAMMA && g >= 2) {
+                // general EOS: the primitives of the group's four output cells in ONE rolled loop body (a full Newton solve per
+                // cell; inlined into the four steps it made the consumer 47-57 KB of code, far beyond the instruction cache).
+                // The cells are read back from global memory: this thread stored them a moment ago.
+#pragma unroll 1
+                for (int c = 0; c < YZ_CH; ++c) {
+                    if (c < left) {
+                        const long long oc = o + (long long)(c - YZ_CH) * sa;
+                        T uo[NF], pv[6];
+#pragma unroll
+                        for (int f = 0; f < NF; ++f) uo[f] = ((const T*)P.out[f])[oc];
+                        emit_primitives<T, EOS>(k, uo, pv, cnt);
+#pragma unroll
+                        for (int qq = 0; qq < 6; ++qq) ((T*)P.prim[qq])[oc] = pv[qq];
+                    }
+                }
+            }
             if (EMIT == 2 && g >= 2) {
                 // primitives of the INPUT state of this group's output cells = the four cells of the previous group's ring
                 // tile; done after the four steps, when only the carried window is alive in registers
                 load_fence();
-#pragma unroll
-                for (int c = 0; c < YZ_CH; ++c) {           // unrolled: rolled measured 0.449 vs 0.421 ms (four independent chains)
+                auto emit_in_cell = [&](int c) {
                     if (c < left) {
                         // momenta in NATURAL order (x, y, z), so that |M|^2 rounds as in the element-wise pass this replaces
                         // (same bits): slots of a y sweep hold (My, Mz, Mx), of a z sweep (Mz, Mx, My)
@@ -1298,6 +1314,13 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                         ((T*)P.prim[ysweep ? 3 : 5])[oc] = pv[4];
                         ((T*)P.prim[ysweep ? 4 : 3])[oc] = pv[5];
                     }
+                };
+                if constexpr (EOS == EOS_GAMMA) {
+#pragma unroll
+                    for (int c = 0; c < YZ_CH; ++c) emit_in_cell(c);       // unrolled: rolled measured 0.449 vs 0.421 ms (four independent chains)
+                } else {
+#pragma unroll 1
+                    for (int c = 0; c < YZ_CH; ++c) emit_in_cell(c);       // general EOS: one copy of the Newton solve (instruction cache)
                 }
             }
             if (g >= 2) left -= YZ_CH;
