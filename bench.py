@@ -40,9 +40,9 @@ HBM_FALLBACK_GBS = 6650.0       # B200_PROFILING.md fallback when MEASURED_PEAKS
 # marched cell (producer 96.1 + consumer 78.0, profiles/r2_sass_mix.md: executed-instruction counts of the ncu capture)
 # x 1.0625 marched cells per updated cell (segments of 128 re-march 8 halo cells)
 FP64_PER_CELL_SWEEP = 185.0
-# fp64 issue rate: 16 lanes per SM sub-partition = 64 results/clk/SM nominal; the round-1 micro-benchmark on this pool
-# measured 58.9 (DFMA) / 60.9 (DADD) results/clk/SM, so 60 is used as the measured ALU peak
-FP64_RESULTS_PER_CLK_SM = 60.0
+# fp64 issue rate: 16 lanes per SM sub-partition = 64 results/clk/SM nominal; measured 63.9 with the pipe saturated
+# (tests/probes/fp64_issue_probe.cu, run by test_fp64_issue_rate_probe; record in profiles/parity_r2.json)
+FP64_RESULTS_PER_CLK_SM = 63.9
 
 
 def sampler_clock_mhz(sampler):
@@ -321,7 +321,7 @@ def ours(args):
                     "unit": "G fp64 warp-lane results/s", "frac": fp64_ach / fp64_peak,
                     "per_cell_sweep": FP64_PER_CELL_SWEEP, "clock_mhz": clk,
                     "results_per_clk_sm": FP64_RESULTS_PER_CLK_SM,
-                    "note": "per-cell count and peak: profiles/r2_sass_mix.md; measured 58.9-60.9 results/clk/SM (nominal 64)"}
+                    "note": "per-cell count: profiles/r2_sass_mix.md; peak: measured 63.9 results/clk/SM (tests/probes/fp64_issue_probe.cu; nominal 64)"}
     step_gbs = value / world * B_STEP * (args.precision / 64.0) / 1e9
     step_roofline = {"bytes_per_cell_update": B_STEP * (args.precision / 64.0), "achieved": step_gbs,
                      "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,

@@ -387,6 +387,21 @@ def test_options_state_rules_and_combinations(oracle):
     assert np.allclose(p_ana, (c["gamma"] - 1.0) * e_now, rtol=1e-12, atol=0)
 
 
+def test_fp64_issue_rate_probe():
+    # the measured numbers DESIGN.md 7.1 and bench.py's alu_roofline use (FP64_RESULTS_PER_CLK_SM = 60): the probe is
+    # tests/probes/fp64_issue_probe.cu, built here with nvcc for sm_100a; its line goes to the parity record
+    import json, os, subprocess, tempfile
+    src = os.path.join(os.path.dirname(os.path.abspath(__file__)), "probes", "fp64_issue_probe.cu")
+    with tempfile.TemporaryDirectory() as d:
+        exe = os.path.join(d, "probe")
+        subprocess.run(["nvcc", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, src], check=True)
+        out = subprocess.run([exe], check=True, capture_output=True, text=True).stdout
+    r = json.loads(out.strip().splitlines()[-1])
+    parity.record("probe fp64 issue rate", {}, **r)
+    assert 6.0 <= r["dfma_dependent_latency_cycles"] <= 12.0, r
+    assert 54.0 <= r["fp64_results_per_clk_per_sm"] <= 66.0, r        # nominal 64 (16 lanes per sub-partition)
+
+
 def test_host_buffer_entry_points(oracle):
     c = inputs.random_state(21, 17, 13, seed=8, kind="smooth")
     ref, _ = parity.run_oracle(oracle, c, steps=2)
