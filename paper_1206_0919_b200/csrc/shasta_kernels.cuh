@@ -1,10 +1,12 @@
 // shasta_kernels.cuh -- sm_100a device code of the fused SHASTA sweep.
 //
 // One sweep along an axis = one kernel launch that reads the five conserved fields once and
-// writes them once (80 B/cell in fp64).  Every pencil is processed by a MARCHING thread: it walks
-// along the sweep axis with the "front" cell i and keeps a rolling register window, so every
-// quantity of eqs. (15)-(22) is computed exactly once per cell / per interface --
-// not 5x (U-hat) and 2x (A) per cell as in the paper's Listing 1.
+// writes them once (80 B/cell in fp64).  Every pencil is processed by MARCHING along the sweep axis with
+// the "front" cell i and a rolling register window, so every quantity of eqs. (15)-(22)
+// is computed exactly once per cell / per interface -- not 5x (U-hat) and 2x (A) per cell as in the
+// paper's Listing 1.  The march is run by warp PAIRS (a producer and a consumer
+// warp per 32 pencils, setmaxnreg 96/160), in groups of 4 cells fed by TMA: sweep_yz_kernel (y, z) and
+// sweep_x2_kernel (x) below; sweep_cell_kernel is the paper's one-thread-per-cell decomposition.
 //
 // Pipeline of one march step with front cell i (dependency radius 4):
 //   S1  (v,p)_i        = cons2prim(U_i)                                  phases 3-4
@@ -18,12 +20,13 @@
 // axis (source term lambda*Delta(p)), slots 2,3 = the perpendicular momenta (source
 // free), slot 4 = R.  The kernels therefore never branch on the axis.
 //
-// The kernel is bound by the fp64 pipe (64 results/clk/SM on B200, measured) about as much as by HBM
-// (DESIGN.md 7), so the arithmetic is written for a minimal fp64 instruction count:
+// The kernel is bound by the fp64 pipe (63.9 results/clk/SM on B200, measured: tests/probes) about as much
+// as by HBM, so the arithmetic is written for a minimal fp64 instruction count:
 //   * no fp64 division or library sqrt on the common path: MUFU.RCP64H / MUFU.RSQ64H seeds (2^-20,
 //     measured) + Newton steps written out below;
-//   * the flux limiter's min/max/sign run on the integer pipe (sign-magnitude ordering of doubles);
-//   * the register window rotates by NAME (march loop unrolled by 4, compile-time slots), not by moves.
+//   * the flux limiter is two DSETP with |.| modifiers + selects (limiter<double>);
+//   * vacuum / causality-clamped cells are handled behind one warp vote per four cells (c2p_group);
+//   * the register window rotates by NAME (march unrolled by 4, compile-time slots), not by moves.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
