@@ -417,6 +417,25 @@ def test_fp64_issue_rate_probe():
     assert 54.0 <= r["fp64_results_per_clk_per_sm"] <= 66.0, r        # nominal 64 (16 lanes per sub-partition)
 
 
+@pytest.mark.parametrize("mass", [0.0, 1.0])
+def test_fp32_with_batch_graph_and_general_eos(oracle, mass):
+    # the fp32 storage path through the same option combinations as fp64: batch of 2, graph cycles, both analytic EOS
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    cs = [inputs.random_state(40, 12, 10, seed=90 + b, kind="smooth", gamma=5.0 / 3.0, mass=mass) for b in range(2)]
+    c = cs[0]
+    s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], mass, batch=2, graph=1, precision=32)
+    s.set_state(*[torch.from_numpy(np.stack([cb[k] for cb in cs])).cuda() for k in ("e", "n", "vx", "vy", "vz")])
+    s.step(7)
+    got = {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
+    got.update({k: v.cpu().numpy() for k, v in s.get_primitives().items()})
+    assert s.graph_launch_count == 1
+    for b in range(2):
+        ref, _ = parity.run_oracle(oracle, cs[b], steps=7)
+        for k, (emax, el1) in parity.field_errors({k: v[b] for k, v in got.items()}, ref).items():
+            assert emax <= 2e-4 and el1 <= 5e-6, (b, k, emax, el1)      # fp32 storage: a few 1e-7 per operation, 7 steps
+
+
 def test_host_buffer_entry_points(oracle):
     c = inputs.random_state(21, 17, 13, seed=8, kind="smooth")
     ref, _ = parity.run_oracle(oracle, c, steps=2)
