@@ -148,7 +148,7 @@ int make_tensor_maps(shasta_t* h)
 {
     h->have_tmap = false;
     const size_t es = esize(h);
-    if (((size_t)h->nx * es) % 16 != 0 || h->nx < 4) return 0;
+    if (((size_t)h->nx * es) % 16 != 0 || h->nx < 8) return 0;
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
@@ -158,11 +158,11 @@ int make_tensor_maps(shasta_t* h)
     }
     const cuuint64_t dims[2] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny * (cuuint64_t)h->nz * (cuuint64_t)h->nbatch};
     const cuuint64_t strides[1] = {(cuuint64_t)h->nx * es};
-    const cuuint32_t box[2] = {(cuuint32_t)XV_CH, 32u};
+    // 32 B rows with the 32 B swizzle either way: four fp64 cells (one group of the march) or eight fp32 cells (two groups)
+    const cuuint32_t box[2] = {(cuuint32_t)(es == 8 ? XV_CH : 2 * XV_CH), 32u};
     const cuuint32_t estr[2] = {1u, 1u};
-    // fp64: rows of 32 B, 32 B swizzle; fp32: rows of 16 B (one swizzle atom), dense tiles
     const CUtensorMapDataType dt = es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-    const CUtensorMapSwizzle swz = es == 8 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE;
+    const CUtensorMapSwizzle swz = CU_TENSOR_MAP_SWIZZLE_32B;
     for (int b = 0; b < 2; ++b)
         for (int f = 0; f < NF; ++f) {
             CUresult r = ((EncodeTiledFn)fn)(&h->tmap[b][f], dt, 2, h->U[b][f], dims, strides,

@@ -1344,10 +1344,16 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
 // as it has READ it (top of its group), not when it has finished the group.
 constexpr int X2_G = 3;
 
+// fp32 storage with TMA ("SUPER" in the kernel): a ring / staging tile holds EIGHT cells of a row, [32 rows][8 cells] = the
+// same 32 B rows and 32 B swizzle as an fp64 tile, filled by one TMA box {8, 32}: a 4-cell group of the march is one half
+// of it.  With {4, 32} boxes of 16 B rows the fp32 x sweep spent 25 % of its stall samples waiting for TMA data (ncu) and
+// ran slower than the fp64 one: the TMA unit works per row piece, and 16 B pieces are the worst case.
+template <typename T> struct X2Stride { static constexpr int value = sizeof(T) == 4 ? 2 * XV_TILE : XV_TILE; };
+
 template <typename T>
 struct alignas(256) X2Pair {
-    T ring[X2_G][NF][XV_TILE];
-    T outb[NF][XV_TILE];
+    T ring[X2_G][NF][X2Stride<T>::value];
+    T outb[NF][X2Stride<T>::value];
     T msg[2][YZ_CH][2][32][2];
     unsigned long long bar[4];            // bar[q], q < 3: TMA completion of ring tile q; bar[3]: scratch (early release)
 };                                        // fp64: 28928 B; 4 pairs = 113 KB per CTA: two CTAs per SM, exactly
@@ -1384,8 +1390,13 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
     const int nsteps = (j1 - j0) + 2 * GH;
     const int ngroups = (nsteps + XV_CH - 1) / XV_CH;
     const int col = lane & 3, rsub = lane >> 2;             // element map of the LSU group copies: col, rows rsub + 8 kk
-    const int sw = sizeof(T) == 8 ? (lane >> 2) & 1 : 0;    // 32 B swizzle of this lane's row (fp64 tiles only)
+    constexpr bool SUPER = TMA && sizeof(T) == 4;           // fp32 + TMA: 8-cell tiles, a group is one half (see X2Pair)
+    constexpr int FS = X2Stride<T>::value;                // elements between the fields of a tile
+    const int sw = (sizeof(T) == 8 || SUPER) ? (lane >> 2) & 1 : 0;    // 32 B swizzle of this lane's row (32 B rows only)
     constexpr int XALIGN = 16 / (int)sizeof(T);             // cells per 16 B: TMA boxes start at 16 B aligned cells
+    // SUPER: group G is half (G + 1) & 1 of the 8-cell tile (G + 1) >> 1 of this segment, which starts at cell
+    // j0 - 8 + 8 ((G + 1) >> 1) (j0 is a multiple of 8: x segments are); element offset of (row, half h, cell c) in it:
+    auto soff = [](int row, int h, int c) { return row * 8 + 4 * (h ^ ((row >> 2) & 1)) + c; };
 
     if (producer) {
         if (sizeof(T) == 8) {
@@ -1412,6 +1423,55 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
 #pragma unroll 1
         for (int g = -1; g < ngroups; ++g) {
             if (g >= 1) bar_sync64(bar_id + 2 + ((g - 1) & 1));     // the consumer has read what it needs of group g-2
+            const T *tp, *tc;
+            if constexpr (SUPER) {
+                // fp32: 8-cell tiles.  Group G touches tile (G + 1) >> 1; a tile inside [0, N) is ONE TMA box {8, 32} per
+                // field, requested when its first group comes up (two groups ahead of its second half); a tile that touches
+                // a boundary is filled half by half through the ghost map (cp.async)
+                auto tile_x = [&](int G) { return j0 - 8 + 8 * ((G + 1) >> 1); };
+                auto tile_tma = [&](int G) { const int xs = tile_x(G); return xs >= 0 && xs + 8 <= N; };
+                auto first_touch = [&](int G) { return G == 0 || ((G + 1) & 1) == 0; };
+                const int G = g + 1;
+                if (G < ngroups) {
+                    const int hh = (G + 1) & 1, qs = ((G + 1) >> 1) % X2_G, xs = tile_x(G);
+                    if (tile_tma(G)) {
+                        if (first_touch(G) && elect_one()) {
+                            mbar_expect_tx(&S.bar[qs], NF * FS * (unsigned)sizeof(T));
+#pragma unroll
+                            for (int f = 0; f < NF; ++f)
+                                tma_load_2d(&S.ring[qs][f][0], maps.in + maps.fidx[f], xs, (int)row0, &S.bar[qs]);
+                        }
+                    } else {
+                        const int gi = ghost_index(xs + 4 * hh + col, N, P.periodic);
+                        T* dst = &S.ring[qs][0][0];
+#pragma unroll 1
+                        for (int kk = 0; kk < 4; ++kk) {
+                            const int row = rsub + 8 * kk;
+                            if (row < nrows) {
+                                const long long o = (row0 + row) * (long long)N + gi;
+                                const int so = soff(row, hh, col);
+#pragma unroll
+                                for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * FS + so, (const T*)P.in[f] + o);
+                            }
+                        }
+                        cp_async_commit();
+                    }
+                }
+                if (g < 0) continue;
+                const int hh = (g + 1) & 1, qs = ((g + 1) >> 1) % X2_G;
+                if (tile_tma(g)) {
+                    if (first_touch(g)) {
+                        mbar_wait(&S.bar[qs], (phase >> qs) & 1u);
+                        phase ^= 1u << qs;
+                    }
+                } else {
+                    if (G < ngroups && !tile_tma(G)) cp_async_wait<1>(); else cp_async_wait<0>();
+                    __syncwarp();
+                }
+                tc = &S.ring[qs][0][lane * 8 + 4 * (hh ^ sw)];
+                tp = hh ? &S.ring[qs][0][lane * 8 + 4 * sw + 3]                                   // cell 3 of half 0, same tile
+                        : &S.ring[(qs + X2_G - 1) % X2_G][0][lane * 8 + 4 * (1 ^ sw) + 3];       // cell 3 of half 1, previous tile
+            } else {
             if (g + 1 < ngroups) {
                 const int xg = ilo + XV_CH * (g + 1);
                 if (group_is_tma(g + 1)) {
@@ -1431,7 +1491,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                             const long long o = (row0 + row) * (long long)N + gi;
                             const int so = xv_off<T>(row, col);
 #pragma unroll
-                            for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * XV_TILE + so, (const T*)P.in[f] + o);
+                            for (int f = 0; f < NF; ++f) cp_async_elem<T>(dst + f * FS + so, (const T*)P.in[f] + o);
                         }
                     }
                     cp_async_commit();
@@ -1449,38 +1509,48 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                 __syncwarp();
             }
             const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;           // tile of group g-1
-            const T* tp = &S.ring[qm][0][xv_off<T>(lane, 3)];
-            const T* tc = &S.ring[q0][0][lane * 4];
+            tp = &S.ring[qm][0][xv_off<T>(lane, 3)];
+            tc = &S.ring[q0][0][lane * 4];
+            }
             T mm[4][4];
             struct {
                 const T *tp, *tc;
                 int sw;
+                // SUPER: tc points at this lane's 16 B half row (four cells): one LDS.128; else at its 4-cell row with the
+                // two 16 B halves swizzled (fp64) or dense (fp32 without TMA)
                 __device__ __forceinline__ void first(T (&um)[NF], T (&c0)[NF], T (&c1)[NF]) const
                 {
                     um[NF - 1] = c0[NF - 1] = c1[NF - 1] = T(0);
 #pragma unroll
                     for (int f = 0; f < NP; ++f) {
-                        um[f] = tp[f * XV_TILE];
-                        load2(tc + f * XV_TILE + 2 * sw, c0[f], c1[f]);
+                        um[f] = tp[f * FS];
+                        if constexpr (SUPER) load2(tc + f * FS, c0[f], c1[f]);
+                        else load2(tc + f * FS + 2 * sw, c0[f], c1[f]);
                     }
                 }
                 __device__ __forceinline__ void second(T (&c2)[NF], T (&c3)[NF]) const
                 {
                     c2[NF - 1] = c3[NF - 1] = T(0);
 #pragma unroll
-                    for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (1 ^ sw), c2[f], c3[f]);
+                    for (int f = 0; f < NP; ++f) {
+                        if constexpr (SUPER) load2(tc + f * FS + 2, c2[f], c3[f]);
+                        else load2(tc + f * FS + 2 * (1 ^ sw), c2[f], c3[f]);
+                    }
                 }
                 __device__ __forceinline__ void pair(int pi, T (&a)[NF], T (&b)[NF]) const      // cells 2 pi, 2 pi + 1
                 {
                     a[NF - 1] = b[NF - 1] = T(0);
 #pragma unroll
-                    for (int f = 0; f < NP; ++f) load2(tc + f * XV_TILE + 2 * (pi ^ sw), a[f], b[f]);
+                    for (int f = 0; f < NP; ++f) {
+                        if constexpr (SUPER) load2(tc + f * FS + 2 * pi, a[f], b[f]);
+                        else load2(tc + f * FS + 2 * (pi ^ sw), a[f], b[f]);
+                    }
                 }
                 __device__ __forceinline__ void cell(int j, T (&u)[NF]) const                   // cell j of the group
                 {
                     u[NF - 1] = T(0);
 #pragma unroll
-                    for (int f = 0; f < NP; ++f) u[f] = tc[f * XV_TILE + 2 * ((j >> 1) ^ sw) + (j & 1)];
+                    for (int f = 0; f < NP; ++f) u[f] = SUPER ? tc[f * FS + j] : tc[f * FS + 2 * ((j >> 1) ^ sw) + (j & 1)];
                 }
             } ld = {tp, tc, sw};
             T* mq = &S.msg[g & 1][0][0][lane][0];
@@ -1507,14 +1577,24 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
 #pragma unroll 1
         for (int g = 0; g < ngroups; ++g) {
             bar_sync64(bar_id + (g & 1));
-            const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;
-            const T* tp = &S.ring[qm][0][lane * 4 + 2 * (1 ^ sw)];          // cells 2, 3 of group g-1
-            const T* tc = &S.ring[q0][0][lane * 4];
+            const T *tp, *tc;
+            int ho = 0;                 // SUPER: half of the staging tile that takes this group's outputs (cells of group g-1)
+            if constexpr (SUPER) {
+                const int hh = (g + 1) & 1, qs = ((g + 1) >> 1) % X2_G;
+                tc = &S.ring[qs][0][lane * 8 + 4 * (hh ^ sw)];
+                tp = hh ? &S.ring[qs][0][lane * 8 + 4 * sw + 2]                                   // cells 2, 3 of half 0, same tile
+                        : &S.ring[(qs + X2_G - 1) % X2_G][0][lane * 8 + 4 * (1 ^ sw) + 2];       // cells 2, 3 of half 1, previous tile
+                ho = g & 1;
+            } else {
+                const int qm = (q0 == 0) ? X2_G - 1 : q0 - 1;
+                tp = &S.ring[qm][0][lane * 4 + 2 * (1 ^ sw)];           // cells 2, 3 of group g-1
+                tc = &S.ring[q0][0][lane * 4];
+            }
             T* mq = &S.msg[g & 1][0][0][lane][0];
             q0 = (q0 + 1 == X2_G) ? 0 : q0 + 1;
             T uq[NF], ua[NF], c0[NF], c1[NF], c2[NF], msg[4], un[NF], uo[NF];
 #pragma unroll
-            for (int f = 0; f < NF; ++f) load2(tp + f * XV_TILE, uq[f], ua[f]);
+            for (int f = 0; f < NF; ++f) load2(tp + f * FS, uq[f], ua[f]);
             // Early release of the tile of group g-1 (the producer's next TMA request refills it).  BAR.ARV does NOT wait
             // for shared-memory loads in flight (measured: issued right behind the LDS, 2.6 % of the cells of a 256^3
             // sweep then differed from run to run), so a 4-byte store whose data depends on all five loads goes first:
@@ -1527,36 +1607,54 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
             }
             const int jf = ilo + XV_CH * g - GH;                            // first output cell of this group
             const bool any_out = g >= 2;                                    // jf >= j0
-            if (TMA && store_pending) {                                     // outb is rewritten below: the TMA must have read it
+            if (TMA && store_pending && (!SUPER || ho == 0)) {              // outb is rewritten below: the TMA must have read it
                 if (lane == 0) tma_store_wait_read();
                 __syncwarp();
                 store_pending = false;
             }
-            T* ob = &S.outb[0][lane * 4];
+            // first and second cell pair of this lane's row in the staging tile
+            T* ob = SUPER ? &S.outb[0][lane * 8 + 4 * (ho ^ sw)] : &S.outb[0][lane * 4 + 2 * sw];
+            T* ob2 = SUPER ? ob + 2 : &S.outb[0][lane * 4 + 2 * (1 ^ sw)];
             if constexpr (EOS != EOS_GAMMA || SHK_GEOM_C) hs.group(k, mq);       // S3 + geometry (general EOS)
             load2(mq, msg[0], msg[1]); load2(mq + 64, msg[2], msg[3]);
             co.template step<0>(uq, ua, msg, uo);
             if (any_out && jf < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, uo, pv, cnt); }
             load_fence();
 #pragma unroll
-            for (int f = 0; f < NF; ++f) load2(tc + f * XV_TILE + 2 * sw, c0[f], c1[f]);
+            for (int f = 0; f < NF; ++f) load2(tc + f * FS + (SUPER ? 0 : 2 * sw), c0[f], c1[f]);
             load2(mq + 128, msg[0], msg[1]); load2(mq + 192, msg[2], msg[3]);
             co.template step<1>(ua, c0, msg, un);
             if (any_out && jf + 1 < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, un, pv, cnt); }
 #pragma unroll
-            for (int f = 0; f < NF; ++f) store2(ob + f * XV_TILE + 2 * sw, uo[f], un[f]);
+            for (int f = 0; f < NF; ++f) store2(ob + f * FS, uo[f], un[f]);
             load2(mq + 256, msg[0], msg[1]); load2(mq + 320, msg[2], msg[3]);
             co.template step<2>(c0, c1, msg, uo);
             if (any_out && jf + 2 < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, uo, pv, cnt); }
             load_fence();
 #pragma unroll
-            for (int f = 0; f < NF; ++f) c2[f] = tc[f * XV_TILE + 2 * (1 ^ sw)];
+            for (int f = 0; f < NF; ++f) c2[f] = tc[f * FS + (SUPER ? 2 : 2 * (1 ^ sw))];
             load2(mq + 384, msg[0], msg[1]); load2(mq + 448, msg[2], msg[3]);
             co.template step<3>(c1, c2, msg, un);
             if (any_out && jf + 3 < j1 && lane < nrows) { T pv[6]; finish_cell<T, EOS, false>(k, un, pv, cnt); }
 #pragma unroll
-            for (int f = 0; f < NF; ++f) store2(ob + f * XV_TILE + 2 * (1 ^ sw), uo[f], un[f]);
+            for (int f = 0; f < NF; ++f) store2(ob2 + f * FS, uo[f], un[f]);
             if (!any_out) continue;
+            if constexpr (SUPER && !EMIT) {
+                // fp32: the staging tile holds eight cells; it leaves as one TMA box {8, 32} per field when its second half
+                // is done (segments are multiples of 8 cells), or after its first half at the ragged end of the grid, where
+                // the box is clipped at N (then j1 == N <= jf + 4, so the stale second half lies outside the grid)
+                if (ho == 1 || g == ngroups - 1) {
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) {
+#pragma unroll
+                        for (int f = 0; f < NF; ++f) tma_store_2d(maps.out + maps.fidx[f], jf - 4 * ho, (int)row0, &S.outb[f][0]);
+                        tma_store_commit();
+                    }
+                    store_pending = true;
+                }
+                continue;
+            }
             // the finished group leaves as one TMA box per field when all of its cells are output cells of this segment (or
             // are clipped by the grid edge); otherwise (ragged segment end, odd start, EMIT) through the LSU
             if (TMA && !EMIT && (jf % XALIGN) == 0 && (jf + XV_CH <= j1 || j1 == N)) {
@@ -1577,7 +1675,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
                         const int row = rsub + 8 * kk;
                         if (row < nrows) {
                             const long long o = (row0 + row) * (long long)N + jo;
-                            const int so = xv_off<T>(row, col);
+                            const int so = SUPER ? soff(row, ho, col) : xv_off<T>(row, col);
                             T u[NF];
 #pragma unroll
                             for (int f = 0; f < NF; ++f) {
