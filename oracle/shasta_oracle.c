@@ -69,6 +69,7 @@ typedef struct oracle_shasta {
     int bc;
     int predictor;                /* 0 = R1 (reading G4): predictor = eq. (17) alone; 1 = R2: predictor = eqs. (17)-(22) */
     double diff;                  /* Listing 1 'diff': factor on A^ph; 1 = paper default, 0 = "n/af" */
+    int adkind;                   /* antidiffusion term: 0 = phoenical (eq. (19), default), 1 = explicit (PAPER.md:123 footnote) */
     long long step_index;
     int table[64];
     int ntable;
@@ -228,8 +229,12 @@ static double min3(double a, double b, double c)
 /* Phoenical antidiffusion with flux limiter on ONE field of an extended pencil.
    Unew[j] is written for j = lo..hi-1; needs Uhat at j-2..j+2 and U at j-3..j+3
    (Fig. 3).  diff multiplies A^ph (Listing 1 'diff', reading G13). */
-void oracle_antidiffuse(int n, const double *U, const double *Uhat, double diff,
-                        double *Unew, int lo, int hi)
+/* kind 0 = the paper's phoenical term, eq. (19); kind 1 = the EXPLICIT antidiffusion of the original SHASTA (Boris & Book:
+   A^ex_j = 1/8 Dhat_j), the best known of the "different anti-diffusion terms [that] are possible" of the paper's footnote 1
+   (the paper names none of them: SURVEY.md 8(f) f2).  At rest it leaves the residual damping -1/64 delta^4 U
+   that the phoenical term removes (pin: tests/test_oracle_variants.py). */
+void oracle_antidiffuse_kind(int n, const double *U, const double *Uhat, double diff, int kind,
+                             double *Unew, int lo, int hi)
 {
     (void)n;
     for (int j = lo; j < hi; ++j) {
@@ -243,13 +248,20 @@ void oracle_antidiffuse(int n, const double *U, const double *Uhat, double diff,
             double Dip = U[i + 2] - U[i + 1];
             double Dim = U[i] - U[i - 1];
             /* eq. (19), evaluation order of reading G14 */
-            double Aph = diff * (0.125 * (Dh - 0.125 * ((Dip + Dim) - 2.0 * Di)));
+            double Aph = kind == 0 ? diff * (0.125 * (Dh - 0.125 * ((Dip + Dim) - 2.0 * Di)))
+                                   : diff * (0.125 * Dh);
             double s = sgn(Aph);                            /* eq. (20) */
             double m = min3(s * Dhp, fabs(Aph), s * Dhm);
             A[k] = s * (m > 0.0 ? m : 0.0);                 /* eq. (21) */
         }
         Unew[j] = Uhat[j] - A[1] + A[0];                    /* eq. (22) */
     }
+}
+
+void oracle_antidiffuse(int n, const double *U, const double *Uhat, double diff,
+                        double *Unew, int lo, int hi)
+{
+    oracle_antidiffuse_kind(n, U, Uhat, diff, 0, Unew, lo, hi);
 }
 
 /* ------------------------------------------------------------ boundary --- */
@@ -270,9 +282,9 @@ static int ghost_index(int j, int N, int bc)
      predictor  0 = R1 (reading G4, the default): half step = eq. (17) alone with lambda/2;
                 1 = R2: half step = the complete kernel with lambda/2, i.e. eq. (17) AND eqs. (18)-(22), which is what
                 Listing 2 suggests (the ordinary prop kernels run after half_cfl).  Radius 6. */
-void oracle_sweep_pencil_eos(int N, double *U[NF], int a, double lambda, double gamma,
-                             double mass, int bc, unsigned long long counts[2], double diff, int predictor,
-                             const eos_table_t *tab)
+void oracle_sweep_pencil_full(int N, double *U[NF], int a, double lambda, double gamma,
+                              double mass, int bc, unsigned long long counts[2], double diff, int predictor,
+                              const eos_table_t *tab, int adkind)
 {
     const int g = predictor ? G2 : G;         /* ghost depth */
     const int NE = N + 2 * g;                 /* extended length, j = -g .. N+g-1 at offset +g */
@@ -313,7 +325,7 @@ void oracle_sweep_pencil_eos(int N, double *U[NF], int a, double lambda, double 
         } else {
             /* R2: transport j = -5 .. N+4, then eqs. (18)-(22) j = -3 .. N+2 */
             oracle_transport(NE, Ue[f], eps, src, h, Up[f], h_lo - 2, h_hi + 2);
-            oracle_antidiffuse(NE, Ue[f], Up[f], diff, Ut[f], h_lo, h_hi);
+            oracle_antidiffuse_kind(NE, Ue[f], Up[f], diff, adkind, Ut[f], h_lo, h_hi);
         }
     }
     /* 4. half-step primitives, j = -3 .. N+2 */
@@ -331,7 +343,7 @@ void oracle_sweep_pencil_eos(int N, double *U[NF], int a, double lambda, double 
     }
     /* 6.+7. antidiffusion, limiter, update: j = 0 .. N-1 */
     for (int f = 0; f < NF; ++f)
-        oracle_antidiffuse(NE, Ue[f], Uh[f], diff, Un[f], g, g + N);
+        oracle_antidiffuse_kind(NE, Ue[f], Uh[f], diff, adkind, Un[f], g, g + N);
     /* 8. relativistic correction Pi written back (reading G8) */
     for (int j = 0; j < N; ++j) {
         double M[3] = { Un[1][g + j], Un[2][g + j], Un[3][g + j] };
@@ -342,6 +354,13 @@ void oracle_sweep_pencil_eos(int N, double *U[NF], int a, double lambda, double 
         U[4][j] = Un[4][g + j];
     }
     free(buf);
+}
+
+void oracle_sweep_pencil_eos(int N, double *U[NF], int a, double lambda, double gamma,
+                             double mass, int bc, unsigned long long counts[2], double diff, int predictor,
+                             const eos_table_t *tab)
+{
+    oracle_sweep_pencil_full(N, U, a, lambda, gamma, mass, bc, counts, diff, predictor, tab, 0);
 }
 
 void oracle_sweep_pencil_ex(int N, double *U[NF], int a, double lambda, double gamma,
@@ -413,7 +432,8 @@ int oracle_set_eos_table(oracle_t *o, const double *p, int ne, int nn, double e_
     o->have_tab = 1;
     return 0;
 }
-/* keys: 0 boundary (0 outflow, 1 periodic), 1 EOS mass m, 3 step index, 4 predictor (0 = R1, 1 = R2), 5 diff >= 0 */
+/* keys: 0 boundary (0 outflow, 1 periodic), 1 EOS mass m, 3 step index, 4 predictor (0 = R1, 1 = R2), 5 diff >= 0,
+   6 antidiffusion term (0 = phoenical, 1 = explicit) */
 int oracle_set_option(oracle_t *o, int key, double value)
 {
     if (!o) return -1;
@@ -423,6 +443,7 @@ int oracle_set_option(oracle_t *o, int key, double value)
     case 3: if (value < 0.0) return -1; o->step_index = (long long)value; return 0;
     case 4: if (value != 0.0 && value != 1.0) return -1; o->predictor = (int)value; return 0;
     case 5: if (!(value >= 0.0)) return -1; o->diff = value; return 0;
+    case 6: if (value != 0.0 && value != 1.0) return -1; o->adkind = (int)value; return 0;
     default: return -1;
     }
 }
@@ -487,8 +508,8 @@ static void sweep_grid(oracle_t *o, int a)
             for (int j = 0; j < N; ++j) P[f][j] = o->U[f][base + j * stride[a]];
         }
         unsigned long long cnt[2] = { 0, 0 };
-        oracle_sweep_pencil_eos(N, P, a, o->lambda, o->gamma, o->mass, o->bc, cnt, o->diff, o->predictor,
-                                o->have_tab ? &o->tab : NULL);
+        oracle_sweep_pencil_full(N, P, a, o->lambda, o->gamma, o->mass, o->bc, cnt, o->diff, o->predictor,
+                                 o->have_tab ? &o->tab : NULL, o->adkind);
         for (int f = 0; f < NF; ++f)
             for (int j = 0; j < N; ++j) o->U[f][base + j * stride[a]] = P[f][j];
         c0 += cnt[0]; c1 += cnt[1];

@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "shasta_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle_shasta.so")
 
-BOUNDARY, EOS_MASS, STEP_INDEX, PREDICTOR, DIFF = 0, 1, 3, 4, 5
+BOUNDARY, EOS_MASS, STEP_INDEX, PREDICTOR, DIFF, ANTIDIFFUSION = 0, 1, 3, 4, 5, 6
+PHOENICAL, EXPLICIT = 0, 1
 R1, R2 = 0, 1
 OUTFLOW, PERIODIC = 0, 1
 BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
@@ -81,6 +82,7 @@ def lib(variant: str = "strict"):
         L.oracle_qminus.argtypes = [C.c_double, C.c_double]
         L.oracle_transport.argtypes = [C.c_int, _dp, _dp, _dp, C.c_double, _dp, C.c_int, C.c_int]
         L.oracle_antidiffuse.argtypes = [C.c_int, _dp, _dp, C.c_double, _dp, C.c_int, C.c_int]
+        L.oracle_antidiffuse_kind.argtypes = [C.c_int, _dp, _dp, C.c_double, C.c_int, _dp, C.c_int, C.c_int]
         L.oracle_prim2cons.argtypes = [C.c_double] * 7 + [_dp]
         L.oracle_cons2prim.restype = C.c_int
         L.oracle_cons2prim.argtypes = [C.c_double] * 7 + [_dp, C.POINTER(C.c_int)]
@@ -90,6 +92,9 @@ def lib(variant: str = "strict"):
                                           C.c_double, C.c_int, C.POINTER(C.c_ulonglong)]
         L.oracle_sweep_pencil_ex.argtypes = [C.c_int, C.POINTER(_dp), C.c_int, C.c_double, C.c_double,
                                              C.c_double, C.c_int, C.POINTER(C.c_ulonglong), C.c_double, C.c_int]
+        L.oracle_sweep_pencil_full.argtypes = [C.c_int, C.POINTER(_dp), C.c_int, C.c_double, C.c_double,
+                                               C.c_double, C.c_int, C.POINTER(C.c_ulonglong), C.c_double, C.c_int,
+                                               C.POINTER(EosTable), C.c_int]
         L.oracle_set_eos_table.argtypes = [C.c_void_p, _dp, C.c_int, C.c_int, C.c_double, C.c_double]
         L.oracle_eos_table_P.restype = C.c_double
         L.oracle_eos_table_P.argtypes = [C.POINTER(EosTable), C.c_double, C.c_double]
@@ -146,10 +151,13 @@ def transport(U, eps, f, lam, lo, hi):
     return out
 
 
-def antidiffuse(U, Uhat, lo, hi, diff=1.0):
+def antidiffuse(U, Uhat, lo, hi, diff=1.0, kind=PHOENICAL):
     U, Uhat = _arr(U), _arr(Uhat)
     out = np.zeros_like(U)
-    lib().oracle_antidiffuse(len(U), _p(U), _p(Uhat), diff, _p(out), lo, hi)
+    if kind == PHOENICAL:
+        lib().oracle_antidiffuse(len(U), _p(U), _p(Uhat), diff, _p(out), lo, hi)
+    else:
+        lib().oracle_antidiffuse_kind(len(U), _p(U), _p(Uhat), diff, kind, _p(out), lo, hi)
     return out
 
 
@@ -190,13 +198,15 @@ def project(E, M):
     return m, r
 
 
-def sweep_pencil(U5, axis, lam, gamma, mass=0.0, bc=OUTFLOW, diff=1.0, predictor=R1):
+def sweep_pencil(U5, axis, lam, gamma, mass=0.0, bc=OUTFLOW, diff=1.0, predictor=R1, antidiffusion=PHOENICAL):
     """U5: (5, N) array; returns the swept copy and the counts [Pi fired, vacuum]."""
     U5 = np.array(U5, dtype=np.float64, order="C")
     N = U5.shape[1]
     ptrs = (_dp * 5)(*[_p(U5[f]) for f in range(5)])
     cnt = (C.c_ulonglong * 2)(0, 0)
-    if diff == 1.0 and predictor == R1:
+    if antidiffusion != PHOENICAL:
+        lib().oracle_sweep_pencil_full(N, ptrs, axis, lam, gamma, mass, bc, cnt, diff, predictor, None, antidiffusion)
+    elif diff == 1.0 and predictor == R1:
         lib().oracle_sweep_pencil(N, ptrs, axis, lam, gamma, mass, bc, cnt)
     else:
         lib().oracle_sweep_pencil_ex(N, ptrs, axis, lam, gamma, mass, bc, cnt, diff, predictor)
@@ -217,7 +227,7 @@ class Oracle:
     """Same call sequence as the product's C ABI (include/shasta.h) with host arrays."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, variant="strict",
-                 predictor=R1, diff=1.0, eos_table=None):
+                 predictor=R1, diff=1.0, eos_table=None, antidiffusion=PHOENICAL):
         self._L = lib(variant)
         self.shape = (nz, ny, nx)
         self._h = self._L.oracle_create(nx, ny, nz, dx, lam, eos_gamma)
@@ -229,6 +239,8 @@ class Oracle:
             self.set_option(PREDICTOR, predictor)
         if diff != 1.0:
             self.set_option(DIFF, diff)
+        if antidiffusion != PHOENICAL:
+            self.set_option(ANTIDIFFUSION, antidiffusion)
         if eos_table is not None:           # (p2d (nn, ne), e_max, n_max)
             a = np.ascontiguousarray(eos_table[0], dtype=np.float64)
             self._chk(self._L.oracle_set_eos_table(self._h, _p(a), a.shape[1], a.shape[0], float(eos_table[1]),

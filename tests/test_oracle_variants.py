@@ -5,6 +5,9 @@ diff      PAPER.md:159, 279 (`const float diff = 1.0f`, "fine controlled applica
           update is U^{n+1} - U^n = (1 - diff) * 1/8 * second difference of U, exactly (eqs. (17)-(22) with Q+- = 1/2).
 n/af      PAPER.md:201-205 (Fig. 7 "n/af": no anti-flux) = diff 0.  Pin: equals P3's closed form for uniform eps
           (Lax-Wendroff + 1/8 diffusion, the textbook SHASTA transport stage).
+explicit  PAPER.md:123, footnote 1 ("Different anti-diffusion terms are possible"): the explicit term of the original SHASTA,
+          A^ex_j = 1/8 Dhat_j (Boris & Book).  Pin (textbook property): at rest, limiter inactive, the explicit scheme leaves
+          the residual damping U^{n+1} - U^n = -1/64 delta^4 U, where the phoenical one gives exactly 0 (P4).
 R2        PAPER.md:302-313 (Listing 2 runs the ordinary prop kernels after half_cfl): the half step is the whole
           kernel with lambda/2, eq. (17) AND eqs. (18)-(22).  Pins: P14 (acoustic wave) must still give order >= 1.8;
           the Riemann problem converges to the exact solution (P8 gates); R2 differs from R1 (the option is live).
@@ -118,3 +121,26 @@ def test_diff_below_one_adds_viscosity_monotonically(oracle):
         over.append(p["vx"].max()); l1.append(err)
     assert over[0] >= over[1] >= over[2] >= over[3]
     assert l1[3] > l1[0]
+
+
+def test_explicit_antidiffusion_leaves_the_fourth_difference_at_rest(oracle):
+    # v = 0, uniform pressure: U^ = U + 1/8 d2 U; explicit antidiffusion removes 1/8 d2 U^  ->  U^{n+1} = U - 1/64 d4 U
+    N = 48
+    x = np.arange(N, dtype=np.float64)
+    n = 1.0 + 0.02 * x + 0.0004 * x * x + 2e-7 * x ** 4             # monotone and smooth: the limiter does not bind
+    U = np.array([oracle.prim2cons(1.0, n[j], 0.0, 0.0, 0.0, GAM) for j in range(N)]).T.copy()
+    V, _ = oracle.sweep_pencil(U, 0, 0.4, GAM, bc=oracle.OUTFLOW, antidiffusion=oracle.EXPLICIT)
+    W, _ = oracle.sweep_pencil(U, 0, 0.4, GAM, bc=oracle.OUTFLOW)
+    R0 = U[4]
+    d4 = np.zeros_like(R0)
+    d4[2:-2] = R0[4:] - 4 * R0[3:-1] + 6 * R0[2:-2] - 4 * R0[1:-3] + R0[:-4]
+    inner = slice(6, -6)
+    assert np.max(np.abs(d4[inner])) > 1e-6                          # the pin has something to see
+    assert np.max(np.abs((V[4] - R0)[inner] + d4[inner] / 64.0)) <= 1e-15 * np.abs(R0).max()
+    assert np.max(np.abs((W[4] - R0)[inner])) <= 4e-16 * np.abs(R0).max()        # phoenical: nothing left (P4)
+    # the building block alone, against the formula retyped: A = 1/8 (U^_{j+1} - U^_j) where the limiter is inactive
+    Uh = R0 + 0.0
+    Uh[1:-1] = R0[1:-1] + 0.125 * ((R0[2:] - R0[1:-1]) - (R0[1:-1] - R0[:-2]))
+    out = oracle.antidiffuse(R0, Uh, 4, N - 4, kind=oracle.EXPLICIT)
+    want = Uh[4:N - 4] - 0.125 * ((Uh[5:N - 3] - Uh[4:N - 4]) - (Uh[4:N - 4] - Uh[3:N - 5]))
+    assert np.max(np.abs(out[4:N - 4] - want)) <= 4e-16 * np.abs(R0).max()
