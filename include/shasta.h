@@ -163,7 +163,31 @@ long long shasta_step_index(const shasta_t* h);
  * says that the sweep fills its shared-memory tiles without TMA (no 16 B row strides, SHASTA_NO_TMA, ...). */
 const char* shasta_kernel_name(const shasta_t* h, int axis);
 
-const char* shasta_last_error(const shasta_t* h);   /* h may be NULL: error of the last failed create */
+const char* shasta_last_error(const shasta_t* h);   /* h may be NULL: error of the last failed create or handle-less
+                                                       call (shasta_conserved_totals_static) on this thread */
+
+/*
+ * The conserved totals of eqs. (12)-(14) for callers that may not allocate: CUDA-graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc.  No handle; this call makes no cudaMalloc, cudaMallocHost, cudaFree
+ * or allocating library call, and does not synchronise.
+ *   ncell                 number of cells, 0 <= ncell <= shasta_conserved_totals_static_max_cells() = 2^26 = 67 108 864
+ *                         (a 406^3 grid; 256^3 is 2^24).  Beyond that: SHASTA_EINVAL, nothing launched.
+ *   E_dev .. R_dev        DEVICE pointers, ncell doubles each (the caller's; read only)
+ *   dv                    cell volume dx^3
+ *   totals_dev            DEVICE pointer to 5 doubles (the caller's): dv * sum of E, Mx, My, Mz, R, compensated fp64
+ *                         summation; written asynchronously on `stream`
+ * Scratch: the per-block partial sums (which shasta_conserved_totals keeps in memory its handle allocated) live in a
+ * file-scope `static __device__` array of 320 KiB that every GPU loading libshasta.so holds until the process exits;
+ * its address is looked up once per device, on the first call made with that device current (make that first call
+ * outside stream capture).  All calls on a device share the array and it keeps the last call's contents; nothing in
+ * it has to start at zero (every slot a call reads it has written before).  Calls that can overlap on the GPU --
+ * different streams, or graph branches, without an ordering between them -- RACE on it: order them.  The pointers
+ * must belong to the current device.  Errors are reported through shasta_last_error(NULL).
+ */
+int shasta_conserved_totals_static(long long ncell, const double* E_dev, const double* Mx_dev, const double* My_dev,
+                                   const double* Mz_dev, const double* R_dev, double dv, double* totals_dev,
+                                   void* stream);
+long long shasta_conserved_totals_static_max_cells(void);
 
 #ifdef __cplusplus
 }

@@ -8,6 +8,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 using namespace shk;
@@ -1087,5 +1088,102 @@ const char* shasta_kernel_name(const shasta_t* h, int axis)
 }
 
 const char* shasta_last_error(const shasta_t* h) { return h ? h->err : g_create_err; }
+
+}  // extern "C"
+
+// ---------------------------------------------------------------- conserved totals without any allocation
+// shasta_conserved_totals_static: the block partial sums of totals_kernel go to a file-scope device array instead of
+// the handle's cudaMalloc'ed d_partial, and a second small kernel folds them on the device (the handle path folds
+// them on the host through pinned memory, also an allocation).  One block per STATIC_CHUNK cells, so the array's
+// size bounds the grid: STATIC_MAX_CELLS.
+namespace {
+
+constexpr int STATIC_CHUNK = RED_THREADS * 64;                 // cells one block sums (64 per thread)
+constexpr int STATIC_MAX_BLOCKS = 4096;
+constexpr long long STATIC_MAX_CELLS = (long long)STATIC_CHUNK * STATIC_MAX_BLOCKS;   // 2^26 = 67 108 864 (406^3)
+
+// 4096 * 5 * 2 doubles = 320 KiB on every GPU that loads the library, until exit.  In host code this name is only a
+// stand-in for the symbol: kernels get the address cudaGetSymbolAddress returns (static_partial_ptr below).
+static __device__ __align__(256) double g_static_partial[STATIC_MAX_BLOCKS * NF * 2];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+double* g_static_ptr[STATIC_MAX_DEVICES] = {};                 // device address of g_static_partial, per device
+std::mutex g_static_mutex;
+
+// address of the array on the CURRENT device, looked up once per device
+int static_partial_ptr(double** out)
+{
+    shasta_t* h = nullptr;                                      // CK/fail report to shasta_last_error(NULL)
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES)
+        return fail(h, SHASTA_EINVAL, "shasta_conserved_totals_static: device %d beyond the %d this build tracks", dev,
+                    STATIC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        double* p = nullptr;
+        CK(cudaGetSymbolAddress((void**)&p, g_static_partial));
+        if (!p) return fail(h, SHASTA_ECUDA, "cudaGetSymbolAddress(g_static_partial) returned NULL on device %d", dev);
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return 0;
+}
+
+// fold `nblocks` (sum, compensation) pairs per field: warp f takes field f; out[f] = dv * total
+__global__ void __launch_bounds__(32 * NF) totals_fold_kernel(int nblocks, const double* __restrict__ partial, double dv,
+                                                              double* __restrict__ out)
+{
+    const int f = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double s = 0.0, c = 0.0;
+    for (int b = lane; b < nblocks; b += 32) {
+        const double x = partial[(b * NF + f) * 2 + 0];
+        const double t = s + x;
+        c += partial[(b * NF + f) * 2 + 1] + ((fabs(s) >= fabs(x)) ? ((s - t) + x) : ((x - t) + s));
+        s = t;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        const double so = __shfl_down_sync(0xffffffffu, s, o);
+        const double co = __shfl_down_sync(0xffffffffu, c, o);
+        const double t = s + so;
+        c += co + ((fabs(s) >= fabs(so)) ? ((s - t) + so) : ((so - t) + s));
+        s = t;
+    }
+    if (lane == 0) out[f] = dv * (s + c);
+}
+
+}  // namespace
+
+extern "C" {
+
+long long shasta_conserved_totals_static_max_cells(void) { return STATIC_MAX_CELLS; }
+
+int shasta_conserved_totals_static(long long ncell, const double* E_dev, const double* Mx_dev, const double* My_dev,
+                                   const double* Mz_dev, const double* R_dev, double dv, double* totals_dev, void* stream)
+{
+    shasta_t* h = nullptr;
+    if (ncell < 0) return fail(h, SHASTA_EINVAL, "shasta_conserved_totals_static: ncell = %lld < 0", ncell);
+    if (ncell > STATIC_MAX_CELLS)
+        return fail(h, SHASTA_EINVAL,
+                    "shasta_conserved_totals_static: ncell = %lld exceeds the %lld cells the static scratch array covers "
+                    "(use shasta_conserved_totals of a handle)", ncell, STATIC_MAX_CELLS);
+    if (!totals_dev) return fail(h, SHASTA_EINVAL, "shasta_conserved_totals_static: NULL output");
+    if (ncell > 0 && (!E_dev || !Mx_dev || !My_dev || !Mz_dev || !R_dev))
+        return fail(h, SHASTA_EINVAL, "shasta_conserved_totals_static: NULL field");
+    double* partial = nullptr;
+    int rc = static_partial_ptr(&partial);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nblocks = (int)((ncell + STATIC_CHUNK - 1) / STATIC_CHUNK);
+    // every slot [0, nblocks) is written by the first kernel before the second reads it (stream order), and no slot
+    // beyond is read: nothing in the array has to start at zero, whatever the previous call left there
+    if (nblocks > 0) {
+        totals_kernel<double><<<nblocks, RED_THREADS, 0, st>>>(ncell, E_dev, Mx_dev, My_dev, Mz_dev, R_dev, partial);
+        CK(cudaGetLastError());
+    }
+    totals_fold_kernel<<<1, 32 * NF, 0, st>>>(nblocks, partial, dv, totals_dev);
+    CK(cudaGetLastError());
+    return 0;
+}
 
 }  // extern "C"

@@ -23,6 +23,7 @@ SYMBOLS = (
     "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_step", "shasta_sweep",
     "shasta_get_primitives", "shasta_get_primitives_host", "shasta_conserved_totals", "shasta_diagnostics",
     "shasta_launch_count", "shasta_graph_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
+    "shasta_conserved_totals_static", "shasta_conserved_totals_static_max_cells",
 )
 
 _lib = None
@@ -65,6 +66,9 @@ def load():
     L.shasta_kernel_name.restype = C.c_char_p
     L.shasta_last_error.argtypes = [_vp]
     L.shasta_last_error.restype = C.c_char_p
+    L.shasta_conserved_totals_static.argtypes = [C.c_longlong] + [_dp] * 5 + [C.c_double, _dp, _vp]
+    L.shasta_conserved_totals_static_max_cells.argtypes = []
+    L.shasta_conserved_totals_static_max_cells.restype = C.c_longlong
     _lib = L
     return L
 
@@ -95,6 +99,24 @@ def _host(t):
     if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
         raise ValueError("expected a contiguous float64 CPU tensor")
     return C.c_void_p(t.data_ptr())
+
+
+def conserved_totals_static_max_cells():
+    return int(load().shasta_conserved_totals_static_max_cells())
+
+
+def conserved_totals_static(E, Mx, My, Mz, R, dv, out, stream=None):
+    """shasta_conserved_totals_static: dv * sums of five float64 CUDA tensors into `out` (5 doubles, CUDA), no allocation,
+    asynchronous on `stream`.  Marshalling only; sizes beyond the static scratch array raise ShastaError."""
+    L = load()
+    n = E.numel()
+    if any(t.numel() != n for t in (Mx, My, Mz, R)) or out.numel() != 5:
+        raise ValueError("five fields of equal size and an output of 5 doubles expected")
+    rc = L.shasta_conserved_totals_static(n, _dev(E), _dev(Mx), _dev(My), _dev(Mz), _dev(R), float(dv), _dev(out),
+                                          _stream_ptr(stream))
+    if rc != 0:
+        raise ShastaError(f"shasta_conserved_totals_static failed ({rc}): {L.shasta_last_error(None).decode()}")
+    return out
 
 
 class Shasta:
