@@ -71,6 +71,11 @@ typedef struct shasta shasta_t;   /* opaque */
                                  replayed; 2 (default) = 1 for grids below 2^22 cells, where a sweep lasts ~10 us and the
                                  "orchestration overhead" of PAPER.md:155 shows, else 0.  Same kernels, same results.  */
 
+#define SHASTA_ANTIDIFFUSION 14 /* 0 (default) = phoenical antidiffusion, eq. (19): A = diff/8 (D^ - 1/8 (D_{j+1} - 2 D_j + D_{j-1}));
+                                 1 = explicit antidiffusion, A = diff/8 D^ (differences of the transported-diffused field
+                                 only): the variant of PAPER.md:123, footnote 1.  Same kernels: the
+                                 coefficient of the second difference is a kernel constant (-1/8 or 0)                 */
+
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only
  * (eqs. (15)-(17)); dx enters shasta_conserved_totals.  0 < lambda <= 0.5

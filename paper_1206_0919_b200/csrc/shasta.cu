@@ -34,6 +34,7 @@ struct shasta {
     int tab_ne, tab_nn;
     double tab_de, tab_dn;
     double diff;            // factor on the antidiffusive flux; 1 by default
+    int explicit_ad;        // SHASTA_ANTIDIFFUSION: 0 = phoenical eq. (19) (default), 1 = explicit (PAPER.md:123 footnote 1)
     int cell_path;          // 1 = run the per-cell kernels also for the default scheme (A/B datapoint, tests)
     int predictor;          // 0 = R1 (eq. (17) alone), 1 = R2 (complete kernel at lambda/2): per-cell kernels
     int periodic;
@@ -250,6 +251,7 @@ Consts<T> make_consts(const shasta_t* h)
     k.hlam = (T)(0.5 * h->lambda);
     k.qlam = (T)(0.25 * h->lambda);
     k.aq = (T)(0.125 * h->diff);
+    k.ad2 = h->explicit_ad ? (T)0 : (T)-0.125;
     k.d.gam = h->gamma;
     k.d.gm1 = h->gamma - 1.0;
     k.d.g2 = h->gamma * h->gamma;
@@ -804,6 +806,11 @@ int shasta_set_option(shasta_t* h, int key, double value)
         return 0;
     case SHASTA_CELL_PATH:
         h->cell_path = value != 0.0;
+        return 0;
+    case SHASTA_ANTIDIFFUSION:
+        if (value != 0.0 && value != 1.0)
+            return fail(h, SHASTA_EINVAL, "SHASTA_ANTIDIFFUSION must be 0 (phoenical) or 1 (explicit)");
+        h->explicit_ad = (int)value;
         return 0;
     case SHASTA_PREDICTOR:
         if (value != 0.0 && value != 1.0) return fail(h, SHASTA_EINVAL, "SHASTA_PREDICTOR must be 0 (R1) or 1 (R2)");

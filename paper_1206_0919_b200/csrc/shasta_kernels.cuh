@@ -88,6 +88,8 @@ struct Consts {
     T hlam;     // lambda/2 (predictor; corrector source factor)
     T qlam;     // lambda/4 (predictor source factor 1/2 * lambda/2)
     T aq;       // diff / 8: outer factor of eq. (19) times the paper's `diff`; 1/8 by default
+    T ad2;      // factor of the second difference of Delta inside eq. (19): -1/8 = phoenical (default), 0 = explicit
+                // antidiffusion A = diff/8 D^ (footnote 1); f2
     EosD d;
 };
 
@@ -916,10 +918,12 @@ struct Consumer {
     T dh[2][NF];        // D^_4, D^_5                                         slot (PH-k)&1
     T a5[NF];           // A_5
     T aq;               // diff / 8
+    T ad2;              // -1/8 (phoenical) | 0 (explicit antidiffusion)
 
-    __device__ __forceinline__ void init(T aq_)
+    __device__ __forceinline__ void init(T aq_, T ad2_)
     {
         aq = aq_;
+        ad2 = ad2_;
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
             dl[0][f] = dl[1][f] = dl[2][f] = dl[3][f] = fc[f] = T(0);
@@ -946,7 +950,7 @@ struct Consumer {
             fc[f] = fl;
             const T dh3 = uh2 - uh[H3][f];                                       // eq. (18)
             const T d2 = t_fma(T(-2), dl[D4][f], dl[D3][f] + dl[D5][f]);         // reading G14
-            const T aph = aq * t_fma(T(-0.125), d2, dh[E4][f]);                  // eq. (19) (x diff: exact scaling, same bits as the oracle)
+            const T aph = aq * t_fma(ad2, d2, dh[E4][f]);                        // eq. (19) (x diff: exact scaling, same bits as the oracle)
             const T a4 = limiter<T>(aph, dh3, dh[E5][f]);                        // eqs. (20),(21)
             un[f] = uh[H4][f] - (a4 - a5[f]);                                    // eq. (22)
             a5[f] = a4;
@@ -1231,7 +1235,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
         Cnt cnt;
         cnt.zero();
         Consumer<T> co;
-        co.init(k.aq);
+        co.init(k.aq, k.ad2);
         HalfStep<T, EOS> hs;
         hs.init();
         // element offset of the output cell of the NEXT step: cell ilo - 4 (the first two groups store nothing)
@@ -1569,7 +1573,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
         Cnt cnt;
         cnt.zero();
         Consumer<T> co;
-        co.init(k.aq);
+        co.init(k.aq, k.ad2);
         HalfStep<T, EOS> hs;
         hs.init();
         int q0 = 0;                     // ring tile of group g
@@ -1725,11 +1729,11 @@ __device__ __forceinline__ double cell_transport(double um, double u0, double up
 }
 // eqs. (18)-(21): limited antidiffusive flux at interface (i, i+1); uh at i-1..i+2, u at i-1..i+2
 __device__ __forceinline__ double cell_antiflux(double hm, double h0, double h1, double h2, double um, double u0, double u1,
-                                                double u2, double diff)
+                                                double u2, double diff, double ad2)
 {
     const double Dh = h1 - h0, Dhp = h2 - h1, Dhm = h0 - hm;     // eq. (18)
     const double Di = u1 - u0, Dip = u2 - u1, Dim = u0 - um;
-    const double aph = diff * (0.125 * (Dh - 0.125 * ((Dip + Dim) - 2.0 * Di)));     // eq. (19), G14
+    const double aph = diff * (0.125 * fma(ad2, (Dip + Dim) - 2.0 * Di, Dh));        // eq. (19), G14; ad2 = -1/8 | 0
     const double sg = (aph > 0.0) - (aph < 0.0);                 // eq. (20)
     double m = fmin(fmin(sg * Dhp, fabs(aph)), sg * Dhm);
     return sg * fmax(m, 0.0);                                    // eq. (21)
@@ -1794,9 +1798,9 @@ __global__ void __launch_bounds__(128) sweep_cell_kernel(const __grid_constant__
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 const double a1 = cell_antiflux(up[f][q - 1], up[f][q], up[f][q + 1], up[f][q + 2], w.u[f][c - 1], w.u[f][c],
-                                                w.u[f][c + 1], w.u[f][c + 2], diff);
+                                                w.u[f][c + 1], w.u[f][c + 2], diff, k.ad2);
                 const double a0 = cell_antiflux(up[f][q - 2], up[f][q - 1], up[f][q], up[f][q + 1], w.u[f][c - 2], w.u[f][c - 1],
-                                                w.u[f][c], w.u[f][c + 1], diff);
+                                                w.u[f][c], w.u[f][c + 1], diff, k.ad2);
                 ut[f][m + 3] = up[f][q] - a1 + a0;                          // eq. (22)
             }
         }
@@ -1821,8 +1825,8 @@ __global__ void __launch_bounds__(128) sweep_cell_kernel(const __grid_constant__
             uh[m + 2] = cell_transport(w.u[f][c - 1], w.u[f][c], w.u[f][c + 1], lam * vh[q - 1], lam * vh[q], lam * vh[q + 1],
                                        lam, fm, fp);
         }
-        const double a1 = cell_antiflux(uh[1], uh[2], uh[3], uh[4], w.u[f][W - 1], w.u[f][W], w.u[f][W + 1], w.u[f][W + 2], diff);
-        const double a0 = cell_antiflux(uh[0], uh[1], uh[2], uh[3], w.u[f][W - 2], w.u[f][W - 1], w.u[f][W], w.u[f][W + 1], diff);
+        const double a1 = cell_antiflux(uh[1], uh[2], uh[3], uh[4], w.u[f][W - 1], w.u[f][W], w.u[f][W + 1], w.u[f][W + 2], diff, k.ad2);
+        const double a0 = cell_antiflux(uh[0], uh[1], uh[2], uh[3], w.u[f][W - 2], w.u[f][W - 1], w.u[f][W], w.u[f][W + 1], diff, k.ad2);
         un[f] = uh[2] - a1 + a0;                                            // eq. (22)
     }
     // 8. Pi written back (G8), primitives in the last sweep of a step

@@ -12,8 +12,9 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libshasta.so")
 
-BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH, NO_DEFER, PRIMS_RAW, BATCH, GRAPH = range(14)
+BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH, NO_DEFER, PRIMS_RAW, BATCH, GRAPH, ANTIDIFFUSION = range(15)
 R1, R2 = 0, 1
+PHOENICAL, EXPLICIT = 0, 1
 OUTFLOW, PERIODIC = 0, 1
 BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 
@@ -123,7 +124,8 @@ class Shasta:
     """One solver handle = shasta_create ... shasta_destroy.  Method names follow the C ABI."""
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, precision=64,
-                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0, batch=1, graph=None, eos_table=None):
+                 segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0, batch=1, graph=None, eos_table=None,
+                 antidiffusion=PHOENICAL):
         L = load()
         self._L = L
         self._h = _vp()
@@ -156,6 +158,8 @@ class Shasta:
             self.set_option(GRAPH, graph)
         if eos_table is not None:
             self.set_eos_table(*eos_table)
+        if antidiffusion:
+            self.set_option(ANTIDIFFUSION, antidiffusion)
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:

@@ -77,9 +77,10 @@ def record(name, rep, **meta):
     _RECORD[name] = dict(meta, fields=rep)
 
 
-def run_oracle(oracle, c, steps=None, table=None, variant="strict", predictor=0, diff=1.0, eos_table=None):
+def run_oracle(oracle, c, steps=None, table=None, variant="strict", predictor=0, diff=1.0, eos_table=None,
+               antidiffusion=0):
     o = oracle.Oracle(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"],
-                      variant=variant, predictor=predictor, diff=diff, eos_table=eos_table)
+                      variant=variant, predictor=predictor, diff=diff, eos_table=eos_table, antidiffusion=antidiffusion)
     if table is not None:
         o.set_sweep_table(table)
     o.set_state(c["e"], c["n"], c["vx"], c["vy"], c["vz"])
@@ -90,12 +91,12 @@ def run_oracle(oracle, c, steps=None, table=None, variant="strict", predictor=0,
 
 
 def run_gpu(c, steps=None, table=None, precision=64, segment=0, host_io=False, no_tma=0, predictor=0, diff=1.0,
-            cell_path=0, eos_table=None):
+            cell_path=0, eos_table=None, antidiffusion=0, batch=1, graph=None):
     import torch
     from paper_1206_0919_b200.shasta import Shasta
     s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"],
                precision=precision, segment=segment, no_tma=no_tma, predictor=predictor, diff=diff, cell_path=cell_path,
-               eos_table=eos_table)
+               eos_table=eos_table, antidiffusion=antidiffusion, batch=batch, graph=graph)
     if table is not None:
         s.set_sweep_table(table)
     if host_io:

@@ -504,6 +504,59 @@ def test_variant_general_eos_per_cell(oracle):
     assert_kernel_parity(got, ref, "general EOS R2", tol_cons=1e-11, tol_prim=1e-11)
 
 
+# explicit antidiffusion (PAPER.md:123 footnote 1; oracle pin: test_explicit_antidiffusion_leaves_the_fourth_difference_at_rest)
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("diff", [1.0, 0.5])
+def test_variant_explicit_antidiffusion_fused_kernels(oracle, bc, diff):
+    c = inputs.random_state(37, 19, 23, seed=41 + bc, kind="rough", boundary=bc)     # ragged: cp.async tiles
+    ref, _ = parity.run_oracle(oracle, c, steps=2, diff=diff, antidiffusion=1)
+    got, s = parity.run_gpu(c, steps=2, diff=diff, antidiffusion=1)
+    assert s.kernel_name(0).startswith("sweep_x2_kernel")
+    assert_kernel_parity(got, ref, f"explicit antidiffusion diff {diff} bc {bc}")
+    # the variant is a different scheme, not a no-op: the default result is far from it at this tolerance
+    dflt, _ = parity.run_gpu(c, steps=2, diff=diff)
+    assert parity.field_errors(dflt, ref)["E"][0] > 1e-6
+    c = inputs.random_state(64, 33, 6, seed=42 + bc, kind="rough", boundary=bc)      # TMA-fed shapes
+    ref, _ = parity.run_oracle(oracle, c, steps=2, diff=diff, antidiffusion=1)
+    got, _ = parity.run_gpu(c, steps=2, diff=diff, antidiffusion=1)
+    assert_kernel_parity(got, ref, f"explicit antidiffusion diff {diff} bc {bc} (tma)")
+
+
+@pytest.mark.parametrize("predictor", [0, 1])
+def test_variant_explicit_antidiffusion_per_cell_kernels(oracle, predictor):
+    # with the R2 predictor the half step runs eqs. (18)-(22) too: the variant applies there as well
+    for bc in (inputs.OUTFLOW, inputs.PERIODIC):
+        c = inputs.random_state(37, 19, 23, seed=43 + bc, kind="rough", boundary=bc)
+        ref, _ = parity.run_oracle(oracle, c, steps=2, predictor=predictor, antidiffusion=1)
+        got, s = parity.run_gpu(c, steps=2, predictor=predictor, antidiffusion=1, cell_path=1)
+        assert s.kernel_name(0) == "sweep_cell_kernel"
+        assert_kernel_parity(got, ref, f"explicit antidiffusion per-cell predictor {predictor} bc {bc}")
+
+
+def test_variant_explicit_antidiffusion_general_eos_batch_and_graph(oracle):
+    # general-EOS kernels (S3 in the consumer), two events per launch, graph replay of whole table cycles
+    cs = [inputs.random_state(24, 20, 28, seed=44 + b, kind="rough", gamma=5.0 / 3.0, mass=1.0, boundary=inputs.PERIODIC)
+          for b in range(2)]
+    refs = [parity.run_oracle(oracle, c, steps=6, antidiffusion=1)[0] for c in cs]
+    c2 = dict(cs[0])
+    for k in ("e", "n", "vx", "vy", "vz"):
+        c2[k] = np.stack([c[k] for c in cs])
+    got, s = parity.run_gpu(c2, steps=6, antidiffusion=1, batch=2, graph=1)
+    assert s.graph_launch_count >= 1
+    for b in range(2):
+        assert_kernel_parity({k: v[b] for k, v in got.items()}, refs[b], f"explicit antidiffusion general EOS event {b}",
+                             tol_cons=1e-11, tol_prim=1e-11)
+
+
+def test_variant_explicit_antidiffusion_config1(oracle):
+    c = inputs.shock_tube(400, 0.01)
+    ref, _ = parity.run_oracle(oracle, c, antidiffusion=1)
+    got, _ = parity.run_gpu(c, antidiffusion=1)
+    rep = parity.field_report(got, ref)
+    parity.record("config1 eR=0.01 variant antidiffusion=explicit", rep, steps=c["steps"])
+    parity.assert_parity(got, ref, TOL64, label="config1 explicit antidiffusion")
+
+
 # ------------------------------------------------------------------ T2: the configs
 # Bars (north_star): fp64 err_max <= 1e-10 per field, err_L1 reported (expected <= 1e-12).  Configs 3 and 4
 # amplify rounding noise: two equally valid fp64 evaluations of the ORACLE (strict vs FMA-contracted build) already
