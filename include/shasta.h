@@ -76,6 +76,11 @@ typedef struct shasta shasta_t;   /* opaque */
                                  only): the variant of PAPER.md:123, footnote 1.  Same kernels: the
                                  coefficient of the second difference is a kernel constant (-1/8 or 0)                 */
 
+#define SHASTA_BOUNDARY_Z 15   /* boundary rule of the z sweeps only: -1 (default) = as SHASTA_BOUNDARY; 0 = outflow, 1 = periodic.
+                                 For a rank of a z-slab decomposition: its grid carries 4 halo
+                                 planes per neighbour, refreshed with shasta_set_planes before each z sweep, and its z
+                                 sweeps run with 0 whatever the global rule is                                           */
+
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only
  * (eqs. (15)-(17)); dx enters shasta_conserved_totals.  0 < lambda <= 0.5
@@ -122,6 +127,19 @@ int shasta_set_conserved(shasta_t* h, const double* E_dev, const double* Mx_dev,
                          const double* Mz_dev, const double* R_dev, void* stream);
 int shasta_get_conserved(shasta_t* h, double* E_dev, double* Mx_dev, double* My_dev, double* Mz_dev,
                          double* R_dev, void* stream);
+
+/*
+ * Planes z0 .. z0+nplanes-1 (z is the slowest axis: one contiguous block of nplanes*nx*ny values per field) of the CURRENT
+ * conserved state, copied to / from DEVICE arrays of nplanes*nx*ny doubles in field order E, Mx, My, Mz, R (NULL = skip
+ * the field).  Asynchronous on `stream`; fp32 storage converts.  For the halo exchange of a z-slab decomposition
+ * (SURVEY.md 8(e)): a rank sends the 4 planes next to each interface and writes what it receives into its halo planes
+ * before every z sweep (paper_1206_0919_b200/zslab.py).  set_planes invalidates the primitive fields.  SHASTA_ESTATE
+ * before the first set_state or with SHASTA_BATCH > 1, SHASTA_EINVAL for planes outside [0, nz).
+ */
+int shasta_get_planes(shasta_t* h, int z0, int nplanes, double* E_dev, double* Mx_dev, double* My_dev, double* Mz_dev,
+                      double* R_dev, void* stream);
+int shasta_set_planes(shasta_t* h, int z0, int nplanes, const double* E_dev, const double* Mx_dev, const double* My_dev,
+                      const double* Mz_dev, const double* R_dev, void* stream);
 
 /*
  * Advance nsteps time steps dt = lambda*dx.  One step = three fused sweep kernels, one per axis in

@@ -38,6 +38,7 @@ struct shasta {
     int cell_path;          // 1 = run the per-cell kernels also for the default scheme (A/B datapoint, tests)
     int predictor;          // 0 = R1 (eq. (17) alone), 1 = R2 (complete kernel at lambda/2): per-cell kernels
     int periodic;
+    int periodic_z;         // SHASTA_BOUNDARY_Z: -1 = as `periodic`; 0 | 1 = rule of the z sweeps only (z-slab ranks: 0)
     int precision;          // 64 | 32
     int seg_override;
     int no_tma;             // test hook: 1 = x sweep through cp.async even where TMA is possible
@@ -90,6 +91,7 @@ int fail(shasta_t* h, int code, const char* fmt, ...)
     } while (0)
 
 size_t esize(const shasta_t* h) { return h->precision == 64 ? 8 : 4; }
+int axis_periodic(const shasta_t* h, int axis) { return (axis == 2 && h->periodic_z >= 0) ? h->periodic_z : h->periodic; }
 
 int make_tensor_maps(shasta_t* h);
 int make_yz_maps(shasta_t* h);
@@ -426,7 +428,7 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
     P.nx = h->nx;
     P.N = n[axis];
     P.stride_axis = stride[axis];
-    P.periodic = h->periodic;
+    P.periodic = axis_periodic(h, axis);
     P.axis = axis;
     P.odiv = 0x7fffffff;
     P.counts = h->d_counts;
@@ -516,7 +518,7 @@ int launch_cell_sweep(shasta_t* h, int axis, bool emit, cudaStream_t st)
     }
     P.in[4] = h->U[src][4]; P.out[4] = h->U[dst][4];
     P.prim[0] = h->prim[0]; P.prim[1] = h->prim[1]; P.prim[2] = h->prim[2];
-    P.nx = h->nx; P.N = n[axis]; P.stride_axis = stride[axis]; P.periodic = h->periodic; P.axis = axis;
+    P.nx = h->nx; P.N = n[axis]; P.stride_axis = stride[axis]; P.periodic = axis_periodic(h, axis); P.axis = axis;
     P.counts = h->d_counts;
     const Consts<double> k = make_consts<double>(h);
     const unsigned blocks = (unsigned)((h->ncell + 127) / 128);
@@ -724,6 +726,7 @@ int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lamb
     h->dx = dx; h->lambda = lambda; h->gamma = eos_gamma; h->mass = 0.0;
     h->precision = 64;
     h->diff = 1.0;
+    h->periodic_z = -1;
     h->graph_mode = 2;
     memcpy(h->table, kBranch, sizeof(kBranch));
     h->ntable = 18;
@@ -806,6 +809,11 @@ int shasta_set_option(shasta_t* h, int key, double value)
         return 0;
     case SHASTA_CELL_PATH:
         h->cell_path = value != 0.0;
+        return 0;
+    case SHASTA_BOUNDARY_Z:
+        if (value != -1.0 && value != 0.0 && value != 1.0)
+            return fail(h, SHASTA_EINVAL, "SHASTA_BOUNDARY_Z must be -1 (as SHASTA_BOUNDARY), 0 or 1");
+        h->periodic_z = (int)value;
         return 0;
     case SHASTA_ANTIDIFFUSION:
         if (value != 0.0 && value != 1.0)
@@ -933,6 +941,67 @@ int shasta_get_conserved(shasta_t* h, double* E, double* Mx, double* My, double*
             int rc = export_field(h, h->U[h->cur][f], dst[f], (cudaStream_t)stream);
             if (rc) return rc;
         }
+    return 0;
+}
+
+// planes z0 .. z0+nplanes-1 of the current conserved state (z is the slowest axis: one contiguous block per field)
+static int plane_range(shasta_t* h, const char* who, int z0, int nplanes, size_t* off, long long* cnt)
+{
+    if (!h->have_state) return fail(h, SHASTA_ESTATE, "%s: no state set", who);
+    if (h->nbatch != 1) return fail(h, SHASTA_ESTATE, "%s: not with SHASTA_BATCH > 1", who);
+    if (z0 < 0 || nplanes < 0 || (long long)z0 + nplanes > h->nz)
+        return fail(h, SHASTA_EINVAL, "%s: planes [%d, %d) outside [0, %d)", who, z0, z0 + nplanes, h->nz);
+    int rc = check_device(h);
+    if (rc) return rc;
+    *off = (size_t)z0 * (size_t)h->nx * (size_t)h->ny;
+    *cnt = (long long)nplanes * h->nx * h->ny;
+    return 0;
+}
+
+int shasta_get_planes(shasta_t* h, int z0, int nplanes, double* E, double* Mx, double* My, double* Mz, double* R,
+                      void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    size_t off; long long cnt;
+    int rc = plane_range(h, "shasta_get_planes", z0, nplanes, &off, &cnt);
+    if (rc || cnt == 0) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* dst[NF] = {E, Mx, My, Mz, R};
+    for (int f = 0; f < NF; ++f) {
+        if (!dst[f]) continue;
+        if (h->precision == 64) {
+            CK(cudaMemcpyAsync(dst[f], (const double*)h->U[h->cur][f] + off, sizeof(double) * (size_t)cnt,
+                               cudaMemcpyDeviceToDevice, st));
+        } else {
+            convert_kernel<float, double><<<ew_grid(h, 256), 256, 0, st>>>(cnt, (const float*)h->U[h->cur][f] + off, dst[f]);
+            CK(cudaGetLastError());
+            h->launches++;
+        }
+    }
+    return 0;
+}
+
+int shasta_set_planes(shasta_t* h, int z0, int nplanes, const double* E, const double* Mx, const double* My,
+                      const double* Mz, const double* R, void* stream)
+{
+    if (!h) return SHASTA_EINVAL;
+    size_t off; long long cnt;
+    int rc = plane_range(h, "shasta_set_planes", z0, nplanes, &off, &cnt);
+    if (rc || cnt == 0) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const double* src[NF] = {E, Mx, My, Mz, R};
+    for (int f = 0; f < NF; ++f) {
+        if (!src[f]) continue;
+        if (h->precision == 64) {
+            CK(cudaMemcpyAsync((double*)h->U[h->cur][f] + off, src[f], sizeof(double) * (size_t)cnt,
+                               cudaMemcpyDeviceToDevice, st));
+        } else {
+            convert_kernel<double, float><<<ew_grid(h, 256), 256, 0, st>>>(cnt, src[f], (float*)h->U[h->cur][f] + off);
+            CK(cudaGetLastError());
+            h->launches++;
+        }
+    }
+    h->prims_valid = false;
     return 0;
 }
 

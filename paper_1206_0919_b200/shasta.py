@@ -12,7 +12,7 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libshasta.so")
 
-BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH, NO_DEFER, PRIMS_RAW, BATCH, GRAPH, ANTIDIFFUSION = range(15)
+BOUNDARY, EOS_MASS, PRECISION, STEP_INDEX, SEGMENT, VARIANT, NO_TMA, PREDICTOR, DIFF, CELL_PATH, NO_DEFER, PRIMS_RAW, BATCH, GRAPH, ANTIDIFFUSION, BOUNDARY_Z = range(16)
 R1, R2 = 0, 1
 PHOENICAL, EXPLICIT = 0, 1
 OUTFLOW, PERIODIC = 0, 1
@@ -21,7 +21,7 @@ BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 # every symbol include/shasta.h declares
 SYMBOLS = (
     "shasta_create", "shasta_destroy", "shasta_set_option", "shasta_set_eos_table", "shasta_set_sweep_table", "shasta_set_state",
-    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_step", "shasta_sweep",
+    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_get_planes", "shasta_set_planes", "shasta_step", "shasta_sweep",
     "shasta_get_primitives", "shasta_get_primitives_host", "shasta_conserved_totals", "shasta_diagnostics",
     "shasta_launch_count", "shasta_graph_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
     "shasta_conserved_totals_static", "shasta_conserved_totals_static_max_cells",
@@ -51,6 +51,8 @@ def load():
     L.shasta_set_state_host.argtypes = [_vp] + [_dp] * 5 + [_vp]
     L.shasta_set_conserved.argtypes = [_vp] + [_dp] * 5 + [_vp]
     L.shasta_get_conserved.argtypes = [_vp] + [_dp] * 5 + [_vp]
+    L.shasta_get_planes.argtypes = [_vp, C.c_int, C.c_int] + [_dp] * 5 + [_vp]
+    L.shasta_set_planes.argtypes = [_vp, C.c_int, C.c_int] + [_dp] * 5 + [_vp]
     L.shasta_step.argtypes = [_vp, C.c_int, _vp]
     L.shasta_sweep.argtypes = [_vp, C.c_int, C.c_int, _vp]
     L.shasta_get_primitives.argtypes = [_vp] + [_dp] * 6 + [_vp]
@@ -125,7 +127,7 @@ class Shasta:
 
     def __init__(self, nx, ny, nz, dx, lam, eos_gamma, boundary=OUTFLOW, eos_mass=0.0, precision=64,
                  segment=0, no_tma=0, predictor=0, diff=1.0, cell_path=0, no_defer=0, batch=1, graph=None, eos_table=None,
-                 antidiffusion=PHOENICAL):
+                 antidiffusion=PHOENICAL, boundary_z=None):
         L = load()
         self._L = L
         self._h = _vp()
@@ -160,6 +162,8 @@ class Shasta:
             self.set_eos_table(*eos_table)
         if antidiffusion:
             self.set_option(ANTIDIFFUSION, antidiffusion)
+        if boundary_z is not None:
+            self.set_option(BOUNDARY_Z, boundary_z)
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
@@ -215,6 +219,20 @@ class Shasta:
         self._chk(self._L.shasta_get_conserved(self._h, *[_dev(t) for t in out], _stream_ptr(stream)),
                   "shasta_get_conserved")
         return dict(zip(("E", "Mx", "My", "Mz", "R"), out))
+
+    def get_planes(self, z0, nplanes, out=None, stream=None):
+        """planes z0 .. z0+nplanes-1 of the conserved state as a (5, nplanes, ny, nx) CUDA tensor (fields E, Mx, My, Mz, R)"""
+        import torch
+        if out is None:
+            out = torch.empty((5, int(nplanes), self.ny, self.nx), dtype=torch.float64, device="cuda")
+        self._chk(self._L.shasta_get_planes(self._h, int(z0), int(nplanes), *[_dev(out[f]) for f in range(5)],
+                                            _stream_ptr(stream)), "shasta_get_planes")
+        return out
+
+    def set_planes(self, z0, planes, stream=None):
+        """planes: (5, nplanes, ny, nx) CUDA tensor written over planes z0 .. z0+nplanes-1 of the conserved state"""
+        self._chk(self._L.shasta_set_planes(self._h, int(z0), int(planes.shape[1]), *[_dev(planes[f]) for f in range(5)],
+                                            _stream_ptr(stream)), "shasta_set_planes")
 
     def get_primitives(self, stream=None, out=None):
         import torch

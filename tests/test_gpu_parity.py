@@ -557,6 +557,57 @@ def test_variant_explicit_antidiffusion_config1(oracle):
     parity.assert_parity(got, ref, TOL64, label="config1 explicit antidiffusion")
 
 
+# ------------------------------------------------------------------ z-slab decomposition (host logic: test_zslab.py)
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("world", [2, 3])
+def test_zslab_in_process_equals_the_single_domain_run(oracle, bc, world):
+    # the slabs of one event as `world` handles on this GPU, planes carried by shasta_get_planes / shasta_set_planes:
+    # same kernels, same neighbourhood for every owned cell -> the same bits as one handle over the whole grid
+    import torch
+    from paper_1206_0919_b200 import zslab
+    c = inputs.random_state(40, 24, 29, seed=51 + bc, kind="rough", boundary=bc)
+    one, s1 = parity.run_gpu(c, steps=6)
+    slabs = [zslab.make_gpu_slab(c, world, r) for r in range(world)]
+    assert [sl.s.nz for sl in slabs] == [sl.lay.nz_local for sl in slabs]
+    zslab.step_in_process(slabs, 6)
+    U = torch.cat([sl.owned_conserved() for sl in slabs], dim=1).cpu().numpy()
+    for f, k in enumerate(parity.CONS):
+        assert np.array_equal(U[f], one[k]), k
+    prims = [sl.s.get_primitives() for sl in slabs]
+    for k in parity.PRIM:
+        assert np.array_equal(torch.cat([sl.owned(p[k]) for sl, p in zip(slabs, prims)], dim=0).cpu().numpy(), one[k]), k
+    ref, _ = parity.run_oracle(oracle, c, steps=6)
+    assert_kernel_parity(dict(zip(parity.CONS, U), **{k: one[k] for k in parity.PRIM}), ref, f"zslab world {world} bc {bc}")
+    # totals: every slab sums its owned planes (no process group here: no all-reduce), the sum is the event's
+    tot = sum(zslab.conserved_totals_distributed(sl, c["dx"]).cpu().numpy() for sl in slabs)
+    t1 = np.array(s1.conserved_totals())
+    assert np.max(np.abs(tot - t1)) <= 1e-12 * abs(t1[0])
+
+
+def test_planes_round_trip_and_errors():
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta, ShastaError
+    c = inputs.random_state(12, 10, 9, seed=5, kind="rough")
+    for precision in (64, 32):
+        s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], precision=precision)
+        with pytest.raises(ShastaError):
+            s.get_planes(0, 1)                                   # no state yet
+        s.set_state(*[torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")])
+        U = torch.stack(list(s.get_conserved().values()))
+        assert torch.equal(s.get_planes(2, 4), U[:, 2:6])
+        s.set_planes(5, U[:, 0:3].contiguous())
+        V = torch.stack(list(s.get_conserved().values()))
+        assert torch.equal(V[:, 5:8], U[:, 0:3]) and torch.equal(V[:, :5], U[:, :5]) and torch.equal(V[:, 8:], U[:, 8:])
+        for z0, n in ((-1, 2), (7, 3), (0, 10)):
+            with pytest.raises(ShastaError):
+                s.get_planes(z0, n)
+        assert s.get_planes(9, 0).shape[1] == 0
+    b = Shasta(8, 8, 8, 0.1, 0.4, 4.0 / 3.0, batch=2)
+    b.set_state(*[torch.full((2, 8, 8, 8), v, dtype=torch.float64, device="cuda") for v in (1.0, 1.0, 0.0, 0.0, 0.0)])
+    with pytest.raises(ShastaError):
+        b.get_planes(0, 1)
+
+
 # ------------------------------------------------------------------ T2: the configs
 # Bars (north_star): fp64 err_max <= 1e-10 per field, err_L1 reported (expected <= 1e-12).  Configs 3 and 4
 # amplify rounding noise: two equally valid fp64 evaluations of the ORACLE (strict vs FMA-contracted build) already
