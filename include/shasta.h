@@ -140,6 +140,14 @@ int shasta_get_planes(shasta_t* h, int z0, int nplanes, double* E_dev, double* M
                       double* R_dev, void* stream);
 int shasta_set_planes(shasta_t* h, int z0, int nplanes, const double* E_dev, const double* Mx_dev, const double* My_dev,
                       const double* Mz_dev, const double* R_dev, void* stream);
+/* Zero-copy form of the two calls above: the DEVICE address of plane z0 (0 <= z0 <= nz) of conserved field `field`
+ * (0..4 = E, Mx, My, Mz, R) inside the handle's CURRENT state buffer, so that a halo exchange can send from and receive
+ * into the planes themselves (ncclSend/ncclRecv, peer copies).  Elements are the storage type (double, or float with
+ * SHASTA_PRECISION 32), planes z0.. follow contiguously up to plane nz.  The handle keeps ownership.  The address is
+ * valid only until the next shasta_sweep / shasta_step / shasta_set_* call on the handle (the state buffers ping-pong):
+ * ask again before every exchange, and order the writes before the next sweep on its stream.  After writing owned
+ * planes through it, primitive fields written earlier are stale (halo planes: nobody reads theirs). */
+int shasta_plane_ptr(shasta_t* h, int field, int z0, void** ptr_dev);
 
 /*
  * Advance nsteps time steps dt = lambda*dx.  One step = three fused sweep kernels, one per axis in

@@ -1005,6 +1005,18 @@ int shasta_set_planes(shasta_t* h, int z0, int nplanes, const double* E, const d
     return 0;
 }
 
+int shasta_plane_ptr(shasta_t* h, int field, int z0, void** ptr_dev)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (!ptr_dev) return fail(h, SHASTA_EINVAL, "shasta_plane_ptr: NULL output");
+    if (field < 0 || field >= NF) return fail(h, SHASTA_EINVAL, "shasta_plane_ptr: field %d outside [0, 5)", field);
+    size_t off; long long cnt;
+    int rc = plane_range(h, "shasta_plane_ptr", z0, 0, &off, &cnt);
+    if (rc) return rc;
+    *ptr_dev = (char*)h->U[h->cur][field] + off * esize(h);
+    return 0;
+}
+
 int shasta_step(shasta_t* h, int nsteps, void* stream)
 {
     if (!h) return SHASTA_EINVAL;

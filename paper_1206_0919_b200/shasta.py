@@ -21,7 +21,7 @@ BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 # every symbol include/shasta.h declares
 SYMBOLS = (
     "shasta_create", "shasta_destroy", "shasta_set_option", "shasta_set_eos_table", "shasta_set_sweep_table", "shasta_set_state",
-    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_get_planes", "shasta_set_planes", "shasta_step", "shasta_sweep",
+    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_get_planes", "shasta_set_planes", "shasta_plane_ptr", "shasta_step", "shasta_sweep",
     "shasta_get_primitives", "shasta_get_primitives_host", "shasta_conserved_totals", "shasta_diagnostics",
     "shasta_launch_count", "shasta_graph_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
     "shasta_conserved_totals_static", "shasta_conserved_totals_static_max_cells",
@@ -53,6 +53,7 @@ def load():
     L.shasta_get_conserved.argtypes = [_vp] + [_dp] * 5 + [_vp]
     L.shasta_get_planes.argtypes = [_vp, C.c_int, C.c_int] + [_dp] * 5 + [_vp]
     L.shasta_set_planes.argtypes = [_vp, C.c_int, C.c_int] + [_dp] * 5 + [_vp]
+    L.shasta_plane_ptr.argtypes = [_vp, C.c_int, C.c_int, C.POINTER(_vp)]
     L.shasta_step.argtypes = [_vp, C.c_int, _vp]
     L.shasta_sweep.argtypes = [_vp, C.c_int, C.c_int, _vp]
     L.shasta_get_primitives.argtypes = [_vp] + [_dp] * 6 + [_vp]
@@ -122,6 +123,14 @@ def conserved_totals_static(E, Mx, My, Mz, R, dv, out, stream=None):
     return out
 
 
+class _DeviceMemory:
+    """memory owned by a handle, seen through __cuda_array_interface__ (torch.as_tensor makes a view, not a copy)"""
+
+    def __init__(self, ptr, shape, typestr):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (int(ptr), False),
+                                         "version": 2, "strides": None}
+
+
 class Shasta:
     """One solver handle = shasta_create ... shasta_destroy.  Method names follow the C ABI."""
 
@@ -142,6 +151,8 @@ class Shasta:
         self.set_option(BOUNDARY, boundary)
         self.set_option(EOS_MASS, eos_mass)
         self.set_option(PRECISION, precision)
+        self._typestr = "<f8" if int(precision) == 64 else "<f4"
+        self._views = {}
         if segment:
             self.set_option(SEGMENT, segment)
         if no_tma:
@@ -167,6 +178,7 @@ class Shasta:
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
+            self._views = {}
             self._L.shasta_destroy(self._h)
             self._h = _vp()
 
@@ -233,6 +245,24 @@ class Shasta:
         """planes: (5, nplanes, ny, nx) CUDA tensor written over planes z0 .. z0+nplanes-1 of the conserved state"""
         self._chk(self._L.shasta_set_planes(self._h, int(z0), int(planes.shape[1]), *[_dev(planes[f]) for f in range(5)],
                                             _stream_ptr(stream)), "shasta_set_planes")
+
+    def plane_views(self, z0, nplanes):
+        """shasta_plane_ptr: the planes z0 .. z0+nplanes-1 of the five conserved fields as five CUDA tensors (nplanes, ny, nx)
+        that ALIAS the handle's current state buffer (storage dtype); valid until the next sweep / step / set_* call."""
+        import torch
+        if not (0 <= z0 and nplanes >= 1 and z0 + nplanes <= self.nz):
+            raise ValueError("planes outside the grid")
+        out = []
+        for f in range(5):
+            p = _vp()
+            self._chk(self._L.shasta_plane_ptr(self._h, f, int(z0), C.byref(p)), "shasta_plane_ptr")
+            key = (p.value, int(nplanes))                # the two state buffers live as long as the handle: wrap each once
+            t = self._views.get(key)
+            if t is None:
+                t = torch.as_tensor(_DeviceMemory(p.value, (int(nplanes), self.ny, self.nx), self._typestr), device="cuda")
+                self._views[key] = t
+            out.append(t)
+        return out
 
     def get_primitives(self, stream=None, out=None):
         import torch

@@ -4,13 +4,13 @@ The step has exactly one exchange: a sweep reads 4 ghost cells per side (DESIGN.
 slabs.  Rank r owns nz_r consecutive planes; its solver's grid carries G = 4 halo planes per neighbour and runs its z
 sweeps with the outflow rule (SHASTA_BOUNDARY_Z 0): the copy-edge ghosts then only feed the outer 4 planes, which are
 halo and get overwritten.  Before EVERY z sweep each rank sends the 4 owned planes next to each interface and writes
-what it receives into its halo planes (shasta_get_planes / shasta_set_planes + NCCL send/recv); x and y sweeps need
-nothing.  A face without a neighbour (first/last rank of an outflow run) has no halo: the solver's own ghost rule is
+what it receives into its halo planes (NCCL send/recv straight from and into the planes of the handle's state buffer,
+shasta_plane_ptr; or staged through shasta_get_planes / shasta_set_planes); x and y sweeps need nothing.  A face without a neighbour (first/last rank of an outflow run) has no halo: the solver's own ghost rule is
 the physical boundary there.  A periodic run wraps rank 0 <-> world-1.  Every owned cell therefore sees the same
 9-point neighbourhood as in the single-domain run and is updated by the same kernel: the results are identical.
 
 Orchestration and message passing only: every arithmetic step stays in the kernels behind the C ABI.  The solver is
-any object with the binding's sweep / get_planes / set_planes (paper_1206_0919_b200.shasta.Shasta); the two drivers
+any object with the binding's sweep / get_planes / set_planes [/ plane_views] (paper_1206_0919_b200.shasta.Shasta); the two drivers
 below differ only in who carries the planes: torch.distributed (one process per GPU: nccl; gloo on CPU tensors, used by
 tests/test_zslab.py with world_size 2) or plain copies between slabs living in one process (one GPU, tests).
 Not overlapped with the interior yet (the exchange is 4 planes x 5 fields per face, 10.5 MB at 256^3).
@@ -76,18 +76,38 @@ class ZSlab:
         self.s, self.lay, self.table = solver, lay, tuple(table)
         self.step_index = 0
 
-    # the owned planes next to each interface, as the neighbour's halo
-    def planes_for_lo(self):
-        return self.s.get_planes(self.lay.lo, G) if self.lay.lo_nb is not None else None
+    # A message is a LIST of tensors.  With a solver that offers plane_views (shasta_plane_ptr) the five tensors alias
+    # the field planes themselves: sent from and received into place, no staging copies.  Otherwise (get_planes /
+    # set_planes only) it is one packed (5, G, ny, nx) tensor, received into a staging tensor and written by commit().
+    def _take(self, z0):
+        pv = getattr(self.s, "plane_views", None)
+        return pv(z0, G) if pv is not None else [self.s.get_planes(z0, G)]
 
-    def planes_for_hi(self):
-        return self.s.get_planes(self.lay.lo + self.lay.nz - G, G) if self.lay.hi_nb is not None else None
+    def outgoing(self):
+        """(to_lo, to_hi): the owned planes next to each interface (None: no neighbour there)"""
+        lay = self.lay
+        return (self._take(lay.lo) if lay.lo_nb is not None else None,
+                self._take(lay.lo + lay.nz - G) if lay.hi_nb is not None else None)
 
-    def put_halo(self, from_lo, from_hi):
+    def incoming(self, to_lo, to_hi):
+        """(from_lo, from_hi): where the neighbours' planes land: the halo planes themselves, or staging tensors shaped
+        like the outgoing messages"""
+        import torch
+        lay = self.lay
+        if hasattr(self.s, "plane_views"):
+            return (self.s.plane_views(0, G) if lay.lo_nb is not None else None,
+                    self.s.plane_views(lay.lo + lay.nz, G) if lay.hi_nb is not None else None)
+        return ([torch.empty_like(t) for t in to_lo] if to_lo is not None else None,
+                [torch.empty_like(t) for t in to_hi] if to_hi is not None else None)
+
+    def commit(self, from_lo, from_hi):
+        """staging tensors -> halo planes (nothing to do when the messages were received in place)"""
+        if hasattr(self.s, "plane_views"):
+            return
         if from_lo is not None:
-            self.s.set_planes(0, from_lo)
+            self.s.set_planes(0, from_lo[0])
         if from_hi is not None:
-            self.s.set_planes(self.lay.lo + self.lay.nz, from_hi)
+            self.s.set_planes(self.lay.lo + self.lay.nz, from_hi[0])
 
     def owned(self, t):
         """owned planes of a local field tensor (..., nz_local, ny, nx)"""
@@ -99,38 +119,43 @@ class ZSlab:
 
 # ---------------------------------------------------------------------------------------------- exchange
 def exchange_distributed(slab: ZSlab, group=None):
-    """Halo refresh between ranks.  Message "up" (tag 0): my top planes -> hi neighbour's lo halo; "down" (tag 1): my
-    bottom planes -> lo neighbour's hi halo.  Sends are posted up-then-down and receives lo-then-hi, so that with two
-    periodic ranks (both neighbours the same peer) the in-order matching of nccl pairs them right; gloo uses the tags."""
-    import torch
+    """Halo refresh between ranks.  Messages "up" (tags 0..): my top planes -> hi neighbour's lo halo; "down" (tags 8..):
+    my bottom planes -> lo neighbour's hi halo.  Sends are posted up-then-down and receives lo-then-hi, field by field, so
+    that with two periodic ranks (both neighbours the same peer) the in-order matching of nccl pairs them right; gloo
+    matches by tag.  One batch = one NCCL group: no ordering deadlock."""
     import torch.distributed as dist
     lay = slab.lay
     if lay.lo_nb is None and lay.hi_nb is None:
         return
-    to_lo, to_hi = slab.planes_for_lo(), slab.planes_for_hi()
-    from_lo = torch.empty_like(to_lo) if to_lo is not None else None
-    from_hi = torch.empty_like(to_hi) if to_hi is not None else None
+    to_lo, to_hi = slab.outgoing()
+    from_lo, from_hi = slab.incoming(to_lo, to_hi)
     ops = []
-    if to_hi is not None:
-        ops.append(dist.P2POp(dist.isend, to_hi, lay.hi_nb, group, 0))
-    if to_lo is not None:
-        ops.append(dist.P2POp(dist.isend, to_lo, lay.lo_nb, group, 1))
-    if from_lo is not None:
-        ops.append(dist.P2POp(dist.irecv, from_lo, lay.lo_nb, group, 0))
-    if from_hi is not None:
-        ops.append(dist.P2POp(dist.irecv, from_hi, lay.hi_nb, group, 1))
+    for i, t in enumerate(to_hi or ()):
+        ops.append(dist.P2POp(dist.isend, t, lay.hi_nb, group, i))
+    for i, t in enumerate(to_lo or ()):
+        ops.append(dist.P2POp(dist.isend, t, lay.lo_nb, group, 8 + i))
+    for i, t in enumerate(from_lo or ()):
+        ops.append(dist.P2POp(dist.irecv, t, lay.lo_nb, group, i))
+    for i, t in enumerate(from_hi or ()):
+        ops.append(dist.P2POp(dist.irecv, t, lay.hi_nb, group, 8 + i))
     for w in dist.batch_isend_irecv(ops):
         w.wait()
-    slab.put_halo(from_lo, from_hi)
+    slab.commit(from_lo, from_hi)
 
 
 def exchange_in_process(slabs):
-    """The same refresh for slabs that live in one process (rank order): pack everything, then unpack."""
-    msgs = [(sl.planes_for_lo(), sl.planes_for_hi()) for sl in slabs]
-    for sl in slabs:
+    """The same refresh for slabs that live in one process (rank order): device-to-device copies in stream order."""
+    msgs = [sl.outgoing() for sl in slabs]
+    for sl, (to_lo, to_hi) in zip(slabs, msgs):
         lay = sl.lay
-        sl.put_halo(msgs[lay.lo_nb][1] if lay.lo_nb is not None else None,
-                    msgs[lay.hi_nb][0] if lay.hi_nb is not None else None)
+        from_lo, from_hi = sl.incoming(to_lo, to_hi)
+        if from_lo is not None:
+            for d, src in zip(from_lo, msgs[lay.lo_nb][1]):
+                d.copy_(src)
+        if from_hi is not None:
+            for d, src in zip(from_hi, msgs[lay.hi_nb][0]):
+                d.copy_(src)
+        sl.commit(from_lo, from_hi)
 
 
 # ---------------------------------------------------------------------------------------------- time steps

@@ -559,8 +559,8 @@ def test_variant_explicit_antidiffusion_config1(oracle):
 
 # ------------------------------------------------------------------ z-slab decomposition (host logic: test_zslab.py)
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
-@pytest.mark.parametrize("world", [2, 3])
-def test_zslab_in_process_equals_the_single_domain_run(oracle, bc, world):
+@pytest.mark.parametrize("world,zero_copy", [(2, True), (3, True), (3, False)])
+def test_zslab_in_process_equals_the_single_domain_run(oracle, bc, world, zero_copy):
     # the slabs of one event as `world` handles on this GPU, planes carried by shasta_get_planes / shasta_set_planes:
     # same kernels, same neighbourhood for every owned cell -> the same bits as one handle over the whole grid
     import torch
@@ -569,6 +569,12 @@ def test_zslab_in_process_equals_the_single_domain_run(oracle, bc, world):
     one, s1 = parity.run_gpu(c, steps=6)
     slabs = [zslab.make_gpu_slab(c, world, r) for r in range(world)]
     assert [sl.s.nz for sl in slabs] == [sl.lay.nz_local for sl in slabs]
+    if not zero_copy:                                  # the staged exchange: a solver without plane_views
+        class Staged:
+            def __init__(self, s):
+                self.sweep, self.get_planes, self.set_planes, self.get_primitives = s.sweep, s.get_planes, s.set_planes, s.get_primitives
+        for sl in slabs:
+            sl.s = Staged(sl.s)
     zslab.step_in_process(slabs, 6)
     U = torch.cat([sl.owned_conserved() for sl in slabs], dim=1).cpu().numpy()
     for f, k in enumerate(parity.CONS):
@@ -595,6 +601,12 @@ def test_planes_round_trip_and_errors():
         s.set_state(*[torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")])
         U = torch.stack(list(s.get_conserved().values()))
         assert torch.equal(s.get_planes(2, 4), U[:, 2:6])
+        views = s.plane_views(2, 4)                              # aliases of the state buffer, storage dtype
+        assert views[0].dtype == (torch.float64 if precision == 64 else torch.float32)
+        assert all(torch.equal(v.double(), U[f, 2:6]) for f, v in enumerate(views))
+        views[4].mul_(2.0)
+        assert torch.equal(s.get_planes(2, 4)[4], 2.0 * U[4, 2:6])
+        views[4].mul_(0.5)
         s.set_planes(5, U[:, 0:3].contiguous())
         V = torch.stack(list(s.get_conserved().values()))
         assert torch.equal(V[:, 5:8], U[:, 0:3]) and torch.equal(V[:, :5], U[:, :5]) and torch.equal(V[:, 8:], U[:, 8:])
