@@ -40,6 +40,14 @@ namespace shk {
 constexpr int NF = 5;       // E, M_par, M_perp1, M_perp2, R
 constexpr int GH = 4;       // ghost depth = dependency radius of one sweep
 constexpr double VAC_E = 0x1p-498;      // reading G7: a cell with !(E >= 2^-498) is vacuum (E^2, |M|^2 not representable below)
+// Newton on v stops once a step is below NEWT_DV: the step taken is (to first order) the error BEFORE it, and the error
+// after it is 2^-20 of that (slope seeded by rcp64h) plus the quadratic term, i.e. below 1e-16 -- the iterate is converged
+// to fp64 without spending one more iteration on confirming it (a step <= 1e-15, the rule of PAPER.md:109's iteration in
+// the oracle, bounds the same error from the other side).
+#ifndef SHK_NEWT_DV
+#define SHK_NEWT_DV 1e-10
+#endif
+constexpr double NEWT_DV = SHK_NEWT_DV;
 constexpr int EOS_GAMMA = 0;    // p = (Gamma-1) e            (m = 0): closed-form velocity
 constexpr int EOS_MASS = 1;     // p = (Gamma-1)(e - m n)     (m > 0): safeguarded Newton
 constexpr int EOS_TABLE = 2;    // p = bilinear table P(e, n) (reading T1): the same safeguarded Newton
@@ -318,8 +326,7 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
             if (!(vn >= lo && vn <= hi)) vn = double(0.5) * (lo + hi);
             const double dv = fabs(vn - v);
             v = vn;
-            const double tol = 1e-15;
-            if (__all_sync(__activemask(), dv <= tol)) break;
+            if (__all_sync(__activemask(), dv <= NEWT_DV)) break;
         }
         o.w = fmax(fma(-v, v, double(1)), double(0));
         const double eraw = fma(-Mabs, v, E);
@@ -566,7 +573,7 @@ __device__ __forceinline__ void c2p_pairs_general(const Consts<T>& k, const PL& 
         na.init(k.d, ua); nb.init(k.d, ub);
         for (int it = 0; it < 48; ++it) {
             const double da = na.iter(k.d), db = nb.iter(k.d);
-            if (__all_sync(0xffffffffu, fmax(da, db) <= 1e-15)) break;
+            if (__all_sync(0xffffffffu, fmax(da, db) <= NEWT_DV)) break;
         }
         na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);
         store2(scr + 256 * pi, (T)va, (T)pa);
@@ -884,7 +891,7 @@ struct HalfStep {
                 nb.init_em(k.d, (double)b0, (double)b1, (double)b2, (double)b3);
                 for (int it = 0; it < 48; ++it) {
                     const double da = na.iter(k.d), db = nb.iter(k.d);
-                    if (__all_sync(__activemask(), fmax(da, db) <= 1e-15)) break;
+                    if (__all_sync(__activemask(), fmax(da, db) <= NEWT_DV)) break;
                 }
                 double va, pa, vb, pb;
                 na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);
