@@ -148,6 +148,12 @@ int shasta_set_planes(shasta_t* h, int z0, int nplanes, const double* E_dev, con
  * ask again before every exchange, and order the writes before the next sweep on its stream.  After writing owned
  * planes through it, primitive fields written earlier are stale (halo planes: nobody reads theirs). */
 int shasta_plane_ptr(shasta_t* h, int field, int z0, void** ptr_dev);
+/* From now on the x and y sweeps update the planes z_lo .. z_hi-1 only (default: all, 0 .. nz); the z sweeps and the
+ * element-wise passes still cover every plane.  For a z-slab rank: its halo planes are overwritten before each z sweep
+ * anyway, so sweeping them along x and y is wasted work (8 of 8 + nz/P planes).  After an x or y sweep the planes
+ * outside the range hold stale data (and stale primitives) until they are written again (shasta_set_planes, a z sweep).
+ * 0 <= z_lo < z_hi <= nz, SHASTA_EINVAL otherwise; SHASTA_ESTATE with SHASTA_BATCH > 1. */
+int shasta_set_active_planes(shasta_t* h, int z_lo, int z_hi);
 
 /*
  * Advance nsteps time steps dt = lambda*dx.  One step = three fused sweep kernels, one per axis in

@@ -38,6 +38,7 @@ struct shasta {
     int cell_path;          // 1 = run the per-cell kernels also for the default scheme (A/B datapoint, tests)
     int predictor;          // 0 = R1 (eq. (17) alone), 1 = R2 (complete kernel at lambda/2): per-cell kernels
     int periodic;
+    int az_lo, az_hi;       // shasta_set_active_planes: x and y sweeps update the planes [az_lo, az_hi) only (default all)
     int periodic_z;         // SHASTA_BOUNDARY_Z: -1 = as `periodic`; 0 | 1 = rule of the z sweeps only (z-slab ranks: 0)
     int precision;          // 64 | 32
     int seg_override;
@@ -433,10 +434,14 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
     P.odiv = 0x7fffffff;
     P.counts = h->d_counts;
     const Consts<T> k = make_consts<T>(h);
+    const bool zrange = h->az_lo > 0 || h->az_hi < h->nz;      // single event only (checked in shasta_set_active_planes)
+    P.pbase = 0;
     if (axis == 0) {
         P.npencil = (long long)h->ny * h->nz * h->nbatch;
+        if (zrange) { P.pbase = (long long)h->az_lo * h->ny; P.npencil = (long long)h->az_hi * h->ny; }   // rows y + ny z
+        const long long nrow = P.npencil - P.pbase;
         P.stride_other = 0;
-        P.seg = auto_segment(h, axis, P.N, (P.npencil + 127) / 128);
+        P.seg = auto_segment(h, axis, P.N, (nrow + 127) / 128);
         P.nseg = (P.N + P.seg - 1) / P.seg;
         {
             // producer/consumer warp pairs, 32 rows per pair, 4 pairs per CTA; TMA tiles when possible (fp64, even nx)
@@ -447,7 +452,7 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
             for (int c = 0; c < 3; ++c) maps.fidx[1 + c] = 1 + perm[axis][c];
             if (tma) { maps.in = h->d_xmaps + src * NF; maps.out = h->d_xmaps + dst * NF; }
             const size_t smem = sizeof(X2Smem<T>);
-            dim3 grid((unsigned)((P.npencil + 127) / 128), (unsigned)P.nseg);
+            dim3 grid((unsigned)((nrow + 127) / 128), (unsigned)P.nseg);
             if (tma) {
                 auto kern = sweep_x2_kernel<T, EOS, EMIT == 1, true>;
                 int rc = opt_in_smem(h, (const void*)kern, smem);
@@ -468,8 +473,9 @@ int launch_sweep_t(shasta_t* h, int axis, cudaStream_t st)
             // producer/consumer warp pairs, 32 pencils (one x-block of a row) per pair, 4 pairs per CTA; TMA-fed when possible
             const long long nxb = (h->nx + 31) / 32;
             P.npencil = nxb * n[other] * h->nbatch;                             // pencil GROUPS (all events)
+            if (zrange && axis == 1) { P.pbase = nxb * h->az_lo; P.npencil = nxb * h->az_hi; }   // groups xb + nxb z
             P.odiv = (axis == 2 && h->nbatch > 1) ? h->ny : 0x7fffffff;
-            const long long ctas = (P.npencil + 3) / 4;
+            const long long ctas = (P.npencil - P.pbase + 3) / 4;
             P.seg = auto_segment(h, axis, P.N, ctas);
             P.nseg = (P.N + P.seg - 1) / P.seg;
             const bool tma = h->have_yzmap && !h->no_tma && P.N >= YZ_CH;
@@ -727,6 +733,7 @@ int shasta_create(shasta_t** out, int nx, int ny, int nz, double dx, double lamb
     h->precision = 64;
     h->diff = 1.0;
     h->periodic_z = -1;
+    h->az_lo = 0; h->az_hi = nz;
     h->graph_mode = 2;
     memcpy(h->table, kBranch, sizeof(kBranch));
     h->ntable = 18;
@@ -794,6 +801,8 @@ int shasta_set_option(shasta_t* h, int key, double value)
             return fail(h, SHASTA_ESTATE, "SHASTA_BATCH must be set before the first set_state");
         if ((double)h->nz * value > 2147483647.0 / 2)
             return fail(h, SHASTA_EINVAL, "SHASTA_BATCH: nz * batch too large");
+        if (value != 1.0 && (h->az_lo > 0 || h->az_hi < h->nz))
+            return fail(h, SHASTA_ESTATE, "SHASTA_BATCH > 1: not with shasta_set_active_planes");
         h->nbatch = (int)value;
         h->ncell = h->ncell1 * h->nbatch;
         return 0;
@@ -1002,6 +1011,18 @@ int shasta_set_planes(shasta_t* h, int z0, int nplanes, const double* E, const d
         }
     }
     h->prims_valid = false;
+    return 0;
+}
+
+int shasta_set_active_planes(shasta_t* h, int z_lo, int z_hi)
+{
+    if (!h) return SHASTA_EINVAL;
+    if (z_lo < 0 || z_hi > h->nz || z_lo >= z_hi)
+        return fail(h, SHASTA_EINVAL, "shasta_set_active_planes: need 0 <= z_lo < z_hi <= nz = %d", h->nz);
+    if (h->nbatch != 1 && (z_lo != 0 || z_hi != h->nz))
+        return fail(h, SHASTA_ESTATE, "shasta_set_active_planes: not with SHASTA_BATCH > 1");
+    drop_graphs(h);
+    h->az_lo = z_lo; h->az_hi = z_hi;
     return 0;
 }
 

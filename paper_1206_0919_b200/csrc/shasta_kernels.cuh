@@ -109,7 +109,8 @@ struct SweepParams {
     long long stride_other; // strided kernel: pencil p -> base = (p % nx) + (p / nx) * stride_other
     int nx;                 // extent of the contiguous axis
     int N;                  // extent of the sweep axis
-    long long npencil;      // number of pencils (rows for the x sweep)
+    long long npencil;      // END of the pencil range: pencils (x sweep: rows; y/z: groups of 32 pencils) pbase .. npencil-1
+    long long pbase;        // first pencil of the launch: 0, or the start of the active planes (shasta_set_active_planes)
     int seg;                // cells marched per work item
     int nseg;               // segments per pencil
     int periodic;           // boundary rule (reading G11)
@@ -1105,7 +1106,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
     YzPair<T>& S = reinterpret_cast<YzSmem<T>*>(smem_yz)->pair[warp & 3];
     const int bar_id = 4 * (warp & 3);                      // full0, full1, empty0, empty1 of this pair
     const int nxb = (P.nx + 31) >> 5;
-    const long long pg = (long long)blockIdx.x * 4 + (warp & 3);        // pencil group
+    const long long pg = P.pbase + (long long)blockIdx.x * 4 + (warp & 3);   // pencil group
     const bool idle = pg >= P.npencil;                      // npencil = nxb * n_other pencil GROUPS for this kernel
     const int oth = (int)(pg / nxb);
     const int x0 = 32 * (int)(pg - (long long)oth * nxb);
@@ -1391,7 +1392,7 @@ __global__ void __launch_bounds__(256, (EOS == EOS_GAMMA) ? 2 : GEN_CTAS) sweep_
     const bool producer = warp < 4;
     X2Pair<T>& S = reinterpret_cast<X2Smem<T>*>(smem_x2)->pair[warp & 3];
     const int bar_id = 4 * (warp & 3);                      // full0, full1, empty0, empty1 of this pair
-    const long long row0 = (long long)blockIdx.x * 128 + (warp & 3) * 32;
+    const long long row0 = P.pbase + (long long)blockIdx.x * 128 + (warp & 3) * 32;
     const bool idle = row0 >= P.npencil;
     const int nrows = (int)min(32LL, P.npencil - row0);
     const int j0 = blockIdx.y * P.seg;

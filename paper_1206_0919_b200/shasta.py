@@ -21,7 +21,7 @@ BRANCH = (0, 1, 2, 0, 2, 1, 2, 0, 1, 2, 1, 0, 1, 2, 0, 1, 0, 2)
 # every symbol include/shasta.h declares
 SYMBOLS = (
     "shasta_create", "shasta_destroy", "shasta_set_option", "shasta_set_eos_table", "shasta_set_sweep_table", "shasta_set_state",
-    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_get_planes", "shasta_set_planes", "shasta_plane_ptr", "shasta_step", "shasta_sweep",
+    "shasta_set_state_host", "shasta_set_conserved", "shasta_get_conserved", "shasta_get_planes", "shasta_set_planes", "shasta_plane_ptr", "shasta_set_active_planes", "shasta_step", "shasta_sweep",
     "shasta_get_primitives", "shasta_get_primitives_host", "shasta_conserved_totals", "shasta_diagnostics",
     "shasta_launch_count", "shasta_graph_launch_count", "shasta_step_index", "shasta_kernel_name", "shasta_last_error",
     "shasta_conserved_totals_static", "shasta_conserved_totals_static_max_cells",
@@ -54,6 +54,7 @@ def load():
     L.shasta_get_planes.argtypes = [_vp, C.c_int, C.c_int] + [_dp] * 5 + [_vp]
     L.shasta_set_planes.argtypes = [_vp, C.c_int, C.c_int] + [_dp] * 5 + [_vp]
     L.shasta_plane_ptr.argtypes = [_vp, C.c_int, C.c_int, C.POINTER(_vp)]
+    L.shasta_set_active_planes.argtypes = [_vp, C.c_int, C.c_int]
     L.shasta_step.argtypes = [_vp, C.c_int, _vp]
     L.shasta_sweep.argtypes = [_vp, C.c_int, C.c_int, _vp]
     L.shasta_get_primitives.argtypes = [_vp] + [_dp] * 6 + [_vp]
@@ -245,6 +246,9 @@ class Shasta:
         """planes: (5, nplanes, ny, nx) CUDA tensor written over planes z0 .. z0+nplanes-1 of the conserved state"""
         self._chk(self._L.shasta_set_planes(self._h, int(z0), int(planes.shape[1]), *[_dev(planes[f]) for f in range(5)],
                                             _stream_ptr(stream)), "shasta_set_planes")
+
+    def set_active_planes(self, z_lo, z_hi):
+        self._chk(self._L.shasta_set_active_planes(self._h, int(z_lo), int(z_hi)), "shasta_set_active_planes")
 
     def plane_views(self, z0, nplanes):
         """shasta_plane_ptr: the planes z0 .. z0+nplanes-1 of the five conserved fields as five CUDA tensors (nplanes, ny, nx)

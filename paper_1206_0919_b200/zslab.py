@@ -192,6 +192,7 @@ def make_gpu_slab(c, world: int, rank: int, table=BRANCH, **kw) -> ZSlab:
     lay = layout(c["nz"], world, rank, bool(c["boundary"]))
     s = Shasta(c["nx"], c["ny"], lay.nz_local, c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"],
                boundary_z=(0 if world > 1 else None), **kw)
+    s.set_active_planes(lay.lo, lay.lo + lay.nz)           # x and y sweeps skip the halo planes (refreshed before each z sweep)
     idx = np.asarray(local_planes(lay, c["nz"]))
     s.set_state(*[torch.from_numpy(np.ascontiguousarray(c[k][idx])).cuda() for k in ("e", "n", "vx", "vy", "vz")])
     return ZSlab(s, lay, table)

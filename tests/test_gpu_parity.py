@@ -614,6 +614,34 @@ def test_zslab_fp32_storage_and_general_eos():
     assert max(v[0] for v in errs.values()) <= 1e-13, errs
 
 
+@pytest.mark.parametrize("shape", [(40, 24, 13), (64, 33, 12)])
+def test_active_planes_restrict_the_x_and_y_sweeps(shape):
+    # shasta_set_active_planes: x and y sweeps update planes [3, 9) only -- the same bits there as the full sweep -- and the
+    # z sweep still covers every plane (ragged cp.async shapes and TMA-fed ones)
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta, ShastaError
+    nx, ny, nz = shape
+    c = inputs.random_state(nx, ny, nz, seed=71, kind="rough", boundary=inputs.PERIODIC)
+    st = [torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")]
+    for axis in (0, 1, 2):
+        full = Shasta(nx, ny, nz, c["dx"], c["lam"], c["gamma"], c["boundary"])
+        part = Shasta(nx, ny, nz, c["dx"], c["lam"], c["gamma"], c["boundary"])
+        part.set_active_planes(3, 9)
+        for s in (full, part):
+            s.set_state(*st)
+            s.sweep(axis, 1)
+        a, b = full.get_planes(0, nz), part.get_planes(0, nz)
+        lo, hi = (0, nz) if axis == 2 else (3, 9)
+        assert torch.equal(a[:, lo:hi], b[:, lo:hi]), axis
+        pa, pb = full.get_primitives(), part.get_primitives()
+        assert all(torch.equal(pa[k][lo:hi], pb[k][lo:hi]) for k in pa), axis
+    with pytest.raises(ShastaError):
+        part.set_active_planes(5, 5)
+    with pytest.raises(ShastaError):
+        part.set_active_planes(0, nz + 1)
+    part.set_active_planes(0, nz)
+
+
 def test_planes_round_trip_and_errors():
     import torch
     from paper_1206_0919_b200.shasta import Shasta, ShastaError
