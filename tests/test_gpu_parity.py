@@ -557,6 +557,35 @@ def test_variant_explicit_antidiffusion_config1(oracle):
     parity.assert_parity(got, ref, TOL64, label="config1 explicit antidiffusion")
 
 
+# ------------------------------------------------------------------ long runs (no oracle: properties that hold at any length)
+@pytest.mark.parametrize("precision", [64, 32])
+def test_long_runs_stay_finite_causal_and_conservative(precision):
+    # (a) periodic box, rough state, 1500 steps: E and R are conserved by the flux form (eqs. (17), (22)) -- to rounding in
+    # fp64, to the fp32 storage rounding otherwise -- and every primitive stays finite with |v| < 1;  (b) hotspots
+    # expanding into a near-vacuum exterior through outflow faces, 600 steps: the front runs at the causality clamp
+    # (|M| <= (1 - 1e-12) E, readings G6-G8), nothing becomes NaN, e >= 0
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+
+    def run(c, steps, chunk):
+        s = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"], precision=precision)
+        s.set_state(*[torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")])
+        t0 = np.array(s.conserved_totals())
+        for _ in range(0, steps, chunk):
+            s.step(chunk)
+            p = s.get_primitives()
+            assert all(bool(torch.isfinite(v).all()) for v in p.values())
+            assert float((p["vx"] ** 2 + p["vy"] ** 2 + p["vz"] ** 2).max()) < 1.0
+            assert float(p["e"].min()) >= 0.0 and float(p["p"].min()) >= 0.0 and float(p["n"].min()) >= 0.0
+        return t0, np.array(s.conserved_totals()), s
+
+    t0, t1, _ = run(inputs.random_state(48, 48, 48, seed=3, kind="rough", boundary=inputs.PERIODIC), 1500, 500)
+    tol = 1e-12 if precision == 64 else 1e-6
+    assert abs(t1[0] - t0[0]) <= tol * abs(t0[0]) and abs(t1[4] - t0[4]) <= tol * abs(t0[4])
+    t0, t1, s = run(inputs.hotspots(64, steps=0), 600, 200)
+    assert t1[0] < t0[0] and s.diagnostics()[0] > 0          # matter left through the faces; the clamp did fire at the front
+
+
 # ------------------------------------------------------------------ z-slab decomposition (host logic: test_zslab.py)
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
 @pytest.mark.parametrize("world,zero_copy", [(2, True), (3, True), (3, False)])
