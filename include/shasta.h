@@ -84,7 +84,7 @@ typedef struct shasta shasta_t;   /* opaque */
 /*
  * Create a solver for an nx*ny*nz grid.  The scheme depends on lambda = dt/dx only
  * (eqs. (15)-(17)); dx enters shasta_conserved_totals.  0 < lambda <= 0.5
- * (SHASTA's stability range, the denominators of eq. (15) stay > 0), eos_gamma > 1
+ * (SHASTA's stability range, the denominators of eq. (15) stay > 0), 1 < eos_gamma < 2 (causal sound speed)
  * (4/3 gives p = e/3).  Allocates 2x5 conserved fields (ping-pong, the paper's double
  * buffering PAPER.md:161) + 6 primitive fields on the current device.
  */

@@ -557,6 +557,24 @@ def test_variant_explicit_antidiffusion_config1(oracle):
     parity.assert_parity(got, ref, TOL64, label="config1 explicit antidiffusion")
 
 
+# ------------------------------------------------------------------ parameter range of shasta_create
+@pytest.mark.parametrize("lam", [0.5, 0.25, 0.05])
+@pytest.mark.parametrize("gamma", [1.2, 5.0 / 3.0, 1.8])
+def test_lambda_and_gamma_range(oracle, lam, gamma):
+    # lambda up to the stability limit 0.5 (eq. (15)'s denominators stay > 0) and down to slow flows; Gamma = 1.2 and 5/3
+    # run the closed-form kernels (5/3 is their limit), Gamma = 1.8 the Newton kernels with m = 0 (shasta_create wants
+    # 1 < Gamma < 2: c_s^2 = Gamma - 1 < 1)
+    # Not beyond 1.8: in a cell at the causality clamp the contraction factor of the paper's fixed-point map is
+    # Gamma - 1, and the ORACLE's 200 iterations (reading G9) then stop short of the root -- 0.9^200 = 7e-10 at Gamma = 1.9,
+    # measured 7e-11 in v against bisection, 6e-6 in n = R sqrt(1 - v^2) -- while the kernels' bracketed Newton reaches it.
+    c = inputs.random_state(37, 19, 23, seed=int(100 * lam + 10 * gamma), kind="rough", gamma=gamma, boundary=inputs.PERIODIC)
+    c["lam"] = lam
+    ref, _ = parity.run_oracle(oracle, c, steps=2)
+    got, s = parity.run_gpu(c, steps=2)
+    tol = 1e-12 if gamma < 1.7 else 1e-11
+    assert_kernel_parity(got, ref, f"lambda {lam} gamma {gamma}", tol_cons=tol, tol_prim=tol)
+
+
 # ------------------------------------------------------------------ long runs (no oracle: properties that hold at any length)
 @pytest.mark.parametrize("precision", [64, 32])
 def test_long_runs_stay_finite_causal_and_conservative(precision):
