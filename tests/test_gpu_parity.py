@@ -575,6 +575,57 @@ def test_lambda_and_gamma_range(oracle, lam, gamma):
     assert_kernel_parity(got, ref, f"lambda {lam} gamma {gamma}", tol_cons=tol, tol_prim=tol)
 
 
+# ------------------------------------------------------------------ symmetries of the scheme on the GPU path itself (no oracle)
+def test_energy_scale_homogeneity_is_bitwise():
+    # p = (Gamma-1) e, m = 0: eqs. (9)-(22) are homogeneous of degree one in (E, M) and leave R alone, and v depends on M/E
+    # only.  Scaling e by a power of two must therefore scale E, M, e, p by it EXACTLY and leave R, n, v untouched -- through
+    # the closed-form cons2prim (E^2, |M|^2 up to 2^+-400), the limiter and the causality clamp.  Absolute thresholds
+    # (vacuum 2^-498) are far away.
+    c = inputs.random_state(40, 24, 13, seed=91, kind="rough", boundary=inputs.PERIODIC)
+    base, _ = parity.run_gpu(c, steps=3)
+    for k in (200, -200):
+        sc = 2.0 ** k
+        cs = dict(c)
+        cs["e"] = c["e"] * sc
+        got, _ = parity.run_gpu(cs, steps=3)
+        for f in ("E", "Mx", "My", "Mz", "e", "p"):
+            assert np.array_equal(got[f], base[f] * sc), (k, f)
+        for f in ("R", "n", "vx", "vy", "vz"):
+            assert np.array_equal(got[f], base[f]), (k, f)
+
+
+@pytest.mark.parametrize("shape", [(37, 19, 23), (64, 32, 8)])
+def test_axis_permutation_covariance_is_bitwise(shape):
+    # the x kernel (rows in swizzled 4-cell tiles) and the y/z kernel (x across the lanes) are different code around the same
+    # per-pencil arithmetic: three x sweeps of a conserved state = three y (z) sweeps of the state with the axes rotated
+    # CYCLICALLY (so that the two transverse momenta keep their order in |M|^2 = M_par^2 + (M_perp1^2 + M_perp2^2), which is
+    # not associative).  Starts from conserved fields: prim2cons sums v^2 in natural order, which a rotation changes by an ulp.
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    nx, ny, nz = shape
+    c = inputs.random_state(nx, ny, nz, seed=92, kind="rough", boundary=inputs.PERIODIC)
+    U0 = parity.run_gpu(c, steps=0)[0]
+
+    def sweeps(U, dims, axis):
+        s = Shasta(dims[2], dims[1], dims[0], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"])
+        s.set_conserved(*[torch.from_numpy(np.ascontiguousarray(U[k])).cuda() for k in parity.CONS])
+        s.set_sweep_table([axis] * 3)
+        s.step(1)
+        return {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
+
+    ref = sweeps(U0, (nz, ny, nx), 0)
+    # arrays are (z, y, x).  axis 1: (z', y', x') = (y, x, z);  axis 2: (z', y', x') = (x, z, y);  old component -> new name
+    for axis, perm, new_of in ((1, (1, 2, 0), {"x": "y", "y": "z", "z": "x"}), (2, (2, 0, 1), {"x": "z", "y": "x", "z": "y"})):
+        Ut = {k: np.transpose(U0[k], perm) for k in ("E", "R")}
+        for old, new_ in new_of.items():
+            Ut["M" + new_] = np.transpose(U0["M" + old], perm)
+        got = sweeps(Ut, Ut["E"].shape, axis)
+        back = tuple(np.argsort(perm))
+        names = {"E": "E", "R": "R", **{"M" + old: "M" + new_ for old, new_ in new_of.items()}}
+        for k, kt in names.items():
+            assert np.array_equal(np.transpose(got[kt], back), ref[k]), (axis, k)
+
+
 # ------------------------------------------------------------------ long runs (no oracle: properties that hold at any length)
 @pytest.mark.parametrize("precision", [64, 32])
 def test_long_runs_stay_finite_causal_and_conservative(precision):
