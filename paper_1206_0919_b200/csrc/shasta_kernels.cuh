@@ -299,6 +299,7 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
             }
             v = fmin(fmax(Mabs * fast_rcp(E + Ph), lo), hi);
         }
+        bool done = false;
         for (int it = 0; it < 48; ++it) {
             // no library sqrt / division in the loop: w2 >= 2e-12 (v <= 1 - delta) and dg >= E - (Gamma-1)|M| v > 0
             // are normal positive numbers, so the MUFU-seeded fast_rsqrt / fast_rcp apply (<= 2 ulp; the iteration
@@ -325,9 +326,12 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
             if (g > double(0)) hi = v; else lo = v;
             double vn = v - g * fast_rcp(dg);
             if (!(vn >= lo && vn <= hi)) vn = double(0.5) * (lo + hi);
+            // a lane stops moving with its own first converged step: what it returns does not depend on the lanes it shares
+            // the loop with (an idle lane may solve for garbage, a partner may need more steps) -- run-to-run reproducible
             const double dv = fabs(vn - v);
-            v = vn;
-            if (__all_sync(__activemask(), dv <= NEWT_DV)) break;
+            if (!done) v = vn;
+            done = done || dv <= NEWT_DV;
+            if (__all_sync(__activemask(), done)) break;
         }
         o.w = fmax(fma(-v, v, double(1)), double(0));
         const double eraw = fma(-Mabs, v, E);
@@ -352,11 +356,11 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
 // of TWO cells can run as one loop with two independent dependency chains (c2p_group below).  The Newton iteration of one
 // cell is a serial chain of ~25 dependent fp64 operations per step; with one cell at a time the producer warp issued an
 // instruction every ~7 cycles (round 1: config 3 at a third of the Gamma-law speed).  Same formulas, same bracket, same
-// tolerance; a cell that has converged keeps iterating at its fixed point until its partner (and the warp) is done.
+// tolerance; a cell that has converged stays where it is while its partner (and the warp) finish.
 template <int EOS>
 struct Newt {
     double E, Mabs, R, mR, v, lo, hi, M1, M2;
-    bool vac;
+    bool vac, done;
     __device__ __forceinline__ void init(const EosD& k, const double (&u)[NF])
     {
         init_em(k, u[0], u[1], fma(u[1], u[1], fma(u[2], u[2], u[3] * u[3])), u[4]);
@@ -365,6 +369,7 @@ struct Newt {
     __device__ __forceinline__ void init_em(const EosD& k, double E_, double M1_, double M2_, double R_)
     {
         E = E_; M1 = M1_; M2 = M2_; R = R_;
+        done = false;
         vac = !(E >= VAC_E);
         if (vac) { E = 1.0; M1 = 0.0; M2 = 0.0; }
         const double lim = k.omd * E;
@@ -385,7 +390,7 @@ struct Newt {
         }
         v = fmin(fmax(Mabs * fast_rcp(E + Ph), lo), hi);
     }
-    __device__ __forceinline__ double iter(const EosD& k)
+    __device__ __forceinline__ void iter(const EosD& k)
     {
         const double w2 = fma(-v, v, 1.0);
         const double rw = fast_rsqrt3(w2);              // 2^-58: w enters P, which fixes the root
@@ -407,9 +412,12 @@ struct Newt {
         if (g > 0.0) hi = v; else lo = v;
         double vn = v - g * rcp64h(dg);                 // slope to 2^-20 is enough: the step it scales goes to 0
         if (!(vn >= lo && vn <= hi)) vn = 0.5 * (lo + hi);
+        // The cell stops moving with its own first converged step: its result does not depend on
+        // the cells it shares the loop with (its partner, the other lanes of the vote, an idle lane solving for whatever its
+        // shared-memory slot held) -- the same bits from run to run and for any segmentation of the march.  The loops vote on `done`.
         const double dv = fabs(vn - v);
-        v = vn;
-        return dv;
+        if (!done) v = vn;
+        done = done || dv <= NEWT_DV;
     }
     // v_par = M_par v / |M| and p of the converged state (vacuum: 0, 0)
     __device__ __forceinline__ void finish(const EosD& k, double& vpar, double& p) const
@@ -573,8 +581,8 @@ __device__ __forceinline__ void c2p_pairs_general(const Consts<T>& k, const PL& 
         Newt<EOS> na, nb;
         na.init(k.d, ua); nb.init(k.d, ub);
         for (int it = 0; it < 48; ++it) {
-            const double da = na.iter(k.d), db = nb.iter(k.d);
-            if (__all_sync(0xffffffffu, fmax(da, db) <= NEWT_DV)) break;
+            na.iter(k.d); nb.iter(k.d);
+            if (__all_sync(0xffffffffu, na.done && nb.done)) break;
         }
         na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);
         store2(scr + 256 * pi, (T)va, (T)pa);
@@ -891,8 +899,8 @@ struct HalfStep {
                 na.init_em(k.d, (double)a0, (double)a1, (double)a2, (double)a3);
                 nb.init_em(k.d, (double)b0, (double)b1, (double)b2, (double)b3);
                 for (int it = 0; it < 48; ++it) {
-                    const double da = na.iter(k.d), db = nb.iter(k.d);
-                    if (__all_sync(__activemask(), fmax(da, db) <= NEWT_DV)) break;
+                    na.iter(k.d); nb.iter(k.d);
+                    if (__all_sync(__activemask(), na.done && nb.done)) break;
                 }
                 double va, pa, vb, pb;
                 na.finish(k.d, va, pa); nb.finish(k.d, vb, pb);

@@ -128,6 +128,29 @@ def test_run_to_run_bitwise_reproducible(shape):
             assert np.array_equal(first[k], again[k]), k
 
 
+@pytest.mark.parametrize("eos", ["mass", "table"])
+def test_general_eos_bits_do_not_depend_on_idle_lanes_or_stale_memory(eos):
+    # Newton kernels, ragged shapes (warps with idle lanes / rows whose shared-memory slots hold whatever was there): until a
+    # converged cell was frozen in place, the warp-wide vote let such lanes decide how often the others iterated, and results
+    # moved by an ulp from run to run (found with the scale-homogeneity test).  Other problems run in between to change
+    # what stale memory holds.
+    import hashlib
+    tab = inputs.eos_table("soft") if eos == "table" else None
+    kw = dict(gamma=5.0 / 3.0, mass=1.0 if eos == "mass" else 0.0, boundary=inputs.PERIODIC)
+
+    def digest(r):
+        return hashlib.md5(b"".join(np.ascontiguousarray(r[f]).tobytes() for f in sorted(r))).hexdigest()
+
+    for shape in ((24, 20, 28), (40, 24, 13)):
+        c = inputs.random_state(*shape, seed=93, kind="rough", **kw)
+        seen = set()
+        for rep in range(6):
+            seen.add(digest(parity.run_gpu(c, steps=3, eos_table=tab)[0]))
+            if rep % 2 == 0:
+                parity.run_gpu(inputs.random_state(33, 17, 9, seed=rep, kind="rough", **kw), steps=1, eos_table=tab)
+        assert len(seen) == 1, (shape, seen)
+
+
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
 @pytest.mark.parametrize("shape", [(37, 19, 23), (64, 33, 6)])
 def test_fp32_storage_kernel_level(oracle, bc, shape):
@@ -592,6 +615,18 @@ def test_energy_scale_homogeneity_is_bitwise():
             assert np.array_equal(got[f], base[f] * sc), (k, f)
         for f in ("R", "n", "vx", "vy", "vz"):
             assert np.array_equal(got[f], base[f]), (k, f)
+    # p = (Gamma-1)(e - m n): homogeneous in (e, n) together -- the Newton kernels (MUFU seeds, bracket, warp votes) too
+    c = inputs.random_state(24, 20, 28, seed=93, kind="rough", gamma=5.0 / 3.0, mass=1.0, boundary=inputs.PERIODIC)
+    base, _ = parity.run_gpu(c, steps=3)
+    for k in (200, -200):
+        sc = 2.0 ** k
+        cs = dict(c)
+        cs["e"], cs["n"] = c["e"] * sc, c["n"] * sc
+        got, _ = parity.run_gpu(cs, steps=3)
+        for f in ("E", "Mx", "My", "Mz", "R", "e", "p", "n"):
+            assert np.array_equal(got[f], base[f] * sc), (k, f)
+        for f in ("vx", "vy", "vz"):
+            assert np.array_equal(got[f], base[f]), (k, f)
 
 
 @pytest.mark.parametrize("shape", [(37, 19, 23), (64, 32, 8)])
@@ -705,11 +740,10 @@ def test_zslab_fp32_storage_and_general_eos():
     slabs = [zslab.make_gpu_slab(c, 2, r) for r in range(2)]
     zslab.step_in_process(slabs, 6)
     U = torch.cat([sl.owned_conserved() for sl in slabs], dim=1).cpu().numpy()
-    # not bitwise here: the Newton loop of the general EOS ends on a warp-wide vote over the two cells it solves together,
-    # and which cells share a loop depends on where the march started (as with other segment lengths); a converged cell
-    # that iterates on with its partner can move by an ulp
-    errs = parity.field_errors(dict(zip(parity.CONS, U)), {k: one[k] for k in parity.CONS})
-    assert max(v[0] for v in errs.values()) <= 1e-13, errs
+    # bitwise here too: a cell of the Newton loop stops moving with its own first converged step, whatever the cells it
+    # shares the loop (and the warp vote) with -- which depends on where the march started
+    for f, k in enumerate(parity.CONS):
+        assert np.array_equal(U[f], one[k]), k
 
 
 @pytest.mark.parametrize("shape", [(40, 24, 13), (64, 33, 12)])
