@@ -629,6 +629,48 @@ def test_energy_scale_homogeneity_is_bitwise():
             assert np.array_equal(got[f], base[f]), (k, f)
 
 
+@pytest.mark.parametrize("eos", ["gamma", "mass", "table"])
+@pytest.mark.parametrize("shape,shift", [((37, 19, 23), (5, 3, 7)), ((64, 32, 16), (33, 1, 9)), ((130, 6, 5), (64, 2, 1))])
+def test_translation_invariance_is_bitwise(eos, shape, shift):
+    # periodic box: the state rolled by (sx, sy, sz) cells gives the result rolled by the same shift, bit for bit -- whichever
+    # tile, group phase, segment or lane a cell lands in, and whether its neighbours arrive through the ghost wrap or not
+    nx, ny, nz = shape
+    tab = inputs.eos_table("soft") if eos == "table" else None
+    c = inputs.random_state(nx, ny, nz, seed=95, kind="rough", gamma=5.0 / 3.0, mass=1.0 if eos == "mass" else 0.0,
+                            boundary=inputs.PERIODIC)
+    base, _ = parity.run_gpu(c, steps=6, eos_table=tab)
+    sx, sy, sz = shift
+    cr = dict(c)
+    for k in ("e", "n", "vx", "vy", "vz"):
+        cr[k] = np.ascontiguousarray(np.roll(c[k], (sz, sy, sx), axis=(0, 1, 2)))
+    got, _ = parity.run_gpu(cr, steps=6, eos_table=tab)
+    for k in parity.CONS + parity.PRIM:
+        assert np.array_equal(got[k], np.roll(base[k], (sz, sy, sx), axis=(0, 1, 2))), k
+
+
+@pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_state_uniform_along_an_axis_stays_uniform_bitwise(axis, bc):
+    # a state that does not depend on one coordinate (and has no velocity along it) keeps that property exactly: the sweep
+    # along that axis must be the identity in every cell, edge cells and ghost cells included, and the other sweeps must treat
+    # every copy alike (P11 of the oracle, here on the kernels: 2-D flow in a 3-D grid)
+    shape = [29, 21, 18]                                   # (nz, ny, nx)
+    c2 = inputs.random_state(*[1 if a == axis else n for a, n in ((0, shape[2]), (1, shape[1]), (2, shape[0]))], seed=96,
+                             kind="rough", boundary=bc)
+    c = dict(c2)
+    reps = [1, 1, 1]
+    reps[2 - axis] = shape[2 - axis]
+    for k in ("e", "n", "vx", "vy", "vz"):
+        c[k] = np.ascontiguousarray(np.tile(c2[k], reps))
+    c["v" + "xyz"[axis]] = np.zeros_like(c["e"])
+    c["nz"], c["ny"], c["nx"] = c["e"].shape
+    got, _ = parity.run_gpu(c, steps=6)
+    for k in parity.CONS + parity.PRIM:
+        a = np.moveaxis(got[k], 2 - axis, 0)
+        assert np.array_equal(a, np.broadcast_to(a[0], a.shape)), k
+    assert float(np.abs(got["v" + "xyz"[axis]]).max()) == 0.0
+
+
 @pytest.mark.parametrize("shape", [(37, 19, 23), (64, 32, 8)])
 def test_axis_permutation_covariance_is_bitwise(shape):
     # the x kernel (rows in swizzled 4-cell tiles) and the y/z kernel (x across the lanes) are different code around the same
