@@ -147,3 +147,42 @@ def test_boundary_rules(oracle):
     o = _mk(oracle, c); before = o.get_conserved()["E"].copy(); o.step(10)
     after = o.get_conserved()["E"]
     assert np.array_equal(before[..., :20], after[..., :20]) and np.array_equal(before[..., -20:], after[..., -20:])
+
+
+@pytest.mark.parametrize("mass", [0.0, 1.0])
+def test_P16_translation_invariance_periodic_bitwise(oracle, mass):
+    # periodic box: rolling the state by (sx, sy, sz) cells rolls the result, bit for bit.  A wrong wrap index, a ghost depth
+    # short by one, or a sweep that treats an edge cell differently from an interior one breaks it.
+    c = inputs.random_state(13, 11, 9, seed=5, kind="rough", gamma=5.0 / 3.0, mass=mass, boundary=inputs.PERIODIC)
+    o = _mk(oracle, c)
+    o.step(6)
+    base = {**o.get_conserved(), **o.get_primitives()}
+    sh = (4, 7, 5)                                              # (sz, sy, sx)
+    cr = dict(c)
+    for k in ("e", "n", "vx", "vy", "vz"):
+        cr[k] = np.ascontiguousarray(np.roll(c[k], sh, axis=(0, 1, 2)))
+    o2 = _mk(oracle, cr)
+    o2.step(6)
+    got = {**o2.get_conserved(), **o2.get_primitives()}
+    for k in base:
+        assert np.array_equal(got[k], np.roll(base[k], sh, axis=(0, 1, 2))), k
+
+
+def test_P17_energy_scale_homogeneity_bitwise(oracle):
+    # p = (Gamma-1) e: eqs. (9)-(22) are homogeneous of degree one in (E, M) and v depends on M/E only, so a power-of-two
+    # factor on e scales E, M, e, p exactly and leaves R, n, v alone -- a stray absolute constant anywhere would show
+    c = inputs.random_state(12, 10, 8, seed=6, kind="rough", boundary=inputs.PERIODIC)
+    o = _mk(oracle, c)
+    o.step(3)
+    base = {**o.get_conserved(), **o.get_primitives()}
+    for k in (60, -60):
+        sc = 2.0 ** k
+        cs = dict(c)
+        cs["e"] = c["e"] * sc
+        o2 = _mk(oracle, cs)
+        o2.step(3)
+        got = {**o2.get_conserved(), **o2.get_primitives()}
+        for f in ("E", "Mx", "My", "Mz", "e", "p"):
+            assert np.array_equal(got[f], base[f] * sc), (k, f)
+        for f in ("R", "n", "vx", "vy", "vz"):
+            assert np.array_equal(got[f], base[f]), (k, f)
