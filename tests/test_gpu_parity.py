@@ -734,7 +734,7 @@ def test_long_runs_stay_finite_causal_and_conservative(precision):
 
 # ------------------------------------------------------------------ z-slab decomposition (host logic: test_zslab.py)
 @pytest.mark.parametrize("bc", [inputs.OUTFLOW, inputs.PERIODIC])
-@pytest.mark.parametrize("world,zero_copy", [(2, True), (3, True), (3, False)])
+@pytest.mark.parametrize("world,zero_copy", [(2, True), (3, True), (3, False), (7, True)])     # 7: slabs of 4-5 planes, the minimum
 def test_zslab_in_process_equals_the_single_domain_run(oracle, bc, world, zero_copy):
     # the slabs of one event as `world` handles on this GPU, planes carried by shasta_get_planes / shasta_set_planes:
     # same kernels, same neighbourhood for every owned cell -> the same bits as one handle over the whole grid
