@@ -201,6 +201,38 @@ def test_vacuum_and_superluminal_cells(oracle):
     assert all(np.all(np.isfinite(v)) for v in got.values())
 
 
+def test_vacuum_front_general_eos_sweep_by_sweep(oracle):
+    # p = (Gamma-1)(e - m n), a ball of matter in an EXACT-zero exterior.  Run freely, GPU and oracle drift apart here by 6e-4
+    # within two steps (Gamma-law: 2e-8, next test; the oracle's own strict / FMA builds: 4e-6): just outside the front a
+    # cell's new E is a rounding residue of either sign -- vacuum (v = 0) on one side, a light-like cell (v ~ 1) on the
+    # other -- and that velocity enters Q+- (eq. (15)) of a front cell of size 5e-4.  That is the method's sensitivity at an
+    # exact vacuum, not an arithmetic difference: started from the SAME state, every single sweep of the first two steps
+    # agrees to rounding, which is what this test pins; the free run must stay finite.
+    import torch
+    from paper_1206_0919_b200.shasta import Shasta
+    nx, ny, nz = 40, 36, 44
+    z, y, x = np.meshgrid(np.arange(nz) - nz / 2, np.arange(ny) - ny / 2, np.arange(nx) - nx / 2, indexing="ij")
+    inside = (x * x + y * y + z * z) < 36.0
+    cur = np.stack([np.where(inside, 1.0, 0.0)] + [np.where(inside, 0.2 * f, 0.0) for f in (1.0, -0.5, 0.25)] + [np.where(inside, 0.3, 0.0)])
+    gam, mass, lam = 5.0 / 3.0, 1.0, 0.4
+    free = Shasta(nx, ny, nz, 0.1, lam, gam, eos_mass=mass)
+    free.set_conserved(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in cur])
+    free.step(12)
+    assert all(bool(torch.isfinite(v).all()) for v in list(free.get_conserved().values()) + list(free.get_primitives().values()))
+    for axis in (0, 1, 2, 0, 2, 1):                                     # the sweeps of steps 0 and 1
+        s = Shasta(nx, ny, nz, 0.1, lam, gam, eos_mass=mass)
+        s.set_conserved(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in cur])
+        s.sweep(axis, 0)
+        G = np.stack([v.cpu().numpy() for v in s.get_conserved().values()])
+        A = np.moveaxis(cur, {0: 3, 1: 2, 2: 1}[axis], -1).copy()
+        for i in range(A.shape[1]):
+            for j in range(A.shape[2]):
+                A[:, i, j, :] = oracle.sweep_pencil(A[:, i, j, :], axis, lam, gam, mass, oracle.OUTFLOW)[0]
+        O = np.moveaxis(A, -1, {0: 3, 1: 2, 2: 1}[axis])
+        assert np.max(np.abs(G - O)) <= 1e-13, axis
+        cur = np.ascontiguousarray(O)
+
+
 @pytest.mark.parametrize("shape", [(600, 1, 1), (1, 600, 1), (40, 36, 44)])
 def test_matter_marching_into_exact_vacuum_stays_finite(oracle, shape):
     # E = 0 exterior (accepted by shasta_set_conserved): the numerical diffusion front carries E down through 1e-150,
