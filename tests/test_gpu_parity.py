@@ -180,8 +180,9 @@ def test_fp32_tma_and_cp_async_paths_same_bits(oracle, bc, shape, segment):
         assert emax <= 2e-5 and el1 <= 2e-6, (k, emax, el1)
 
 
-def test_vacuum_and_superluminal_cells(oracle):
-    # E <= 0 cells and |M| > E cells fed through set_conserved: projection + vacuum rule (P13)
+@pytest.mark.parametrize("eos", ["gamma", "mass", "table"])
+def test_vacuum_and_superluminal_cells(oracle, eos):
+    # E <= 0 cells and |M| > E cells fed through set_conserved: projection + vacuum rule (P13), all three EOS kinds
     import torch
     from paper_1206_0919_b200.shasta import Shasta
     rng = np.random.default_rng(5)
@@ -189,10 +190,12 @@ def test_vacuum_and_superluminal_cells(oracle):
     E = rng.uniform(0.5, 2.0, sh); E[2, 3, 4:7] = 0.0; E[4, 1, 9] = -0.1
     M = [rng.uniform(-0.4, 0.4, sh) for _ in range(3)]
     M[0][1, 2, 3] = 5.0
-    R = rng.uniform(0.1, 1.0, sh)
-    o = oracle.Oracle(16, 7, 6, 0.1, 0.4, 4.0 / 3.0)
+    R = rng.uniform(0.1, 1.0, sh) * (1.0 if eos == "gamma" else 0.3)
+    gam = 4.0 / 3.0 if eos == "gamma" else 5.0 / 3.0
+    kw = dict(eos_mass=1.0 if eos == "mass" else 0.0, eos_table=inputs.eos_table("soft") if eos == "table" else None)
+    o = oracle.Oracle(16, 7, 6, 0.1, 0.4, gam, **kw)
     o.set_conserved(E, *M, R); o.step(2)
-    s = Shasta(16, 7, 6, 0.1, 0.4, 4.0 / 3.0)
+    s = Shasta(16, 7, 6, 0.1, 0.4, gam, **kw)
     s.set_conserved(*[torch.from_numpy(a).cuda() for a in (E, *M, R)]); s.step(2)
     ref = dict(o.get_conserved()); ref.update(o.get_primitives())
     got = {k: v.cpu().numpy() for k, v in s.get_conserved().items()}
