@@ -115,3 +115,23 @@ def test_P13b_vacuum_threshold_of_reading_G7(oracle):
             G = 4.0 / 3.0
             v = 2 * Mabs / (G * E + np.sqrt(G * G * E * E - 4 * (G - 1) * Mabs * Mabs))
             assert abs(out[6] - v) <= 1e-12 * v
+
+
+def test_P7_fixed_point_cap_of_reading_G9(oracle):
+    # PAPER.md:109's fixed-point map v <- |M| / (E + P(v)) contracts with factor ~ (Gamma - 1) in a cell at the causality
+    # clamp (|M| = (1 - 1e-12) E, p = (Gamma-1) e).  The oracle stops at |dv| <= 1e-15 or after 200 iterations (reading G9):
+    # converged for the EOS of every config (Gamma <= 5/3) and up to Gamma = 1.8, NOT at Gamma = 1.9 (0.9^200 = 7e-10).
+    # DESIGN.md 3 (G9) states this range; GPU-vs-oracle parity is asserted inside it (test_lambda_and_gamma_range).
+    E, M = 1.0, 1.0 - 1e-12
+    for gamma, converged in ((4.0 / 3.0, True), (5.0 / 3.0, True), (1.8, True), (1.9, False)):
+        out, it, _ = oracle.cons2prim(E, M, 0.0, 0.0, 0.3, gamma)
+        lo, hi = 0.0, M / E
+        for _ in range(200):                                    # the root by bisection, independently
+            mid = 0.5 * (lo + hi)
+            if mid * (E + (gamma - 1.0) * (E - M * mid)) - M > 0.0:
+                hi = mid
+            else:
+                lo = mid
+        err = abs(out[6] - 0.5 * (lo + hi))
+        assert (err <= 1e-13) == converged, (gamma, err, it)
+        assert (it < 200) == converged, (gamma, it)
