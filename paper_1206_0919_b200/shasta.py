@@ -177,11 +177,11 @@ class Shasta:
         if boundary_z is not None:
             self.set_option(BOUNDARY_Z, boundary_z)
 
-    def close(self):
+    def close(self, _null=C.c_void_p):           # _null bound at definition: module globals may be gone when __del__ runs at exit
         if getattr(self, "_h", None) and self._h.value:
             self._views = {}
             self._L.shasta_destroy(self._h)
-            self._h = _vp()
+            self._h = _null()
 
     __del__ = close
 
