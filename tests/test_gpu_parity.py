@@ -615,6 +615,48 @@ def test_variant_explicit_antidiffusion_config1(oracle):
     parity.assert_parity(got, ref, TOL64, label="config1 explicit antidiffusion")
 
 
+# ------------------------------------------------------------------ the step / graph / deferral state machine
+def test_random_call_sequences_equal_plain_stepping():
+    # seeded random sequences of step(k), option changes (launch mode, deferral of the x-last primitives) and reads in between
+    # must land on the bits of one step at a time with no graph and no deferral: shasta_step's bookkeeping (cached graph
+    # cycles per phase, pending primitive output, buffer parity) may not leak into the results
+    import torch
+    from paper_1206_0919_b200 import shasta as sh
+    from paper_1206_0919_b200.shasta import Shasta
+    rng = np.random.default_rng(1234)
+    for trial in range(12):
+        shape = [(24, 20, 28), (64, 32, 16), (37, 19, 23)][trial % 3]
+        kw = dict(gamma=5.0 / 3.0, mass=1.0) if trial % 2 else {}
+        bc = [inputs.OUTFLOW, inputs.PERIODIC][(trial // 2) % 2]
+        c = inputs.random_state(*shape, seed=trial, kind="rough", boundary=bc, **kw)
+        st = [torch.from_numpy(c[k]).cuda() for k in ("e", "n", "vx", "vy", "vz")]
+        total = int(rng.integers(5, 20))
+        ref = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"], graph=0, no_defer=1)
+        ref.set_state(*st)
+        for _ in range(total):
+            ref.step(1)
+        want = {**ref.get_conserved(), **ref.get_primitives()}
+        a = Shasta(c["nx"], c["ny"], c["nz"], c["dx"], c["lam"], c["gamma"], c["boundary"], c["mass"])
+        a.set_state(*st)
+        done, log = 0, []
+        while done < total:
+            op = int(rng.integers(0, 6))
+            if op == 0:
+                g = int(rng.integers(0, 3)); a.set_option(sh.GRAPH, g); log.append(f"graph={g}")
+            elif op == 1:
+                nd = int(rng.integers(0, 2)); a.set_option(sh.NO_DEFER, nd); log.append(f"no_defer={nd}")
+            elif op == 2:
+                a.get_primitives(); log.append("prims")
+            elif op == 3:
+                a.get_conserved(); a.conserved_totals(); log.append("cons")
+            else:
+                k = int(min(rng.integers(1, 9), total - done)); a.step(k); done += k; log.append(f"step{k}")
+        got = {**a.get_conserved(), **a.get_primitives()}
+        assert a.step_index == total
+        for k in want:
+            assert torch.equal(got[k], want[k]), (trial, k, log)
+
+
 # ------------------------------------------------------------------ parameter range of shasta_create
 @pytest.mark.parametrize("lam", [0.5, 0.25, 0.05])
 @pytest.mark.parametrize("gamma", [1.2, 5.0 / 3.0, 1.8])
