@@ -186,3 +186,21 @@ def test_P17_energy_scale_homogeneity_bitwise(oracle):
             assert np.array_equal(got[f], base[f] * sc), (k, f)
         for f in ("R", "n", "vx", "vy", "vz"):
             assert np.array_equal(got[f], base[f]), (k, f)
+
+
+def test_thread_count_does_not_change_a_bit(oracle):
+    # OpenMP runs over independent pencils only: 1 thread and all threads give the same bits
+    import os
+    c = inputs.random_state(14, 9, 11, seed=8, kind="rough", gamma=5.0 / 3.0, mass=1.0, boundary=inputs.PERIODIC)
+    res = []
+    try:
+        for nt in (1, 3, os.cpu_count() or 1):
+            oracle.set_threads(nt)
+            o = _mk(oracle, c)
+            o.step(6)
+            res.append({**o.get_conserved(), **o.get_primitives(), "d": np.array(o.diagnostics())})
+    finally:
+        oracle.set_threads(os.cpu_count() or 1)
+    for r in res[1:]:
+        for k in res[0]:
+            assert np.array_equal(r[k], res[0][k]), k
