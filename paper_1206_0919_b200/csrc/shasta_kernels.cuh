@@ -330,7 +330,7 @@ __device__ __forceinline__ Prim cons2prim_general(const EosD& k, double E, doubl
             // the loop with (an idle lane may solve for garbage, a partner may need more steps) -- run-to-run reproducible
             const double dv = fabs(vn - v);
             if (!done) v = vn;
-            done = done || dv <= NEWT_DV;
+            done = done || !(dv > NEWT_DV);      // NaN (idle lane, garbage): done
             if (__all_sync(__activemask(), done)) break;
         }
         o.w = fmax(fma(-v, v, double(1)), double(0));
@@ -417,7 +417,7 @@ struct Newt {
         // shared-memory slot held) -- the same bits from run to run and for any segmentation of the march.  The loops vote on `done`.
         const double dv = fabs(vn - v);
         if (!done) v = vn;
-        done = done || dv <= NEWT_DV;
+        done = done || !(dv > NEWT_DV);          // a NaN step (an idle lane solving for garbage) counts as done: it must not hold the warp
     }
     // v_par = M_par v / |M| and p of the converged state (vacuum: 0, 0)
     __device__ __forceinline__ void finish(const EosD& k, double& vpar, double& p) const
